@@ -1,0 +1,151 @@
+/*
+ * bf.h -- C ABI of the B200-native coherent beamformer (arXiv 1412.4907 hot path).
+ *
+ * The operation (line numbers are /root/reference/PAPER.md):
+ *
+ *   W[c][b][n] = exp(-i 2 pi f_c/c0 (r_n . s_b))       steering factor e^{-i k0 . r_n} of Eq. 1
+ *                                                      (PAPER.md:23-28), k0 = (2 pi f_c/c0) s_b; the paper
+ *                                                      computes these coefficients on the host between
+ *                                                      iterations -- here a GPU kernel
+ *   y[c][b][t] = sum_n W[c][b][n] x[c][t][n]           per-channel N_b x N_a coefficient matrix times the
+ *                                                      antenna vector (Sec. 2.1; Algorithm 1,
+ *                                                      PAPER.md:66-98)
+ *   P[c][b][j] = sum_{t=j*nint}^{(j+1)*nint-1} |y|^2   "absolute power computation" fused into the kernel
+ *                                                      (PAPER.md:62), reduced on the GPU
+ *
+ * Weights are static between bf_set_geometry calls (the paper's assumption that "beam coefficients
+ * do not need to change within small time frames").  No normalisation is applied.
+ *
+ * Conventions
+ *   - plain C, no exceptions cross the ABI; every call returns a bf_status code (or NULL / 0);
+ *     bf_last_error(ctx) gives a human-readable message for the last failure on that context.
+ *   - "host" / "device" is stated for every pointer.  The caller owns every buffer it passes
+ *     (voltages, powers, workspaces); the context owns only its host-side state.
+ *   - bf_run only enqueues work on `stream` (a cudaStream_t passed as void*, NULL = default
+ *     stream) and returns without synchronising.
+ *   - one context per stream; a context is not thread-safe.
+ *   - there is NO CPU fallback: without an sm_100 device the compute calls fail with
+ *     BF_ECUDA / BF_EUNSUPPORTED.
+ */
+#ifndef BF_H_
+#define BF_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bf_ctx bf_ctx; /* opaque */
+
+enum bf_status {
+  BF_OK = 0,
+  BF_EINVAL = -1,       /* bad argument (NULL, non-positive size, nsamp % nint != 0, non-unit direction ...) */
+  BF_ENOGEOM = -2,      /* bf_run before bf_set_geometry / bf_set_workspace */
+  BF_ECUDA = -3,        /* a CUDA runtime call failed (message in bf_last_error) */
+  BF_EUNSUPPORTED = -4, /* device is not sm_100, or a forced kernel cannot run this shape */
+  BF_ENOMEM = -5        /* workspace too small / host allocation failed */
+};
+
+enum bf_dtype {
+  BF_CI8 = 0, /* complex int8, interleaved (re, im): 2 bytes per antenna-sample (BASELINE.json configs) */
+  BF_CF16 = 1 /* complex IEEE fp16, interleaved (re, im): 4 bytes per antenna-sample */
+};
+
+enum bf_kernel {
+  BF_KERNEL_AUTO = 0, /* pick the fastest kernel that supports the shape */
+  BF_KERNEL_SIMT = 1, /* generic fp32 CUDA-core kernel (any shape; Algorithm 1's structure) */
+  BF_KERNEL_UMMA = 2  /* tcgen05/TMEM tensor-core kernel with the fused |.|^2 + integrate epilogue */
+};
+
+/*
+ * Create a context for nant antennas, nchan channels, nbeam beams, nsamp time samples per channel
+ * per bf_run call and an integration length of nint samples (output has nsamp/nint time bins).
+ * Pure host call (no CUDA).  Returns NULL if any size is <= 0 or nsamp % nint != 0.
+ * The voltage element type defaults to BF_CI8.
+ */
+bf_ctx *bf_create(int nant, int nchan, int nbeam, int nsamp, int nint);
+
+/* Free the context (host state only; caller-owned device memory is untouched).  NULL is allowed. */
+void bf_destroy(bf_ctx *ctx);
+
+/* Select the voltage element type (enum bf_dtype).  Call before bf_workspace_bytes. */
+int bf_set_dtype(bf_ctx *ctx, int dtype);
+
+/* Force a kernel (enum bf_kernel); default BF_KERNEL_AUTO.  BF_EUNSUPPORTED is reported by bf_run
+ * if the forced kernel cannot run the context's shape. */
+int bf_set_kernel(bf_ctx *ctx, int kernel);
+
+/* Which kernel bf_run will launch for this context (enum bf_kernel value, never AUTO). */
+int bf_selected_kernel(const bf_ctx *ctx);
+
+/* Number of kernels this context has launched so far (all streams), for accounting. */
+long long bf_launch_count(const bf_ctx *ctx);
+
+/*
+ * Device workspace: geometry copy + the weight operand.  The caller allocates `bytes` >=
+ * bf_workspace_bytes(ctx) of DEVICE memory, 1024-byte aligned, and keeps it alive while the
+ * context is used.  Returns BF_EINVAL on NULL / misaligned pointer, BF_ENOMEM if too small.
+ */
+size_t bf_workspace_bytes(const bf_ctx *ctx);
+int bf_set_workspace(bf_ctx *ctx, void *dev_ptr, size_t bytes);
+
+/*
+ * Set the array geometry and (re)generate the phase weights on the device (kernel on `stream`):
+ *   ant_xyz_m    HOST fp64 [nant][3]   antenna positions r_n in metres
+ *   chan_freq_hz HOST fp64 [nchan]     channel centre frequencies f_c in Hz
+ *   beam_dir     HOST fp64 [nbeam][3]  unit vectors s_b in the same frame as ant_xyz_m
+ * W = exp(-i 2 pi f_c/c0 (r_n . s_b)); the phase is computed and range-reduced in fp64, then rounded
+ * to the tensor-core operand type (fp16).  The arrays are copied before the call returns.
+ * BF_EINVAL: NULL, non-finite values, | |s_b| - 1 | > 1e-6, f_c <= 0.  BF_ENOGEOM: no workspace yet.
+ */
+int bf_set_geometry(bf_ctx *ctx, const double *ant_xyz_m, const double *chan_freq_hz,
+                    const double *beam_dir, void *stream);
+
+/*
+ * Copy the generated weights back as fp32 (re, im) pairs, HOST [nchan][nbeam][nant][2] -- the values
+ * the kernels actually use (after rounding to the operand type).  Synchronises `stream`.
+ */
+int bf_get_weights(bf_ctx *ctx, float *host_out, void *stream);
+
+/*
+ * The hot path.  voltages: DEVICE, [nchan][nsamp][nant][2] (re, im interleaved) of the context's
+ * dtype, 16-byte aligned.  powers: DEVICE fp32 [nchan][nbeam][nsamp/nint], fully overwritten.
+ * Enqueues on `stream` and returns.  BF_ENOGEOM before bf_set_geometry.
+ */
+int bf_run(bf_ctx *ctx, const void *voltages, float *powers, void *stream);
+
+/*
+ * End-to-end variant with HOST buffers (the paper's PCIe concern: "this data overhead
+ * can essentially be masked by using two CUDA streams ... however this would also require additional
+ * global memory").  The nchan channels are cut into chunks of `chan_per_chunk` channels; chunk k+1 is
+ * copied host->device on `copy_stream` while chunk k is beamformed on `compute_stream`, and each chunk's
+ * powers are copied back device->host behind its kernel.
+ *   host_voltages  HOST (pinned for overlap; pageable works but serialises), same layout as bf_run
+ *   host_powers    HOST fp32 [nchan][nbeam][nsamp/nint]
+ *   staging        DEVICE scratch of >= bf_staging_bytes(ctx, chan_per_chunk) bytes, 1024-byte aligned
+ * Returns after enqueuing; synchronise both streams before reading host_powers.
+ */
+size_t bf_staging_bytes(const bf_ctx *ctx, int chan_per_chunk);
+int bf_run_host(bf_ctx *ctx, const void *host_voltages, float *host_powers, void *staging,
+                size_t staging_bytes, int chan_per_chunk, void *compute_stream, void *copy_stream);
+
+/*
+ * Streaming mode: `nblocks` consecutive input blocks, each one bf_run input, in (pinned) HOST memory
+ * at host_blocks[i]; powers: DEVICE fp32, nblocks outputs back to back.  Block i+1 is copied on
+ * `copy_stream` into one of two staging buffers while block i runs on `compute_stream`
+ * (PAPER.md:140).  staging: DEVICE scratch of >= 2 * (one bf_run input) bytes.
+ */
+int bf_run_streaming(bf_ctx *ctx, const void *const *host_blocks, int nblocks, float *powers,
+                     void *staging, size_t staging_bytes, void *compute_stream, void *copy_stream);
+
+/* Message for the last error on this context ("" if none).  Valid until the next call on ctx. */
+const char *bf_last_error(const bf_ctx *ctx);
+
+/* Library version string. */
+const char *bf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BF_H_ */

@@ -1,0 +1,263 @@
+"""paper_1412_4907_b200 -- thin Python binding over the C-ABI beamformer library (include/bf.h).
+
+Argument marshalling only: every step of the hot path (weights, ingest, contraction, |.|^2,
+integration) runs in the CUDA kernels under ``csrc/``.  PyTorch is used by callers for device
+memory and streams; this module itself needs only ctypes.  There is no CPU fallback: if
+``libbf.so`` has not been built (``python -m paper_1412_4907_b200.build``) loading fails loudly.
+
+The functions carry the same names as the C entry points (bf_create, bf_set_geometry, bf_run ...).
+``Beamformer`` is a small convenience wrapper that owns the context and a torch workspace.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libbf.so")
+
+BF_OK, BF_EINVAL, BF_ENOGEOM, BF_ECUDA, BF_EUNSUPPORTED, BF_ENOMEM = 0, -1, -2, -3, -4, -5
+BF_CI8, BF_CF16 = 0, 1
+BF_KERNEL_AUTO, BF_KERNEL_SIMT, BF_KERNEL_UMMA = 0, 1, 2
+
+# every symbol include/bf.h declares: name -> (restype, argtypes)
+_vp, _i, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
+_dp = ctypes.POINTER(ctypes.c_double)
+SYMBOLS = {
+    "bf_create": (_vp, [_i, _i, _i, _i, _i]),
+    "bf_destroy": (None, [_vp]),
+    "bf_set_dtype": (_i, [_vp, _i]),
+    "bf_set_kernel": (_i, [_vp, _i]),
+    "bf_selected_kernel": (_i, [_vp]),
+    "bf_launch_count": (ctypes.c_longlong, [_vp]),
+    "bf_workspace_bytes": (_sz, [_vp]),
+    "bf_set_workspace": (_i, [_vp, _vp, _sz]),
+    "bf_set_geometry": (_i, [_vp, _dp, _dp, _dp, _vp]),
+    "bf_get_weights": (_i, [_vp, _vp, _vp]),
+    "bf_run": (_i, [_vp, _vp, _vp, _vp]),
+    "bf_staging_bytes": (_sz, [_vp, _i]),
+    "bf_run_host": (_i, [_vp, _vp, _vp, _vp, _sz, _i, _vp, _vp]),
+    "bf_run_streaming": (_i, [_vp, ctypes.POINTER(_vp), _i, _vp, _vp, _sz, _vp, _vp]),
+    "bf_last_error": (ctypes.c_char_p, [_vp]),
+    "bf_version": (ctypes.c_char_p, []),
+}
+
+_lib = None
+
+
+class BfError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"bf error {code}: {msg}")
+        self.code = code
+
+
+def lib() -> ctypes.CDLL:
+    """Load libbf.so (built in-tree).  Fails loudly if it is missing -- there is no fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_1412_4907_b200.build`")
+        L = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+def _ptr(x):
+    """Raw address of a torch tensor / numpy array / int / None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if hasattr(x, "ctypes"):
+        return x.ctypes.data
+    raise TypeError(type(x))
+
+
+def _stream(s):
+    if s is None:
+        return None
+    return s.cuda_stream if hasattr(s, "cuda_stream") else int(s)
+
+
+# ---- same-name wrappers (marshalling only) ---------------------------------------------------
+def bf_create(nant, nchan, nbeam, nsamp, nint):
+    return lib().bf_create(int(nant), int(nchan), int(nbeam), int(nsamp), int(nint))
+
+
+def bf_destroy(ctx):
+    lib().bf_destroy(ctx)
+
+
+def bf_set_dtype(ctx, dtype):
+    return lib().bf_set_dtype(ctx, int(dtype))
+
+
+def bf_set_kernel(ctx, kernel):
+    return lib().bf_set_kernel(ctx, int(kernel))
+
+
+def bf_selected_kernel(ctx):
+    return lib().bf_selected_kernel(ctx)
+
+
+def bf_launch_count(ctx):
+    return int(lib().bf_launch_count(ctx))
+
+
+def bf_workspace_bytes(ctx):
+    return int(lib().bf_workspace_bytes(ctx))
+
+
+def bf_set_workspace(ctx, dev_ptr, nbytes):
+    return lib().bf_set_workspace(ctx, _ptr(dev_ptr), int(nbytes))
+
+
+def bf_set_geometry(ctx, ant_xyz_m, chan_freq_hz, beam_dir, stream=None):
+    import numpy as np
+
+    def dp(a):
+        if a is None:
+            return None, None
+        a = np.ascontiguousarray(a, dtype=np.float64)
+        return a, a.ctypes.data_as(_dp)
+    a, pa = dp(ant_xyz_m)
+    f, pf = dp(chan_freq_hz)
+    d, pd = dp(beam_dir)
+    return lib().bf_set_geometry(ctx, pa, pf, pd, _stream(stream))
+
+
+def bf_get_weights(ctx, host_out, stream=None):
+    return lib().bf_get_weights(ctx, _ptr(host_out), _stream(stream))
+
+
+def bf_run(ctx, voltages, powers, stream=None):
+    return lib().bf_run(ctx, _ptr(voltages), _ptr(powers), _stream(stream))
+
+
+def bf_staging_bytes(ctx, chan_per_chunk):
+    return int(lib().bf_staging_bytes(ctx, int(chan_per_chunk)))
+
+
+def bf_run_host(ctx, host_voltages, host_powers, staging, staging_bytes, chan_per_chunk, compute_stream=None,
+                copy_stream=None):
+    return lib().bf_run_host(ctx, _ptr(host_voltages), _ptr(host_powers), _ptr(staging), int(staging_bytes),
+                             int(chan_per_chunk), _stream(compute_stream), _stream(copy_stream))
+
+
+def bf_run_streaming(ctx, host_blocks, powers, staging, staging_bytes, compute_stream=None, copy_stream=None):
+    n = len(host_blocks)
+    arr = (_vp * n)(*[_ptr(b) for b in host_blocks])
+    return lib().bf_run_streaming(ctx, arr, n, _ptr(powers), _ptr(staging), int(staging_bytes),
+                                  _stream(compute_stream), _stream(copy_stream))
+
+
+def bf_last_error(ctx):
+    s = lib().bf_last_error(ctx)
+    return s.decode() if s else ""
+
+
+def bf_version():
+    return lib().bf_version().decode()
+
+
+# ---- convenience wrapper ---------------------------------------------------------------------
+class Beamformer:
+    """Owns a bf_ctx plus its device workspace (a torch uint8 tensor)."""
+
+    def __init__(self, nant, nchan, nbeam, nsamp, nint, dtype=BF_CI8, kernel=BF_KERNEL_AUTO, device="cuda:0"):
+        import torch
+
+        self.shape = (nant, nchan, nbeam, nsamp, nint)
+        self.ctx = bf_create(nant, nchan, nbeam, nsamp, nint)
+        if not self.ctx:
+            raise BfError(BF_EINVAL, "bf_create rejected the sizes (all > 0, nsamp % nint == 0)")
+        self._check(bf_set_dtype(self.ctx, dtype))
+        self._check(bf_set_kernel(self.ctx, kernel))
+        self.dtype = dtype
+        self.device = torch.device(device)
+        nbytes = bf_workspace_bytes(self.ctx)
+        self.workspace = torch.empty(nbytes + 1024, dtype=torch.uint8, device=self.device)
+        off = (-self.workspace.data_ptr()) % 1024
+        self._check(bf_set_workspace(self.ctx, self.workspace.data_ptr() + off, nbytes))
+        self._staging = None
+
+    def _check(self, rc):
+        if rc != BF_OK:
+            raise BfError(rc, bf_last_error(self.ctx))
+
+    @property
+    def nbin(self):
+        return self.shape[3] // self.shape[4]
+
+    def set_geometry(self, ant_xyz_m, chan_freq_hz, beam_dir, stream=None):
+        self._check(bf_set_geometry(self.ctx, ant_xyz_m, chan_freq_hz, beam_dir, stream))
+
+    def weights(self):
+        import numpy as np
+
+        nant, nchan, nbeam = self.shape[:3]
+        out = np.empty((nchan, nbeam, nant, 2), dtype=np.float32)
+        self._check(bf_get_weights(self.ctx, out))
+        return out[..., 0] + 1j * out[..., 1]
+
+    def empty_powers(self):
+        import torch
+
+        nant, nchan, nbeam, nsamp, nint = self.shape
+        return torch.empty((nchan, nbeam, nsamp // nint), dtype=torch.float32, device=self.device)
+
+    def run(self, voltages, powers=None, stream=None):
+        import torch
+
+        if powers is None:
+            powers = self.empty_powers()
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        self._check(bf_run(self.ctx, voltages, powers, stream))
+        return powers
+
+    def _get_staging(self, nbytes):
+        import torch
+
+        if self._staging is None or self._staging.numel() < nbytes + 1024:
+            self._staging = torch.empty(nbytes + 1024, dtype=torch.uint8, device=self.device)
+        off = (-self._staging.data_ptr()) % 1024
+        return self._staging.data_ptr() + off
+
+    def run_host(self, host_voltages, host_powers, chan_per_chunk, compute_stream, copy_stream):
+        nbytes = bf_staging_bytes(self.ctx, chan_per_chunk)
+        st = self._get_staging(nbytes)
+        self._check(bf_run_host(self.ctx, host_voltages, host_powers, st, nbytes, chan_per_chunk, compute_stream,
+                                copy_stream))
+
+    def run_streaming(self, host_blocks, powers, compute_stream, copy_stream):
+        nant, nchan, nbeam, nsamp, nint = self.shape
+        in_bytes = nchan * nsamp * nant * (2 if self.dtype == BF_CI8 else 4)
+        nbytes = 2 * ((in_bytes + 1023) // 1024 * 1024)
+        st = self._get_staging(nbytes)
+        self._check(bf_run_streaming(self.ctx, host_blocks, powers, st, nbytes, compute_stream, copy_stream))
+
+    @property
+    def selected_kernel(self):
+        return bf_selected_kernel(self.ctx)
+
+    @property
+    def launches(self):
+        return bf_launch_count(self.ctx)
+
+    def close(self):
+        if self.ctx:
+            bf_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,302 @@
+// bf_api.cu -- the C-ABI boundary (include/bf.h): context, validation, workspace, dispatch.
+// Problem statement: PAPER.md:56-64; static weights per buffer: PAPER.md:64, 100; host<->device
+// overlap with two streams: PAPER.md:140.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "bf_internal.h"
+
+#define BF_ALIGN 1024
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+static int fail(bf_ctx *c, int code, const char *fmt, ...) {
+  if (c) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(c->err, sizeof(c->err), fmt, ap);
+    va_end(ap);
+  }
+  return code;
+}
+static int cuda_fail(bf_ctx *c, cudaError_t e, const char *what) {
+  return fail(c, BF_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+size_t bf_in_bytes_per_chan(const bf_ctx *c) {
+  return (size_t)c->nsamp * c->nant * (c->dtype == BF_CI8 ? 2 : 4);
+}
+size_t bf_wop_bytes_per_chan(const bf_ctx *c) {
+  return (size_t)c->nMt * c->nKb * BF_TILE_ROWS * BF_KBLOCK * sizeof(__half);
+}
+static size_t geom_bytes(const bf_ctx *c) {
+  return align_up(sizeof(double) * (3 * (size_t)c->nant + c->nchan + 3 * (size_t)c->nbeam), BF_ALIGN);
+}
+
+extern "C" const char *bf_version(void) { return "paper_1412_4907_b200 0.1 (sm_100a)"; }
+
+extern "C" bf_ctx *bf_create(int nant, int nchan, int nbeam, int nsamp, int nint) {
+  if (nant <= 0 || nchan <= 0 || nbeam <= 0 || nsamp <= 0 || nint <= 0) return nullptr;
+  if (nsamp % nint != 0) return nullptr;  // DESIGN.md reading A8
+  if ((long long)nchan * nbeam > (1LL << 40)) return nullptr;
+  bf_ctx *c = new (std::nothrow) bf_ctx();
+  if (!c) return nullptr;
+  c->nant = nant; c->nchan = nchan; c->nbeam = nbeam; c->nsamp = nsamp; c->nint = nint;
+  c->nbin = nsamp / nint;
+  c->dtype = BF_CI8;
+  c->kernel_forced = BF_KERNEL_AUTO;
+  c->nMt = (nbeam + BF_TILE_BEAMS - 1) / BF_TILE_BEAMS;
+  c->nKb = (2 * nant + BF_KBLOCK - 1) / BF_KBLOCK;
+  c->ws = nullptr; c->ws_bytes = 0;
+  c->d_ant = c->d_freq = c->d_dir = nullptr; c->d_wop = nullptr;
+  c->have_geom = false;
+  c->launches = 0;
+  c->sm_count = 0; c->device_ok = -1;
+  c->have_events = false;
+  c->err[0] = 0;
+  return c;
+}
+
+extern "C" void bf_destroy(bf_ctx *c) {
+  if (!c) return;
+  if (c->have_events)
+    for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_copied[i]); cudaEventDestroy(c->ev_done[i]); }
+  delete c;
+}
+
+extern "C" const char *bf_last_error(const bf_ctx *c) { return c ? c->err : "null context"; }
+
+extern "C" int bf_set_dtype(bf_ctx *c, int dtype) {
+  if (!c) return BF_EINVAL;
+  if (dtype != BF_CI8 && dtype != BF_CF16) return fail(c, BF_EINVAL, "unknown dtype %d", dtype);
+  c->dtype = dtype;
+  return BF_OK;
+}
+
+extern "C" int bf_set_kernel(bf_ctx *c, int kernel) {
+  if (!c) return BF_EINVAL;
+  if (kernel != BF_KERNEL_AUTO && kernel != BF_KERNEL_SIMT && kernel != BF_KERNEL_UMMA)
+    return fail(c, BF_EINVAL, "unknown kernel %d", kernel);
+  c->kernel_forced = kernel;
+  return BF_OK;
+}
+
+extern "C" int bf_selected_kernel(const bf_ctx *c) {
+  if (!c) return BF_EINVAL;
+  if (c->kernel_forced != BF_KERNEL_AUTO) return c->kernel_forced;
+  const char *why;
+  return bf_umma_supported(c, &why) ? BF_KERNEL_UMMA : BF_KERNEL_SIMT;
+}
+
+extern "C" long long bf_launch_count(const bf_ctx *c) { return c ? c->launches : 0; }
+
+extern "C" size_t bf_workspace_bytes(const bf_ctx *c) {
+  if (!c) return 0;
+  return geom_bytes(c) + align_up((size_t)c->nchan * bf_wop_bytes_per_chan(c), BF_ALIGN);
+}
+
+// no fallback: the device must be Blackwell (compute capability 10.x)
+static int probe_device(bf_ctx *c) {
+  if (c->device_ok == 1) return BF_OK;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return cuda_fail(c, e, "cudaGetDevice");
+  int major = 0, sms = 0;
+  e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (e != cudaSuccess) return cuda_fail(c, e, "cudaDeviceGetAttribute");
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (major != 10) {
+    c->device_ok = 0;
+    return fail(c, BF_EUNSUPPORTED, "device compute capability %d.x is not sm_100 (no fallback)", major);
+  }
+  c->sm_count = sms;
+  c->device_ok = 1;
+  return BF_OK;
+}
+
+extern "C" int bf_set_workspace(bf_ctx *c, void *dev_ptr, size_t bytes) {
+  if (!c) return BF_EINVAL;
+  if (!dev_ptr) return fail(c, BF_EINVAL, "workspace pointer is NULL");
+  if (((uintptr_t)dev_ptr) % BF_ALIGN) return fail(c, BF_EINVAL, "workspace must be %d-byte aligned", BF_ALIGN);
+  if (bytes < bf_workspace_bytes(c))
+    return fail(c, BF_ENOMEM, "workspace too small: %zu < %zu", bytes, bf_workspace_bytes(c));
+  c->ws = dev_ptr;
+  c->ws_bytes = bytes;
+  char *p = (char *)dev_ptr;
+  c->d_ant = (double *)p;
+  c->d_freq = c->d_ant + 3 * (size_t)c->nant;
+  c->d_dir = c->d_freq + c->nchan;
+  c->d_wop = (__half *)(p + geom_bytes(c));
+  c->have_geom = false;
+  return BF_OK;
+}
+
+extern "C" int bf_set_geometry(bf_ctx *c, const double *ant, const double *freq, const double *dir, void *stream) {
+  if (!c) return BF_EINVAL;
+  if (!ant || !freq || !dir) return fail(c, BF_EINVAL, "geometry pointer is NULL");
+  for (int i = 0; i < 3 * c->nant; ++i)
+    if (!isfinite(ant[i])) return fail(c, BF_EINVAL, "antenna position %d is not finite", i / 3);
+  for (int i = 0; i < c->nchan; ++i)
+    if (!isfinite(freq[i]) || freq[i] <= 0.0) return fail(c, BF_EINVAL, "channel frequency %d is not positive/finite", i);
+  for (int b = 0; b < c->nbeam; ++b) {
+    double n2 = dir[3 * b] * dir[3 * b] + dir[3 * b + 1] * dir[3 * b + 1] + dir[3 * b + 2] * dir[3 * b + 2];
+    if (!isfinite(n2) || fabs(sqrt(n2) - 1.0) > 1e-6) return fail(c, BF_EINVAL, "beam direction %d is not a unit vector", b);
+  }
+  if (!c->ws) return fail(c, BF_ENOGEOM, "bf_set_workspace must be called before bf_set_geometry");
+  int rc = probe_device(c);
+  if (rc != BF_OK) return rc;
+  size_t na = 3 * (size_t)c->nant, nf = c->nchan, nd = 3 * (size_t)c->nbeam;
+  c->h_geom.resize(na + nf + nd);
+  memcpy(c->h_geom.data(), ant, na * sizeof(double));
+  memcpy(c->h_geom.data() + na, freq, nf * sizeof(double));
+  memcpy(c->h_geom.data() + na + nf, dir, nd * sizeof(double));
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e = cudaMemcpyAsync(c->d_ant, c->h_geom.data(), (na + nf + nd) * sizeof(double), cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) return cuda_fail(c, e, "geometry H2D copy");
+  e = bf_launch_weights(c, st);
+  if (e != cudaSuccess) return cuda_fail(c, e, "weight generator launch");
+  c->launches += 1;
+  c->have_geom = true;
+  return BF_OK;
+}
+
+extern "C" int bf_get_weights(bf_ctx *c, float *host_out, void *stream) {
+  if (!c) return BF_EINVAL;
+  if (!host_out) return fail(c, BF_EINVAL, "output pointer is NULL");
+  if (!c->have_geom) return fail(c, BF_ENOGEOM, "no geometry set");
+  cudaStream_t st = (cudaStream_t)stream;
+  size_t bytes = (size_t)c->nchan * c->nbeam * c->nant * 2 * sizeof(float);
+  float *d = nullptr;  // verification helper: the one place the library allocates device memory itself
+  cudaError_t e = cudaMalloc(&d, bytes);
+  if (e != cudaSuccess) return cuda_fail(c, e, "cudaMalloc (bf_get_weights)");
+  e = bf_launch_decode_weights(c, d, st);
+  if (e == cudaSuccess) { c->launches += 1; e = cudaMemcpyAsync(host_out, d, bytes, cudaMemcpyDeviceToHost, st); }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(d);
+  if (e != cudaSuccess) return cuda_fail(c, e, "bf_get_weights");
+  return BF_OK;
+}
+
+// launch the selected kernel over channels [chan0, chan0 + nchan_run)
+static int launch_range(bf_ctx *c, const void *volt, float *pow, int chan0, int nchan_run, cudaStream_t st) {
+  BfParams p;
+  p.nant = c->nant; p.nbeam = c->nbeam; p.nsamp = c->nsamp; p.nint = c->nint; p.nbin = c->nbin;
+  p.nMt = c->nMt; p.nKb = c->nKb;
+  p.nchan_run = nchan_run;
+  p.volt = volt; p.pow = pow;
+  p.wop = c->d_wop + (size_t)chan0 * (bf_wop_bytes_per_chan(c) / sizeof(__half));
+  int k = c->kernel_forced;
+  const char *why = "";
+  bool umma_ok = bf_umma_supported(c, &why);
+  if (k == BF_KERNEL_AUTO) k = umma_ok ? BF_KERNEL_UMMA : BF_KERNEL_SIMT;
+  if (k == BF_KERNEL_UMMA && !umma_ok) return fail(c, BF_EUNSUPPORTED, "tensor-core kernel cannot run this shape: %s", why);
+  cudaError_t e = (k == BF_KERNEL_UMMA) ? bf_launch_umma(p, c->dtype, c->sm_count, st) : bf_launch_simt(p, c->dtype, st);
+  if (e != cudaSuccess) return cuda_fail(c, e, k == BF_KERNEL_UMMA ? "tensor-core kernel launch" : "SIMT kernel launch");
+  c->launches += 1;
+  return BF_OK;
+}
+
+static int check_run(bf_ctx *c, const void *volt, const void *pow) {
+  if (!c) return BF_EINVAL;
+  if (!volt || !pow) return fail(c, BF_EINVAL, "voltages / powers pointer is NULL");
+  if (!c->have_geom) return fail(c, BF_ENOGEOM, "bf_set_geometry has not been called");
+  return probe_device(c);
+}
+
+extern "C" int bf_run(bf_ctx *c, const void *voltages, float *powers, void *stream) {
+  int rc = check_run(c, voltages, powers);
+  if (rc != BF_OK) return rc;
+  if (((uintptr_t)voltages) % 16) return fail(c, BF_EINVAL, "voltages must be 16-byte aligned");
+  return launch_range(c, voltages, powers, 0, c->nchan, (cudaStream_t)stream);
+}
+
+static int ensure_events(bf_ctx *c) {
+  if (c->have_events) return BF_OK;
+  for (int i = 0; i < 2; ++i) {
+    cudaError_t e = cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventCreate");
+  }
+  c->have_events = true;
+  return BF_OK;
+}
+
+extern "C" size_t bf_staging_bytes(const bf_ctx *c, int chan_per_chunk) {
+  if (!c || chan_per_chunk <= 0) return 0;
+  if (chan_per_chunk > c->nchan) chan_per_chunk = c->nchan;
+  size_t in = align_up((size_t)chan_per_chunk * bf_in_bytes_per_chan(c), BF_ALIGN);
+  size_t out = align_up((size_t)chan_per_chunk * c->nbeam * c->nbin * sizeof(float), BF_ALIGN);
+  return 2 * (in + out);
+}
+
+extern "C" int bf_run_host(bf_ctx *c, const void *host_volt, float *host_pow, void *staging, size_t staging_bytes,
+                           int chan_per_chunk, void *compute_stream, void *copy_stream) {
+  int rc = check_run(c, host_volt, host_pow);
+  if (rc != BF_OK) return rc;
+  if (chan_per_chunk <= 0) return fail(c, BF_EINVAL, "chan_per_chunk must be positive");
+  if (chan_per_chunk > c->nchan) chan_per_chunk = c->nchan;
+  if (!staging || ((uintptr_t)staging) % BF_ALIGN) return fail(c, BF_EINVAL, "staging must be a %d-byte aligned device pointer", BF_ALIGN);
+  if (staging_bytes < bf_staging_bytes(c, chan_per_chunk)) return fail(c, BF_ENOMEM, "staging too small");
+  if ((rc = ensure_events(c)) != BF_OK) return rc;
+  cudaStream_t cs = (cudaStream_t)compute_stream, xs = (cudaStream_t)copy_stream;
+  const size_t in_chan = bf_in_bytes_per_chan(c), out_chan = (size_t)c->nbeam * c->nbin * sizeof(float);
+  const size_t in_buf = align_up((size_t)chan_per_chunk * in_chan, BF_ALIGN);
+  const size_t out_buf = align_up((size_t)chan_per_chunk * out_chan, BF_ALIGN);
+  char *in[2] = {(char *)staging, (char *)staging + in_buf};
+  char *out[2] = {(char *)staging + 2 * in_buf, (char *)staging + 2 * in_buf + out_buf};
+  cudaError_t e;
+  int k = 0;
+  for (int c0 = 0; c0 < c->nchan; c0 += chan_per_chunk, ++k) {
+    int n = c->nchan - c0 < chan_per_chunk ? c->nchan - c0 : chan_per_chunk;
+    int b = k & 1;
+    // staging half b is free once the kernel + D2H that used it two chunks ago are done
+    if (k >= 2 && (e = cudaStreamWaitEvent(xs, c->ev_done[b], 0)) != cudaSuccess) return cuda_fail(c, e, "cudaStreamWaitEvent");
+    e = cudaMemcpyAsync(in[b], (const char *)host_volt + (size_t)c0 * in_chan, (size_t)n * in_chan, cudaMemcpyHostToDevice, xs);
+    if (e != cudaSuccess) return cuda_fail(c, e, "voltage H2D copy");
+    cudaEventRecord(c->ev_copied[b], xs);
+    cudaStreamWaitEvent(cs, c->ev_copied[b], 0);
+    if ((rc = launch_range(c, in[b], (float *)out[b], c0, n, cs)) != BF_OK) return rc;
+    e = cudaMemcpyAsync((char *)host_pow + (size_t)c0 * out_chan, out[b], (size_t)n * out_chan, cudaMemcpyDeviceToHost, cs);
+    if (e != cudaSuccess) return cuda_fail(c, e, "power D2H copy");
+    cudaEventRecord(c->ev_done[b], cs);
+  }
+  // the next call on this context must not overwrite staging that is still in flight
+  cudaStreamWaitEvent(xs, c->ev_done[0], 0);
+  if (k > 1) cudaStreamWaitEvent(xs, c->ev_done[1], 0);
+  return BF_OK;
+}
+
+extern "C" int bf_run_streaming(bf_ctx *c, const void *const *host_blocks, int nblocks, float *powers, void *staging,
+                                size_t staging_bytes, void *compute_stream, void *copy_stream) {
+  int rc = check_run(c, host_blocks, powers);
+  if (rc != BF_OK) return rc;
+  if (nblocks <= 0) return fail(c, BF_EINVAL, "nblocks must be positive");
+  for (int i = 0; i < nblocks; ++i)
+    if (!host_blocks[i]) return fail(c, BF_EINVAL, "host block %d is NULL", i);
+  const size_t in_bytes = (size_t)c->nchan * bf_in_bytes_per_chan(c);
+  const size_t in_buf = align_up(in_bytes, BF_ALIGN);
+  if (!staging || ((uintptr_t)staging) % BF_ALIGN) return fail(c, BF_EINVAL, "staging must be a %d-byte aligned device pointer", BF_ALIGN);
+  if (staging_bytes < 2 * in_buf) return fail(c, BF_ENOMEM, "staging too small: need %zu", 2 * in_buf);
+  if ((rc = ensure_events(c)) != BF_OK) return rc;
+  cudaStream_t cs = (cudaStream_t)compute_stream, xs = (cudaStream_t)copy_stream;
+  const size_t out_elems = (size_t)c->nchan * c->nbeam * c->nbin;
+  char *in[2] = {(char *)staging, (char *)staging + in_buf};
+  cudaError_t e;
+  for (int i = 0; i < nblocks; ++i) {
+    int b = i & 1;
+    if (i >= 2 && (e = cudaStreamWaitEvent(xs, c->ev_done[b], 0)) != cudaSuccess) return cuda_fail(c, e, "cudaStreamWaitEvent");
+    e = cudaMemcpyAsync(in[b], host_blocks[i], in_bytes, cudaMemcpyHostToDevice, xs);
+    if (e != cudaSuccess) return cuda_fail(c, e, "block H2D copy");
+    cudaEventRecord(c->ev_copied[b], xs);
+    cudaStreamWaitEvent(cs, c->ev_copied[b], 0);
+    if ((rc = launch_range(c, in[b], powers + (size_t)i * out_elems, 0, c->nchan, cs)) != BF_OK) return rc;
+    cudaEventRecord(c->ev_done[b], cs);
+  }
+  cudaStreamWaitEvent(xs, c->ev_done[0], 0);
+  if (nblocks > 1) cudaStreamWaitEvent(xs, c->ev_done[1], 0);
+  return BF_OK;
+}

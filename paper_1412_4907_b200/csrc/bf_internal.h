@@ -1,0 +1,65 @@
+// bf_internal.h -- shared declarations of the CUDA path (not part of the public ABI).
+#pragma once
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/bf.h"
+
+// ---- weight operand layout -------------------------------------------
+// The complex contraction y = W x is run as a REAL contraction over k' = 2n + {0,1} against the
+// interleaved (re, im) voltages:
+//   row "re" of beam b:  A[2n] =  W_re, A[2n+1] = -W_im   ->  sum_k' A x' = Re y
+//   row "im" of beam b:  A[2n] =  W_im, A[2n+1] =  W_re   ->  sum_k' A x' = Im y
+// Rows are grouped in M-tiles of 128 rows = 64 beams.  Inside a tile, row r = 32 q + l holds
+// beam 64 mt + 16 q + (l & 15), part (l >> 4) (0 = re, 1 = im): a warp that owns TMEM lanes
+// 32q..32q+31 finds re and im of one beam 16 lanes apart (one shuffle per OUTPUT bin, not per sample).
+// K' is padded to a multiple of 64 (zeros).  Memory: fp16 [chan][mt][kb][128 rows][64 k'] -- every
+// (chan, mt, kb) block is one contiguous 16 KiB K-major tile.
+#define BF_TILE_ROWS 128
+#define BF_TILE_BEAMS 64
+#define BF_KBLOCK 64
+
+__host__ __device__ inline int bf_row_beam(int mt, int r) { return mt * BF_TILE_BEAMS + ((r >> 5) << 4) + (r & 15); }
+__host__ __device__ inline int bf_row_part(int r) { return (r >> 4) & 1; }
+// row of (beam-in-tile bl, part)
+__host__ __device__ inline int bf_beam_row(int bl, int part) { return ((bl >> 4) << 5) + (part << 4) + (bl & 15); }
+
+struct BfParams {
+  int nant, nbeam, nsamp, nint, nbin;
+  int nMt, nKb;
+  int nchan_run;        // channels processed by this launch
+  const void *volt;     // device, first channel of this launch
+  float *pow;           // device, first channel of this launch
+  const __half *wop;    // device, weight operand of the first channel of this launch
+};
+
+struct bf_ctx {
+  int nant, nchan, nbeam, nsamp, nint, nbin;
+  int dtype, kernel_forced;
+  int nMt, nKb;
+  void *ws;
+  size_t ws_bytes;
+  double *d_ant, *d_freq, *d_dir;
+  __half *d_wop;
+  bool have_geom;
+  std::vector<double> h_geom;
+  long long launches;
+  int sm_count;     // 0 = device not probed yet
+  int device_ok;    // -1 unknown, 0 no, 1 yes
+  cudaEvent_t ev_copied[2], ev_done[2];
+  bool have_events;
+  char err[512];
+};
+
+size_t bf_in_bytes_per_chan(const bf_ctx *c);
+size_t bf_wop_bytes_per_chan(const bf_ctx *c);
+
+// kernels (each returns a cudaError_t from the launch)
+cudaError_t bf_launch_weights(const bf_ctx *c, cudaStream_t st);
+cudaError_t bf_launch_decode_weights(const bf_ctx *c, float *d_out, cudaStream_t st);
+cudaError_t bf_launch_simt(const BfParams &p, int dtype, cudaStream_t st);
+bool bf_umma_supported(const bf_ctx *c, const char **why);
+cudaError_t bf_launch_umma(const BfParams &p, int dtype, int sm_count, cudaStream_t st);

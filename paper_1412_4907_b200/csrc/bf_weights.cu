@@ -1,0 +1,80 @@
+// bf_weights.cu -- phase-weight generator (hot-path row a1).
+//
+// W[c][b][n] = exp(-i 2 pi f_c/c0 (r_n . s_b)): the steering factor e^{-i k0.r_n} of Eq. 1
+// (PAPER.md:23-28).  The paper computes the coefficients on the CPU between pipeline iterations
+// (PAPER.md:220); here one kernel writes them straight into the tensor-core operand layout
+// (bf_internal.h).  The phase in turns is formed and range-reduced in fp64 -- at 408 MHz over a
+// 310 m array it is ~200 turns, so an fp32 phase would already cost 6e-5 of the 1e-3 budget --
+// then sincospi, then one rounding to fp16.
+#include "bf_internal.h"
+
+#define BF_C0 299792458.0
+
+__global__ void bf_weights_kernel(const double *__restrict__ ant, const double *__restrict__ freq,
+                                  const double *__restrict__ dir, __half *__restrict__ wop, int nant,
+                                  int nchan, int nbeam, int nMt, int nKb) {
+  // one thread per (chan, mt, row, n-slot) where n-slot covers the padded K' / 2
+  const int npad = nKb * (BF_KBLOCK / 2);
+  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  long long total = (long long)nchan * nMt * BF_TILE_ROWS * npad;
+  if (idx >= total) return;
+  int n = (int)(idx % npad);
+  long long t = idx / npad;
+  int r = (int)(t % BF_TILE_ROWS);
+  t /= BF_TILE_ROWS;
+  int mt = (int)(t % nMt);
+  int c = (int)(t / nMt);
+  int b = bf_row_beam(mt, r);
+  int part = bf_row_part(r);
+  float a0 = 0.f, a1 = 0.f;
+  if (b < nbeam && n < nant) {
+    double dot = ant[3 * n] * dir[3 * b] + ant[3 * n + 1] * dir[3 * b + 1] + ant[3 * n + 2] * dir[3 * b + 2];
+    double turns = freq[c] * dot / BF_C0;
+    turns -= rint(turns);  // |turns| <= 1/2: exact subtraction, no accuracy lost to the big phase
+    double s, co;
+    sincospi(2.0 * turns, &s, &co);
+    double wre = co, wim = -s;  // e^{-i phi}
+    if (part == 0) { a0 = (float)wre; a1 = (float)(-wim); }
+    else           { a0 = (float)wim; a1 = (float)wre; }
+  }
+  int kb = (2 * n) / BF_KBLOCK, kk = (2 * n) % BF_KBLOCK;
+  size_t o = ((((size_t)c * nMt + mt) * nKb + kb) * BF_TILE_ROWS + r) * BF_KBLOCK + kk;
+  *reinterpret_cast<__half2 *>(wop + o) = __floats2half2_rn(a0, a1);
+}
+
+cudaError_t bf_launch_weights(const bf_ctx *c, cudaStream_t st) {
+  long long total = (long long)c->nchan * c->nMt * BF_TILE_ROWS * c->nKb * (BF_KBLOCK / 2);
+  int threads = 256;
+  long long blocks = (total + threads - 1) / threads;
+  bf_weights_kernel<<<(unsigned)blocks, threads, 0, st>>>(c->d_ant, c->d_freq, c->d_dir, c->d_wop, c->nant,
+                                                          c->nchan, c->nbeam, c->nMt, c->nKb);
+  return cudaGetLastError();
+}
+
+// operand layout -> logical fp32 [chan][beam][ant][2] (for bf_get_weights)
+__global__ void bf_decode_weights_kernel(const __half *__restrict__ wop, float *__restrict__ out, int nant,
+                                         int nchan, int nbeam, int nMt, int nKb) {
+  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  long long total = (long long)nchan * nbeam * nant;
+  if (idx >= total) return;
+  int n = (int)(idx % nant);
+  long long t = idx / nant;
+  int b = (int)(t % nbeam);
+  int c = (int)(t / nbeam);
+  int mt = b / BF_TILE_BEAMS, bl = b % BF_TILE_BEAMS;
+  int kb = (2 * n) / BF_KBLOCK, kk = (2 * n) % BF_KBLOCK;
+  size_t base = (((size_t)c * nMt + mt) * nKb + kb) * BF_TILE_ROWS;
+  float wre = __half2float(wop[(base + bf_beam_row(bl, 0)) * BF_KBLOCK + kk]);
+  float wim = __half2float(wop[(base + bf_beam_row(bl, 1)) * BF_KBLOCK + kk]);
+  out[2 * idx] = wre;
+  out[2 * idx + 1] = wim;
+}
+
+cudaError_t bf_launch_decode_weights(const bf_ctx *c, float *d_out, cudaStream_t st) {
+  long long total = (long long)c->nchan * c->nbeam * c->nant;
+  int threads = 256;
+  long long blocks = (total + threads - 1) / threads;
+  bf_decode_weights_kernel<<<(unsigned)blocks, threads, 0, st>>>(c->d_wop, d_out, c->nant, c->nchan, c->nbeam,
+                                                                 c->nMt, c->nKb);
+  return cudaGetLastError();
+}

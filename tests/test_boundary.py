@@ -1,0 +1,95 @@
+"""CPU-side checks of the C-ABI boundary: the library loads, exports every symbol include/bf.h
+declares, and validates its arguments.  No compute calls (no GPU here)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def bf():
+    from paper_1412_4907_b200 import build
+    build.build()
+    import paper_1412_4907_b200 as bf
+    bf.lib()
+    return bf
+
+
+def test_header_symbols_all_exported(bf):
+    hdr = open(os.path.join(ROOT, "include", "bf.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(bf_[a-z_]+)\s*\(", hdr))
+    assert declared, "no declarations found"
+    assert declared == set(bf.SYMBOLS), (declared ^ set(bf.SYMBOLS))
+    L = ctypes.CDLL(bf.LIB_PATH)
+    for name in declared:
+        assert hasattr(L, name), name
+    assert "sm_100a" in bf.bf_version()
+
+
+def test_create_validation(bf):
+    assert bf.bf_create(32, 64, 16, 1024, 16)
+    for bad in [(0, 1, 1, 16, 16), (1, 0, 1, 16, 16), (1, 1, 0, 16, 16), (1, 1, 1, 0, 16), (1, 1, 1, 16, 0),
+                (-3, 1, 1, 16, 16), (32, 64, 16, 1000, 16)]:  # last: nsamp % nint != 0 (reading A8)
+        assert not bf.bf_create(*bad), bad
+    ctx = bf.bf_create(5, 3, 1, 7, 7)  # odd sizes and a single beam are legal
+    assert ctx
+    bf.bf_destroy(ctx)
+    bf.bf_destroy(None)
+
+
+def test_argument_errors_without_gpu(bf):
+    ctx = bf.bf_create(32, 4, 16, 256, 16)
+    assert bf.bf_set_dtype(ctx, 7) == bf.BF_EINVAL
+    assert "dtype" in bf.bf_last_error(ctx)
+    assert bf.bf_set_dtype(ctx, bf.BF_CF16) == bf.BF_OK
+    assert bf.bf_set_dtype(ctx, bf.BF_CI8) == bf.BF_OK
+    assert bf.bf_set_kernel(ctx, 9) == bf.BF_EINVAL
+    assert bf.bf_workspace_bytes(ctx) > 4 * 16 * 32 * 4
+    assert bf.bf_workspace_bytes(ctx) % 1024 == 0
+    assert bf.bf_set_workspace(ctx, None, 1 << 20) == bf.BF_EINVAL
+    assert bf.bf_set_workspace(ctx, 0x1000 + 8, 1 << 30) == bf.BF_EINVAL  # misaligned
+    assert bf.bf_set_workspace(ctx, 0x10000, 16) == bf.BF_ENOMEM
+    # run before geometry
+    assert bf.bf_run(ctx, 0x10000, 0x20000) == bf.BF_ENOGEOM
+    assert bf.bf_run(ctx, None, 0x20000) == bf.BF_EINVAL
+    # geometry validation happens before any device access
+    r = np.zeros((32, 3)); f = np.full(4, 408e6); s = np.tile([0.0, 0.0, 1.0], (16, 1))
+    assert bf.bf_set_geometry(ctx, r, f, s) == bf.BF_ENOGEOM  # no workspace yet
+    assert bf.bf_set_geometry(ctx, None, f, s) == bf.BF_EINVAL
+    s_bad = s.copy(); s_bad[3] = [0.0, 0.0, 1.1]
+    assert bf.bf_set_geometry(ctx, r, f, s_bad) == bf.BF_EINVAL
+    assert "unit vector" in bf.bf_last_error(ctx)
+    f_bad = f.copy(); f_bad[1] = np.nan
+    assert bf.bf_set_geometry(ctx, r, f_bad, s) == bf.BF_EINVAL
+    r_bad = r.copy(); r_bad[0, 0] = np.inf
+    assert bf.bf_set_geometry(ctx, r_bad, f, s) == bf.BF_EINVAL
+    assert bf.bf_staging_bytes(ctx, 2) >= 2 * (2 * 256 * 32 * 2 + 2 * 16 * 16 * 4)
+    assert bf.bf_launch_count(ctx) == 0
+    bf.bf_destroy(ctx)
+
+
+def test_no_device_means_error_not_fallback(bf):
+    """On a box without a GPU the compute entry points must fail loudly (BF_ECUDA/BF_EUNSUPPORTED)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    ctx = bf.bf_create(8, 2, 4, 64, 16)
+    assert bf.bf_set_workspace(ctx, 0x7f0000000000, bf.bf_workspace_bytes(ctx)) == bf.BF_OK  # pointer only recorded
+    r = np.zeros((8, 3)); f = np.full(2, 100e6); s = np.tile([0.0, 0.0, 1.0], (4, 1))
+    rc = bf.bf_set_geometry(ctx, r, f, s)
+    assert rc in (bf.BF_ECUDA, bf.BF_EUNSUPPORTED), rc
+    assert bf.bf_last_error(ctx)
+    bf.bf_destroy(ctx)
+
+
+def test_kernel_selection_is_static_function_of_shape(bf):
+    ctx = bf.bf_create(5, 3, 1, 7, 7)  # odd nant: only the generic kernel takes it
+    assert bf.bf_selected_kernel(ctx) == bf.BF_KERNEL_SIMT
+    bf.bf_set_kernel(ctx, bf.BF_KERNEL_UMMA)
+    assert bf.bf_selected_kernel(ctx) == bf.BF_KERNEL_UMMA  # forced; bf_run would report BF_EUNSUPPORTED
+    bf.bf_destroy(ctx)
