@@ -30,12 +30,13 @@ BF_DEVI bool mbar_try_wait(uint32_t bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
-// Bounded spin: a mis-phased pipeline must fail (trap), not hang the GPU.  try_wait itself sleeps in
-// hardware for a while, so 2^24 polls is seconds, far beyond any legitimate wait.
+// Bounded spin: a mis-phased pipeline must fail (trap), not hang the GPU: give up after ~2 s.
 BF_DEVI void mbar_wait(uint32_t bar, uint32_t parity) {
-  for (uint32_t i = 0; i < (1u << 24); ++i)
-    if (mbar_try_wait(bar, parity)) return;
-  asm volatile("trap;");
+  if (mbar_try_wait(bar, parity)) return;
+  const long long t0 = clock64();
+  while (!mbar_try_wait(bar, parity)) {
+    if (clock64() - t0 > 4000000000LL) asm volatile("trap;");
+  }
 }
 
 // ---- tcgen05 -----------------------------------------------------------------------------------
