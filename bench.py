@@ -1,0 +1,341 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the B200 coherent beamformer (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config medium] [--impl ours|reference]
+
+One "step" is one pass of the whole hot path (ingest -> contraction -> |.|^2 -> integrate) over one
+synthetic `medium` buffer (BASELINE.json configs[1]: 32 antennas, 1024 channels, 128 beams, 32768
+samples, complex int8, nint 64).  Prints ONE JSON line (rank 0).  Metric: beamforming TFLOP/s at
+8 flop per complex MAC.  N > 1 runs one replica per GPU on its own buffer (channels
+are independent, so the path shards with no exchange; "weak" scaling) and reports the aggregate.
+
+--impl reference times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "beamforming TFLOP/s (8 flop/complex MAC)"
+UNIT = "TFLOP/s"
+
+
+def load_peaks():
+    """Measured roofline denominators (driver-written), else the profiling guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            d = json.load(open(path))
+            return {"hbm_gbs": float(d["hbm_gbs"]), "tensor_tflops": float(d.get("bf16_tflops_sustained", d["bf16_tflops"])),
+                    "tensor_tflops_burst": float(d["bf16_tflops"]), "source": "measured"}
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "tensor_tflops": 1400.0, "tensor_tflops_burst": 1590.0, "source": "fallback"}
+
+
+def workload_for(name):
+    import synthetic
+    if name.startswith("sweep-"):
+        return synthetic.make_workload("sweep", nbeam=int(name.split("-")[1]))
+    return synthetic.make_workload(name)
+
+
+def algorithmic_bytes(w):
+    """per channel read the voltages once, the weights once, write the powers."""
+    return w.in_bytes + w.nchan * w.nbeam * w.nant * 4 + w.out_bytes
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        time.sleep(0.05)
+        self.proc.terminate()
+        try:
+            text, _ = self.proc.communicate(timeout=5)
+        except Exception:
+            self.proc.kill()
+            text = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in text.splitlines():
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def time_oracle_sample(w, v_host_fn, target_s=15.0, max_chan=64):
+    """The oracle as it stands on the host cores, on whole channels of the workload; returns
+    (TFLOP/s, cores, description).  v_host_fn(chan_list) -> numpy voltages of those channels."""
+    import numpy as np
+    import oracle
+    cores = oracle.num_threads()
+    # calibrate on `cores` channels (one per thread), then size the sample for ~target_s
+    n0 = min(w.nchan, cores)
+    chans = list(range(n0))
+    ws = w.sub(chan_idx=chans)
+    v = v_host_fn(chans)
+    t0 = time.perf_counter()
+    oracle.beamform(ws.ant_xyz, ws.freqs, ws.beam_dir, v, ws.nint)
+    dt0 = time.perf_counter() - t0
+    per_chan = dt0 / n0
+    n = int(max(n0, min(max_chan, w.nchan, target_s / max(per_chan, 1e-9))))
+    n = max(cores, n // cores * cores) if n >= cores else n
+    n = min(n, w.nchan)
+    if n > n0:
+        chans = list(range(n))
+        ws = w.sub(chan_idx=chans)
+        v = v_host_fn(chans)
+        t0 = time.perf_counter()
+        oracle.beamform(ws.ant_xyz, ws.freqs, ws.beam_dir, v, ws.nint)
+        dt = time.perf_counter() - t0
+    else:
+        n, dt = n0, dt0
+    flop = 8.0 * n * w.nbeam * w.nant * w.nsamp
+    return flop / dt / 1e12, cores, f"{n} of {w.nchan} channels x all {w.nbeam} beams x all {w.nsamp} samples, {dt:.2f} s", dt, n
+
+
+def run_reference(args):
+    """--impl reference: the fp64 oracle on the host cores, each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import numpy as np
+    import oracle
+    w = workload_for(args.config)
+    cores = oracle.num_threads()
+    nchan = min(w.nchan, cores)  # one channel per thread per step keeps K+W steps within minutes
+    chans = list(range(nchan))
+    ws = w.sub(chan_idx=chans)
+    v = w.make_voltages(nchan=nchan)
+    steps = max(1, args.steps)
+    for _ in range(max(0, args.warmup)):
+        oracle.beamform(ws.ant_xyz, ws.freqs, ws.beam_dir, v, ws.nint)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle.beamform(ws.ant_xyz, ws.freqs, ws.beam_dir, v, ws.nint)
+    dt = (time.perf_counter() - t0) / steps
+    flop = 8.0 * nchan * w.nbeam * w.nant * w.nsamp
+    val = flop / dt / 1e12
+    sample = f"{nchan} of {w.nchan} channels x all {w.nbeam} beams x all {w.nsamp} samples per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "nant": w.nant, "nchan": w.nchan, "nbeam": w.nbeam, "nsamp": w.nsamp,
+                   "nint": w.nint, "input": w.dtype, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="medium")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "simt", "umma"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--chan-per-chunk", type=int, default=0, help="e2e: channels per H2D chunk (0 = nchan/8)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    import synthetic
+    import paper_1412_4907_b200 as bf
+
+    bf.lib()  # fail loudly if the CUDA library is missing: there is no fallback
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = world > 1
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if dist:
+        import torch.distributed as td
+        td.init_process_group("nccl", device_id=dev)
+
+    W = max(3, args.warmup)
+    K = max(1, args.steps)
+    w = workload_for(args.config)
+    w.seed += 100 * rank  # every replica beamforms its own buffer
+    peaks = load_peaks()
+    kern = {"auto": bf.BF_KERNEL_AUTO, "simt": bf.BF_KERNEL_SIMT, "umma": bf.BF_KERNEL_UMMA}[args.kernel]
+    dt = bf.BF_CI8 if w.dtype == "ci8" else bf.BF_CF16
+
+    B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint, dtype=dt, kernel=kern, device=dev)
+    B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
+    v = synthetic.fill_voltages_torch(w, dev)
+    P = B.empty_powers()
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        if dist:
+            td.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---------------------------------------------------------------- device-resident timing
+    for _ in range(W):
+        B.run(v, P, stream)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
+    l0 = B.launches
+    barrier()
+    ev[0].record(stream)
+    for k in range(K):
+        B.run(v, P, stream)
+        ev[k + 1].record(stream)
+    barrier()
+    launches = B.launches - l0
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = ev[0].elapsed_time(ev[K])
+    per_launch_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(K)]
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if dist:
+        td.all_reduce(t, op=td.ReduceOp.MAX)
+    total_ms_max = float(t.item())
+    flop_step = 8.0 * w.cmac
+    value = world * flop_step * K / (total_ms_max * 1e-3) / 1e12
+    ms_per_step = total_ms_max / K
+    avg_kernel_ms = statistics.mean(per_launch_ms)
+
+    # roofline of the dominant (only) kernel: a dense contraction -> tensor bound; HBM-bound when
+    # the algorithmic bytes at measured bandwidth take longer than the flops at measured tensor peak
+    abytes = algorithmic_bytes(w)
+    t_hbm = abytes / (peaks["hbm_gbs"] * 1e9)
+    t_tensor = flop_step / (peaks["tensor_tflops"] * 1e12)
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(w.name)
+        except Exception:
+            traffic = None
+    if t_tensor >= t_hbm:
+        ach = flop_step / (avg_kernel_ms * 1e-3) / 1e12
+        roof = {"bound": "tensor", "achieved": ach, "peak": peaks["tensor_tflops"], "unit": "TFLOP/s",
+                "frac": ach / peaks["tensor_tflops"], "traffic": traffic, "peak_kind": peaks["source"] + " sustained bf16/fp16 dense",
+                "kernel_ms": avg_kernel_ms}
+    else:
+        ach = abytes / (avg_kernel_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": ach / peaks["hbm_gbs"], "traffic": traffic, "peak_kind": peaks["source"] + " copy bandwidth",
+                "kernel_ms": avg_kernel_ms}
+
+    # ---------------------------------------------------------------- end to end through the C ABI with HOST buffers
+    e2e = None
+    if not args.no_e2e:
+        hv = torch.empty(v.shape, dtype=v.dtype, pin_memory=True)
+        hv.copy_(v)
+        hp = torch.empty(P.shape, dtype=torch.float32, pin_memory=True)
+        cpc = args.chan_per_chunk or max(1, w.nchan // 8)
+        cs, xs = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+        del v
+        torch.cuda.empty_cache()
+        Ke = min(K, 10)
+        for _ in range(2):
+            B.run_host(hv, hp, cpc, cs, xs)
+        cs.synchronize(); xs.synchronize()
+        barrier()
+        t0 = time.perf_counter()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(cs)
+        for _ in range(Ke):
+            B.run_host(hv, hp, cpc, cs, xs)
+        cs.wait_stream(xs)
+        e1.record(cs)
+        cs.synchronize(); xs.synchronize()
+        barrier()
+        e2e_ms = e0.elapsed_time(e1)
+        te = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
+        if dist:
+            td.all_reduce(te, op=td.ReduceOp.MAX)
+        e2e_ms = float(te.item())
+        e2e = {"value": world * flop_step * Ke / (e2e_ms * 1e-3) / 1e12, "unit": UNIT,
+               "h2d_bytes_per_step": int(w.in_bytes), "d2h_bytes_per_step": int(w.out_bytes), "steps": Ke,
+               "ms_per_step": e2e_ms / Ke, "h2d_gbs": w.in_bytes / (e2e_ms / Ke * 1e-3) / 1e9,
+               "chan_per_chunk": cpc, "api": "bf_run_host (pinned host in/out, 2 streams)"}
+        sample_src = hv
+    else:
+        sample_src = v
+
+    # ---------------------------------------------------------------- oracle on the host cores (rank 0, N=1)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        def v_host(chans):
+            return sample_src[chans].cpu().numpy() if sample_src.is_cuda else sample_src[chans].numpy()
+        val, cores, desc, _, _ = time_oracle_sample(w, v_host)
+        cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f16xf16->f32" if B.selected_kernel == bf.BF_KERNEL_UMMA else "f32",
+            "data": "synthetic",
+            "config": {"workload": w.name, "nant": w.nant, "nchan": w.nchan, "nbeam": w.nbeam, "nsamp": w.nsamp,
+                       "nint": w.nint, "input": w.dtype, "l2": "input buffer (%.0f MB) >> L2 (126 MB), no flush needed" % (w.in_bytes / 1e6),
+                       "kernel": {1: "simt", 2: "umma"}[B.selected_kernel], "parallelism": f"replicas x{world}"},
+            "ant_samples_per_s": world * w.nchan * w.nsamp * w.nant * K / (total_ms_max * 1e-3),
+            "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "context": {"paper_k20_tflops": 1.3, "note": "paper's number is a Tesla K20 with 4-bit input (PAPER.md:15): context, not a baseline for this config"},
+        }
+        print(json.dumps(line))
+    B.close()
+    if dist:
+        td.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

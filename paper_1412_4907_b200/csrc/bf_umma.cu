@@ -29,7 +29,7 @@ constexpr int TILE_T = 256;                 // time samples per tile = UMMA N
 constexpr int EPI_WARPS = 8;
 constexpr int A_TILE_BYTES = BF_TILE_ROWS * 128;   // 128 rows x 64 fp16
 constexpr int B_STAGE_BYTES = TILE_T * 128;        // 256 rows x 64 fp16
-constexpr int MAX_PIECES = 8;               // 16-byte input pieces per convert thread per tile
+constexpr int MAX_INPUT_PIECES = TILE_T * 4;  // 16-byte input pieces per tile at nant = 32
 
 struct Item { int c, g, tt; };
 
@@ -40,6 +40,13 @@ __device__ __forceinline__ Item decode_item(long long idx, int nG, int nTt) {
   it.g = (int)(cg % nG);
   it.c = (int)(cg / nG);
   return it;
+}
+// items are walked in order: (chan, beam group, time tile) with the time tile fastest
+__device__ __forceinline__ void next_item(Item &it, int nG, int nTt) {
+  if (++it.tt == nTt) {
+    it.tt = 0;
+    if (++it.g == nG) { it.g = 0; ++it.c; }
+  }
 }
 
 // int8 x4 (one 32-bit word) -> two half2, exact: 0x6400 | (x ^ 0x80) is the fp16 number 1024 + (x + 128)
@@ -116,8 +123,8 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     constexpr int BINS_PER_TILE = NINT_T == 0 ? 1 : TILE_T / NINT_T;
     const bool vec_ok = (BINS_PER_TILE >= 4) && (p.nbin % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.pow) & 15) == 0);
     int u = 0;
-    for (int i = 0; i < n_items; ++i) {
-      const Item it = decode_item(it0 + i, nG, nTt);
+    Item it = decode_item(it0, nG, nTt);
+    for (int i = 0; i < n_items; ++i, next_item(it, nG, nTt)) {
       const int gm = min(GROUP, nMt - it.g * GROUP);
       for (int m = 0; m < gm; ++m, ++u) {
         if ((u & 1) != grp) continue;
@@ -189,6 +196,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     }
   } else if (warp < MMA_WARP) {
     // =========================================================================== ingest / convert
+    constexpr int PIECES = MAX_INPUT_PIECES / CONV_THREADS;  // 16-byte input pieces per thread per tile
     const int ctid = threadIdx.x - EPI_WARPS * 32;
     const int npr = p.nant / 8;                  // 16-byte pieces per time sample (int8: 2*nant bytes)
     const int npieces = TILE_T * npr;
@@ -198,23 +206,30 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     for (int o = ctid * 16; o < NSTAGE * B_STAGE_BYTES; o += CONV_THREADS * 16) st_shared_v4(sB + o, 0, 0, 0, 0);
     asm volatile("bar.sync 1, %0;" ::"n"(CONV_THREADS) : "memory");
 
-    uint4 cur[MAX_PIECES], nxt[MAX_PIECES];
-    auto load_tile = [&](uint4 (&dst)[MAX_PIECES], const Item &it) {
+    // a thread converts the same pieces of every tile: row t, 16-byte piece q of that row
+    int p_t[PIECES];        // time row inside the tile (TILE_T = not mine)
+    uint32_t p_src[PIECES]; // byte offset inside the tile's input
+    uint32_t p_dst[PIECES]; // byte offset of the first output chunk inside a stage (second chunk: ^ 16)
+#pragma unroll
+    for (int k = 0; k < PIECES; ++k) {
+      const int pc = ctid + k * CONV_THREADS;
+      const int t = pc / npr, q = pc - t * npr;
+      p_t[k] = pc < npieces ? t : TILE_T;
+      p_src[k] = (uint32_t)(t * row_bytes + 16 * q);
+      p_dst[k] = (uint32_t)((t >> 3) * 1024 + (t & 7) * 128 + (((2 * q) ^ (t & 7)) << 4));
+    }
+    auto load_tile = [&](uint4 (&dst)[PIECES], const Item &it) {
       const int t_base = it.tt * TILE_T;
+      const int rows = min(TILE_T, p.nsamp - t_base);
       const char *base = volt + ((size_t)it.c * p.nsamp + t_base) * row_bytes;
 #pragma unroll
-      for (int k = 0; k < MAX_PIECES; ++k) {
-        const int pc = ctid + k * CONV_THREADS;
-        const int t = pc / npr, q = pc - t * npr;
-        if (pc < npieces && t_base + t < p.nsamp) dst[k] = ldg_nc_v4(base + (size_t)t * row_bytes + 16 * q);
+      for (int k = 0; k < PIECES; ++k) {
+        if (p_t[k] < rows) dst[k] = ldg_nc_v4(base + p_src[k]);
         else dst[k] = make_uint4(0u, 0u, 0u, 0u);
       }
     };
     int ag = 0, prev_c = -1, prev_g = -1;
-    if (n_items > 0) load_tile(cur, decode_item(it0, nG, nTt));
-    for (int i = 0; i < n_items; ++i) {
-      const Item it = decode_item(it0 + i, nG, nTt);
-      if (i + 1 < n_items) load_tile(nxt, decode_item(it0 + i + 1, nG, nTt));
+    auto convert_tile = [&](const uint4 (&src)[PIECES], const Item &it, int i) {
       if (it.c != prev_c || it.g != prev_g) {
         // new (channel, beam group): bring its coefficient tiles into the other A buffer
         prev_c = it.c; prev_g = it.g;
@@ -237,32 +252,41 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
       mbar_wait(bar_b_empty + 8 * st, ((i / NSTAGE) & 1) ^ 1);
       const uint32_t sdst = sB + st * B_STAGE_BYTES;
 #pragma unroll
-      for (int k = 0; k < MAX_PIECES; ++k) {
-        const int pc = ctid + k * CONV_THREADS;
-        if (pc < npieces) {
-          const int t = pc / npr, q = pc - t * npr;
+      for (int k = 0; k < PIECES; ++k) {
+        if (p_t[k] < TILE_T) {
           uint32_t h[8];
-          cvt_i8x4_f16x4(cur[k].x, h[0], h[1]);
-          cvt_i8x4_f16x4(cur[k].y, h[2], h[3]);
-          cvt_i8x4_f16x4(cur[k].z, h[4], h[5]);
-          cvt_i8x4_f16x4(cur[k].w, h[6], h[7]);
-          const uint32_t rowaddr = sdst + (t >> 3) * 1024 + (t & 7) * 128;
-          st_shared_v4(rowaddr + (((2 * q) ^ (t & 7)) << 4), h[0], h[1], h[2], h[3]);
-          st_shared_v4(rowaddr + (((2 * q + 1) ^ (t & 7)) << 4), h[4], h[5], h[6], h[7]);
+          cvt_i8x4_f16x4(src[k].x, h[0], h[1]);
+          cvt_i8x4_f16x4(src[k].y, h[2], h[3]);
+          cvt_i8x4_f16x4(src[k].z, h[4], h[5]);
+          cvt_i8x4_f16x4(src[k].w, h[6], h[7]);
+          st_shared_v4(sdst + p_dst[k], h[0], h[1], h[2], h[3]);
+          st_shared_v4(sdst + (p_dst[k] ^ 16u), h[4], h[5], h[6], h[7]);
         }
       }
       fence_proxy_async_smem();
       __syncwarp();
       if (lane == 0) mbar_arrive(bar_b_full + 8 * st);
-#pragma unroll
-      for (int k = 0; k < MAX_PIECES; ++k) cur[k] = nxt[k];
+    };
+    // two register buffers, loads issued one tile ahead of their use
+    uint4 bufA[PIECES], bufB[PIECES];
+    Item itA = decode_item(it0, nG, nTt), itB;
+    if (n_items > 0) load_tile(bufA, itA);
+    for (int i = 0; i < n_items; i += 2) {
+      itB = itA; next_item(itB, nG, nTt);
+      if (i + 1 < n_items) load_tile(bufB, itB);
+      convert_tile(bufA, itA, i);
+      itA = itB; next_item(itA, nG, nTt);
+      if (i + 1 < n_items) {
+        if (i + 2 < n_items) load_tile(bufA, itA);
+        convert_tile(bufB, itB, i + 1);
+      }
     }
   } else if (lane == 0) {
     // =========================================================================== MMA issue (one thread)
     constexpr uint32_t idesc = make_idesc_f16(BF_TILE_ROWS, TILE_T);
     int ag = 0, prev_c = -1, prev_g = -1, ab = 0, u = 0;
-    for (int i = 0; i < n_items; ++i) {
-      const Item it = decode_item(it0 + i, nG, nTt);
+    Item it = decode_item(it0, nG, nTt);
+    for (int i = 0; i < n_items; ++i, next_item(it, nG, nTt)) {
       if (it.c != prev_c || it.g != prev_g) {
         if (ag > 0) tc_commit(bar_a_empty + 8 * ab);  // everything issued so far has left the old buffer
         prev_c = it.c; prev_g = it.g;
@@ -315,8 +339,8 @@ cudaError_t launch_k64(const BfParams &p, int sm_count, cudaStream_t st) {
 
 template <int NINT_T>
 cudaError_t launch_k64_nint(const BfParams &p, int sm_count, cudaStream_t st) {
-  if (p.nMt <= 2) return launch_k64<NINT_T, 2, 4, 4>(p, sm_count, st);
-  return launch_k64<NINT_T, 4, 3, 4>(p, sm_count, st);
+  if (p.nMt <= 2) return launch_k64<NINT_T, 2, 4, 8>(p, sm_count, st);
+  return launch_k64<NINT_T, 4, 3, 8>(p, sm_count, st);
 }
 
 }  // namespace
