@@ -17,13 +17,17 @@
 // beam 64 mt + 16 q + (l & 15), part (l >> 4) (0 = re, 1 = im): a warp that owns TMEM lanes
 // 32q..32q+31 finds re and im of one beam 16 lanes apart (one shuffle per OUTPUT bin, not per sample).
 // K' is padded to a multiple of 64 (zeros).  Memory: fp16 [chan][mt][kb][128 rows][64 k'] -- every
-// (chan, mt, kb) block is one contiguous 16 KiB K-major tile.
+// (chan, mt, kb) block is one contiguous 16 KiB K-major tile, stored as the exact shared-memory image
+// tcgen05.mma wants (128-byte swizzle: the 16-byte chunk index of a row is XORed with row & 7), so one
+// cp.async.bulk per tile brings it in with no fix-up.
 #define BF_TILE_ROWS 128
 #define BF_TILE_BEAMS 64
 #define BF_KBLOCK 64
 
 __host__ __device__ inline int bf_row_beam(int mt, int r) { return mt * BF_TILE_BEAMS + ((r >> 5) << 4) + (r & 15); }
 __host__ __device__ inline int bf_row_part(int r) { return (r >> 4) & 1; }
+// element offset of (row r, column k) inside one 128 x 64 tile (128-byte swizzle)
+__host__ __device__ inline int bf_tile_off(int r, int k) { return r * BF_KBLOCK + ((((k >> 3) ^ (r & 7)) << 3) | (k & 7)); }
 // row of (beam-in-tile bl, part)
 __host__ __device__ inline int bf_beam_row(int bl, int part) { return ((bl >> 4) << 5) + (part << 4) + (bl & 15); }
 

@@ -58,9 +58,9 @@ __global__ void __launch_bounds__(SIMT_BEAMS) bf_simt_kernel(BfParams p, int sam
         if (bb < p.nbeam && nn < p.nant) {
           int mt = bb / BF_TILE_BEAMS, bt = bb % BF_TILE_BEAMS;
           int kb = (2 * nn) / BF_KBLOCK, kk = (2 * nn) % BF_KBLOCK;
-          size_t base = ((size_t)mt * p.nKb + kb) * BF_TILE_ROWS;
-          w.x = __half2float(wc[(base + bf_beam_row(bt, 0)) * BF_KBLOCK + kk]);
-          w.y = __half2float(wc[(base + bf_beam_row(bt, 1)) * BF_KBLOCK + kk]);
+          size_t base = ((size_t)mt * p.nKb + kb) * (BF_TILE_ROWS * BF_KBLOCK);
+          w.x = __half2float(wc[base + bf_tile_off(bf_beam_row(bt, 0), kk)]);
+          w.y = __half2float(wc[base + bf_tile_off(bf_beam_row(bt, 1), kk)]);
         }
         Ws[n][bl] = w;
       }

@@ -1,8 +1,9 @@
 // bf_umma.cu -- the fused tensor-core beamformer for small arrays (2*nant <= 64, complex int8 input):
 // hot-path rows a2..a5 in ONE persistent kernel.
 //
-//   a2 ingest      int8 (re,im) voltages  --LDG.128-->  registers  --PRMT/HSUB2-->  fp16, written
-//                  into shared memory in the 128-byte-swizzled K-major layout tcgen05.mma reads
+//   a2 ingest      int8 (re,im) voltages  --cp.async.bulk (TMA engine)-->  raw shared-memory ring
+//                  --LDS.128 / PRMT / HSUB2-->  fp16, written back to shared memory in the
+//                  128-byte-swizzled K-major layout tcgen05.mma reads
 //                  (the paper fuses its 4-bit unpack into the kernel for the same reason: a separate
 //                  pass "would cancel any speed-up")
 //   a3 contraction per channel D[row][t] = sum_k' A[row][k'] X'[t][k'], rows = (re, im) of 64 beams,
@@ -15,21 +16,24 @@
 //   a5 integrate   sum over nint columns in registers, fp32 store to P[chan][beam][bin]
 //
 // Warp roles (one CTA per SM, persistent over a contiguous range of (chan, beam group, time tile)):
-//   warps 0-7   epilogue: warp w owns TMEM lanes 32*(w&3).., accumulator stage (w>>2)
-//   warps 8..   ingest/convert (CONV_WARPS), also load the coefficient tiles when the channel changes
-//   last warp   TMEM allocation + the single MMA-issuing thread
-// Pipelines (all mbarrier based): voltage stages full/empty (convert <-> MMA), coefficient buffers
-// full/empty, TMEM accumulator stages full/empty (MMA <-> epilogue).
+//   warps 0-15  epilogue: warp w owns TMEM lanes 32*(w&3).. and columns 64*(w>>2).. of every tile
+//   warps 16..  convert (CONV_WARPS): raw int8 stage -> fp16 operand stage
+//   next warp   TMEM allocation + the single MMA-issuing thread
+//   last warp   one thread issuing the bulk copies (voltage tiles; coefficient tiles on channel change)
+// Pipelines (all mbarrier based): raw stages full/empty (TMA <-> convert), operand stages full/empty
+// (convert <-> MMA), coefficient buffers full/empty (TMA <-> MMA), TMEM accumulator stages full/empty
+// (MMA <-> epilogue).
 #include "bf_internal.h"
 #include "ptx.cuh"
 
 namespace {
 
 constexpr int TILE_T = 256;                 // time samples per tile = UMMA N
-constexpr int EPI_WARPS = 8;
+constexpr int EPI_WARPS = 16;
 constexpr int A_TILE_BYTES = BF_TILE_ROWS * 128;   // 128 rows x 64 fp16
 constexpr int B_STAGE_BYTES = TILE_T * 128;        // 256 rows x 64 fp16
 constexpr int MAX_INPUT_PIECES = TILE_T * 4;  // 16-byte input pieces per tile at nant = 32
+constexpr int RAW_STAGE_BYTES = TILE_T * 64;  // 256 time samples x 32 antennas x (re, im) int8
 
 struct Item { int c, g, tt; };
 
@@ -64,6 +68,11 @@ __device__ __forceinline__ void cvt_i8x4_f16x4(uint32_t w, uint32_t &lo, uint32_
 __device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
 }
+__device__ __forceinline__ uint4 ld_shared_v4(uint32_t addr) {
+  uint4 r;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
+  return r;
+}
 __device__ __forceinline__ uint4 ldg_nc_v4(const void *p) {
   uint4 r;
   asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
@@ -72,31 +81,37 @@ __device__ __forceinline__ uint4 ldg_nc_v4(const void *p) {
   return r;
 }
 
-// NINT_T: integration length if it is a power of two <= 256, 0 = multiple of 256 (partial sums are
-// added atomically into a zeroed output).
-template <int NINT_T, int GROUP, int NSTAGE, int CONV_WARPS>
-__global__ void __launch_bounds__((EPI_WARPS + CONV_WARPS + 1) * 32, 1)
+// NINT_T: integration length if it is a power of two <= 64; 0 = a larger multiple of 64 (each epilogue
+// warp adds the partial sum of its 64 columns atomically into a zeroed output).
+template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS>
+__global__ void __launch_bounds__((EPI_WARPS + CONV_WARPS + 2) * 32, 1)
 bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, const int nTt, const int nks) {
   extern __shared__ uint8_t smem_raw[];
   constexpr int CONV_THREADS = CONV_WARPS * 32;
   constexpr int MMA_WARP = EPI_WARPS + CONV_WARPS;
+  constexpr int TMA_WARP = MMA_WARP + 1;
 
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t sA = smem_base;                                  // 2 buffers x GROUP tiles
-  const uint32_t sB = sA + 2 * GROUP * A_TILE_BYTES;              // NSTAGE stages
-  const uint32_t sBar = sB + NSTAGE * B_STAGE_BYTES;              // barriers
+  const uint32_t sA = smem_base;                                  // 2 buffers x GROUP coefficient tiles
+  const uint32_t sB = sA + 2 * GROUP * A_TILE_BYTES;              // NSTAGE fp16 operand stages
+  const uint32_t sR = sB + NSTAGE * B_STAGE_BYTES;                // NRAW raw int8 stages
+  const uint32_t sBar = sR + NRAW * RAW_STAGE_BYTES;              // barriers
   const uint32_t bar_b_full = sBar, bar_b_empty = sBar + 8 * NSTAGE;
-  const uint32_t bar_a_full = sBar + 16 * NSTAGE, bar_a_empty = bar_a_full + 16;
+  const uint32_t bar_r_full = sBar + 16 * NSTAGE, bar_r_empty = bar_r_full + 8 * NRAW;
+  const uint32_t bar_a_full = bar_r_full + 16 * NRAW, bar_a_empty = bar_a_full + 16;
   const uint32_t bar_t_full = bar_a_full + 32, bar_t_empty = bar_t_full + 16;
   const uint32_t s_tmem = bar_t_full + 32;
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // warp index through a shuffle so that the compiler knows it is warp-uniform (role code then
+  // runs on the uniform datapath: descriptors in uniform registers, no per-lane waterfall loops)
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < NSTAGE; ++s) { mbar_init(bar_b_full + 8 * s, CONV_WARPS); mbar_init(bar_b_empty + 8 * s, 1); }
+    for (int s = 0; s < NRAW; ++s) { mbar_init(bar_r_full + 8 * s, 1); mbar_init(bar_r_empty + 8 * s, CONV_WARPS); }
     for (int s = 0; s < 2; ++s) {
-      mbar_init(bar_a_full + 8 * s, CONV_WARPS); mbar_init(bar_a_empty + 8 * s, 1);
-      mbar_init(bar_t_full + 8 * s, 1);          mbar_init(bar_t_empty + 8 * s, EPI_WARPS / 2);
+      mbar_init(bar_a_full + 8 * s, 1); mbar_init(bar_a_empty + 8 * s, 1);
+      mbar_init(bar_t_full + 8 * s, 1);          mbar_init(bar_t_empty + 8 * s, EPI_WARPS);
     }
     fence_barrier_init();
   }
@@ -106,6 +121,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(s_tmem));
+  tmem_base = __shfl_sync(0xffffffffu, tmem_base, 0);
 
   // this CTA's contiguous item range
   const long long it0 = total_items * blockIdx.x / gridDim.x;
@@ -115,180 +131,154 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
 
   if (warp < EPI_WARPS) {
     // =========================================================================== epilogue
-    const int quad = warp & 3, grp = warp >> 2;
-    const uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16) + grp * TILE_T;
+    // 16 warps: warp w owns TMEM lanes 32*(w&3).. and columns 64*(w>>2).. of EVERY accumulator tile.
+    // The TMEM stage is handed back to the MMA thread as soon as this warp's last tcgen05.ld has
+    // landed in registers -- the squaring of that last chunk, the shuffle and the store run in the
+    // shadow of the next tile's MMAs.
+    constexpr int CPW = TILE_T / (EPI_WARPS / 4);                          // columns per warp (64)
+    constexpr int NCH = CPW / 32;                                          // 32-column chunks per warp
+    const int quad = warp & 3, slot = warp >> 2;
+    const uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16) + slot * CPW;
     constexpr int SUB = (NINT_T == 0 || NINT_T > 32) ? 32 : NINT_T;        // columns per partial sum
-    constexpr int NSUB = 32 / SUB;                                          // partial sums per 32-column chunk
-    constexpr int CPB = NINT_T == 0 ? 8 : (NINT_T <= 32 ? 1 : NINT_T / 32);  // chunks per bin
-    constexpr int BINS_PER_TILE = NINT_T == 0 ? 1 : TILE_T / NINT_T;
-    const bool vec_ok = (BINS_PER_TILE >= 4) && (p.nbin % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.pow) & 15) == 0);
+    constexpr int NSUB = 32 / SUB;                                          // partial sums per chunk
+    constexpr int CPB = NINT_T == 0 ? NCH : (NINT_T <= 32 ? 1 : NINT_T / 32);  // chunks per bin
+    constexpr int BINS_PER_WARP = NINT_T == 0 ? 1 : CPW / NINT_T;
+    static_assert(NINT_T == 0 || (NINT_T <= CPW && CPW % NINT_T == 0), "bin must not straddle epilogue warps");
+    const bool vec_ok = (BINS_PER_WARP >= 4) && (p.nbin % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.pow) & 15) == 0);
     int u = 0;
     Item it = decode_item(it0, nG, nTt);
     for (int i = 0; i < n_items; ++i, next_item(it, nG, nTt)) {
       const int gm = min(GROUP, nMt - it.g * GROUP);
       for (int m = 0; m < gm; ++m, ++u) {
-        if ((u & 1) != grp) continue;
-        mbar_wait(bar_t_full + 8 * grp, (u >> 1) & 1);
+        const int acc = u & 1;
+        mbar_wait(bar_t_full + 8 * acc, (u >> 1) & 1);
         tc_fence_after();
         const int mt = it.g * GROUP + m;
         const int beam0 = mt * BF_TILE_BEAMS + quad * 16;
-        if (beam0 < p.nbeam) {  // warp-uniform: this lane quadrant holds real beams
-          const int beam = beam0 + (lane & 15);
-          const bool writer = (lane < 16) && (beam < p.nbeam);
-          float *prow = p.pow + ((size_t)it.c * p.nbeam + beam) * p.nbin;
-          const int bin0 = NINT_T == 0 ? (int)(((long long)it.tt * TILE_T) / p.nint) : it.tt * BINS_PER_TILE;
-          uint32_t r[2][32];
-          BF_TMEM_LD_32x32b_X32(t_lane, r[0]);
-          float binacc = 0.f;
-          float ob[4];
+        if (beam0 >= p.nbeam) {  // warp-uniform: this lane quadrant holds only padding rows
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_t_empty + 8 * acc);
+          continue;
+        }
+        const int beam = beam0 + (lane & 15);
+        const bool writer = (lane < 16) && (beam < p.nbeam);
+        float *prow = p.pow + ((size_t)it.c * p.nbeam + beam) * p.nbin;
+        const int t_first = it.tt * TILE_T + slot * CPW;  // first time sample of this warp's columns
+        const int bin0 = NINT_T == 0 ? t_first / p.nint : t_first / (NINT_T == 0 ? 1 : NINT_T);
+        float binacc = 0.f;
+        float ob[4];
 #pragma unroll
-          for (int ch = 0; ch < 8; ++ch) {
-            tc_wait_ld();
-            if (ch + 1 < 8) { BF_TMEM_LD_32x32b_X32(t_lane + 32 * (ch + 1), r[(ch + 1) & 1]); }
-            const uint32_t *v = r[ch & 1];
+        for (int ch = 0; ch < NCH; ++ch) {
+          uint32_t v[32];
+          BF_TMEM_LD_32x32b_X32(t_lane + acc * TILE_T + 32 * ch, v);
+          tc_wait_ld();
+          if (ch == NCH - 1) {  // all of this warp's columns are in registers: release the stage
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_t_empty + 8 * acc);
+          }
 #pragma unroll
-            for (int s = 0; s < NSUB; ++s) {
-              float sum;
-              if constexpr (SUB == 1) {
-                const float d = __uint_as_float(v[s]);
-                sum = d * d;
-              } else {
-                constexpr int NACC = SUB >= 8 ? 4 : SUB / 2;
-                float2 a[NACC];
+          for (int s = 0; s < NSUB; ++s) {
+            float sum;
+            if constexpr (SUB == 1) {
+              const float d = __uint_as_float(v[s]);
+              sum = d * d;
+            } else {
+              constexpr int NACC = SUB >= 8 ? 4 : SUB / 2;
+              float2 a[NACC];
 #pragma unroll
-                for (int q = 0; q < NACC; ++q) a[q] = make_float2(0.f, 0.f);
+              for (int q = 0; q < NACC; ++q) a[q] = make_float2(0.f, 0.f);
 #pragma unroll
-                for (int j = 0; j < SUB / 2; ++j) {
-                  const float2 d = make_float2(__uint_as_float(v[s * SUB + 2 * j]), __uint_as_float(v[s * SUB + 2 * j + 1]));
-                  a[j % NACC] = ffma2(d, d, a[j % NACC]);
-                }
-                sum = 0.f;
-#pragma unroll
-                for (int q = 0; q < NACC; ++q) sum += a[q].x + a[q].y;
+              for (int j = 0; j < SUB / 2; ++j) {
+                const float2 d = make_float2(__uint_as_float(v[s * SUB + 2 * j]), __uint_as_float(v[s * SUB + 2 * j + 1]));
+                a[j % NACC] = ffma2(d, d, a[j % NACC]);
               }
-              if (CPB > 1) {
-                binacc += sum;
-                if ((ch + 1) % CPB != 0) continue;
-                sum = binacc;
-                binacc = 0.f;
-              }
-              const float tot = sum + __shfl_xor_sync(0xffffffffu, sum, 16);  // re^2 rows + im^2 rows
-              if (NINT_T == 0) {
-                if (writer) atomicAdd(prow + bin0, tot);
-              } else {
-                const int jb = (ch / CPB) * NSUB + s;  // bin index inside the tile (compile-time)
-                const int j = bin0 + jb;
-                if (vec_ok) {
-                  ob[jb & 3] = tot;
-                  if ((jb & 3) == 3 && writer && j < p.nbin)
-                    *reinterpret_cast<float4 *>(prow + j - 3) = make_float4(ob[0], ob[1], ob[2], ob[3]);
-                } else if (writer && j < p.nbin) {
-                  prow[j] = tot;
-                }
+              sum = 0.f;
+#pragma unroll
+              for (int q = 0; q < NACC; ++q) sum += a[q].x + a[q].y;
+            }
+            if (CPB > 1) {
+              binacc += sum;
+              if ((ch + 1) % CPB != 0) continue;
+              sum = binacc;
+              binacc = 0.f;
+            }
+            const float tot = sum + __shfl_xor_sync(0xffffffffu, sum, 16);  // re^2 rows + im^2 rows
+            if (NINT_T == 0) {
+              if (writer && t_first < p.nsamp) atomicAdd(prow + bin0, tot);
+            } else {
+              const int jb = (ch / CPB) * NSUB + s;  // bin index inside this warp's columns (compile-time)
+              const int j = bin0 + jb;
+              if (vec_ok) {
+                ob[jb & 3] = tot;
+                if ((jb & 3) == 3 && writer && j < p.nbin)
+                  *reinterpret_cast<float4 *>(prow + j - 3) = make_float4(ob[0], ob[1], ob[2], ob[3]);
+              } else if (writer && j < p.nbin) {
+                prow[j] = tot;
               }
             }
           }
         }
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar_t_empty + 8 * grp);
       }
     }
   } else if (warp < MMA_WARP) {
-    // =========================================================================== ingest / convert
+    // =========================================================================== convert
     constexpr int PIECES = MAX_INPUT_PIECES / CONV_THREADS;  // 16-byte input pieces per thread per tile
     const int ctid = threadIdx.x - EPI_WARPS * 32;
     const int npr = p.nant / 8;                  // 16-byte pieces per time sample (int8: 2*nant bytes)
     const int npieces = TILE_T * npr;
-    const size_t row_bytes = (size_t)2 * p.nant;
-    const char *volt = reinterpret_cast<const char *>(p.volt);
-    // zero the stages once: K' columns beyond 2*nant must read as 0, never as stale NaN patterns
+    // zero the operand stages once: K' columns beyond 2*nant must read as 0, never as stale NaN patterns
     for (int o = ctid * 16; o < NSTAGE * B_STAGE_BYTES; o += CONV_THREADS * 16) st_shared_v4(sB + o, 0, 0, 0, 0);
     asm volatile("bar.sync 1, %0;" ::"n"(CONV_THREADS) : "memory");
 
-    // a thread converts the same pieces of every tile: row t, 16-byte piece q of that row
-    int p_t[PIECES];        // time row inside the tile (TILE_T = not mine)
-    uint32_t p_src[PIECES]; // byte offset inside the tile's input
-    uint32_t p_dst[PIECES]; // byte offset of the first output chunk inside a stage (second chunk: ^ 16)
+    // a thread converts the same pieces of every tile: row t, 16-byte piece q of that row.  Raw rows
+    // are compact (2*nant bytes), so piece pc sits at byte 16*pc of the raw stage.
+    uint32_t p_dst[PIECES];  // byte offset of the first output chunk inside a stage (second chunk: ^ 16)
 #pragma unroll
     for (int k = 0; k < PIECES; ++k) {
       const int pc = ctid + k * CONV_THREADS;
       const int t = pc / npr, q = pc - t * npr;
-      p_t[k] = pc < npieces ? t : TILE_T;
-      p_src[k] = (uint32_t)(t * row_bytes + 16 * q);
-      p_dst[k] = (uint32_t)((t >> 3) * 1024 + (t & 7) * 128 + (((2 * q) ^ (t & 7)) << 4));
+      p_dst[k] = pc < npieces ? (uint32_t)((t >> 3) * 1024 + (t & 7) * 128 + (((2 * q) ^ (t & 7)) << 4)) : 0xffffffffu;
     }
-    auto load_tile = [&](uint4 (&dst)[PIECES], const Item &it) {
-      const int t_base = it.tt * TILE_T;
-      const int rows = min(TILE_T, p.nsamp - t_base);
-      const char *base = volt + ((size_t)it.c * p.nsamp + t_base) * row_bytes;
+    for (int i = 0; i < n_items; ++i) {
+      const int rs = i % NRAW;
+      mbar_wait(bar_r_full + 8 * rs, (i / NRAW) & 1);
+      uint4 x[PIECES];
 #pragma unroll
-      for (int k = 0; k < PIECES; ++k) {
-        if (p_t[k] < rows) dst[k] = ldg_nc_v4(base + p_src[k]);
-        else dst[k] = make_uint4(0u, 0u, 0u, 0u);
-      }
-    };
-    int ag = 0, prev_c = -1, prev_g = -1;
-    auto convert_tile = [&](const uint4 (&src)[PIECES], const Item &it, int i) {
-      if (it.c != prev_c || it.g != prev_g) {
-        // new (channel, beam group): bring its coefficient tiles into the other A buffer
-        prev_c = it.c; prev_g = it.g;
-        const int ab = ag & 1;
-        mbar_wait(bar_a_empty + 8 * ab, ((ag >> 1) & 1) ^ 1);
-        const int gm = min(GROUP, nMt - it.g * GROUP);
-        const char *wsrc = reinterpret_cast<const char *>(p.wop) + ((size_t)it.c * nMt + (size_t)it.g * GROUP) * A_TILE_BYTES;
-        for (int pc = ctid; pc < gm * (A_TILE_BYTES / 16); pc += CONV_THREADS) {
-          const int row = pc >> 3, j = pc & 7;  // row over gm*128 rows
-          const uint4 w = *reinterpret_cast<const uint4 *>(wsrc + (size_t)pc * 16);
-          const uint32_t dst = sA + ab * GROUP * A_TILE_BYTES + row * 128 + ((j ^ (row & 7)) << 4);
-          st_shared_v4(dst, w.x, w.y, w.z, w.w);
-        }
-        fence_proxy_async_smem();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar_a_full + 8 * ab);
-        ++ag;
-      }
+      for (int k = 0; k < PIECES; ++k)
+        if (p_dst[k] != 0xffffffffu) x[k] = ld_shared_v4(sR + rs * RAW_STAGE_BYTES + 16 * (ctid + k * CONV_THREADS));
       const int st = i % NSTAGE;
       mbar_wait(bar_b_empty + 8 * st, ((i / NSTAGE) & 1) ^ 1);
       const uint32_t sdst = sB + st * B_STAGE_BYTES;
 #pragma unroll
       for (int k = 0; k < PIECES; ++k) {
-        if (p_t[k] < TILE_T) {
+        if (p_dst[k] != 0xffffffffu) {
           uint32_t h[8];
-          cvt_i8x4_f16x4(src[k].x, h[0], h[1]);
-          cvt_i8x4_f16x4(src[k].y, h[2], h[3]);
-          cvt_i8x4_f16x4(src[k].z, h[4], h[5]);
-          cvt_i8x4_f16x4(src[k].w, h[6], h[7]);
+          cvt_i8x4_f16x4(x[k].x, h[0], h[1]);
+          cvt_i8x4_f16x4(x[k].y, h[2], h[3]);
+          cvt_i8x4_f16x4(x[k].z, h[4], h[5]);
+          cvt_i8x4_f16x4(x[k].w, h[6], h[7]);
           st_shared_v4(sdst + p_dst[k], h[0], h[1], h[2], h[3]);
           st_shared_v4(sdst + (p_dst[k] ^ 16u), h[4], h[5], h[6], h[7]);
         }
       }
       fence_proxy_async_smem();
       __syncwarp();
-      if (lane == 0) mbar_arrive(bar_b_full + 8 * st);
-    };
-    // two register buffers, loads issued one tile ahead of their use
-    uint4 bufA[PIECES], bufB[PIECES];
-    Item itA = decode_item(it0, nG, nTt), itB;
-    if (n_items > 0) load_tile(bufA, itA);
-    for (int i = 0; i < n_items; i += 2) {
-      itB = itA; next_item(itB, nG, nTt);
-      if (i + 1 < n_items) load_tile(bufB, itB);
-      convert_tile(bufA, itA, i);
-      itA = itB; next_item(itA, nG, nTt);
-      if (i + 1 < n_items) {
-        if (i + 2 < n_items) load_tile(bufA, itA);
-        convert_tile(bufB, itB, i + 1);
+      if (lane == 0) {
+        mbar_arrive(bar_r_empty + 8 * rs);  // raw bytes are in registers / converted: slot may be refilled
+        mbar_arrive(bar_b_full + 8 * st);
       }
     }
-  } else if (lane == 0) {
-    // =========================================================================== MMA issue (one thread)
+  } else if (warp == MMA_WARP) {
+    // =========================================================================== MMA issue
+    // The whole warp walks the loop (all values warp-uniform); one elected lane issues tcgen05.
     constexpr uint32_t idesc = make_idesc_f16(BF_TILE_ROWS, TILE_T);
     int ag = 0, prev_c = -1, prev_g = -1, ab = 0, u = 0;
     Item it = decode_item(it0, nG, nTt);
     for (int i = 0; i < n_items; ++i, next_item(it, nG, nTt)) {
       if (it.c != prev_c || it.g != prev_g) {
-        if (ag > 0) tc_commit(bar_a_empty + 8 * ab);  // everything issued so far has left the old buffer
+        if (ag > 0 && elect_one()) tc_commit(bar_a_empty + 8 * ab);  // all MMAs so far have left the old buffer
+        __syncwarp();
         prev_c = it.c; prev_g = it.g;
         ab = ag & 1;
         mbar_wait(bar_a_full + 8 * ab, (ag >> 1) & 1);
@@ -296,7 +286,6 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
       }
       const int st = i % NSTAGE;
       mbar_wait(bar_b_full + 8 * st, (i / NSTAGE) & 1);
-      tc_fence_after();
       const int gm = min(GROUP, nMt - it.g * GROUP);
       const uint64_t bdesc = make_sdesc_k_sw128(sB + st * B_STAGE_BYTES);
       for (int m = 0; m < gm; ++m, ++u) {
@@ -305,11 +294,41 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         tc_fence_after();
         const uint64_t adesc = make_sdesc_k_sw128(sA + (ab * GROUP + m) * A_TILE_BYTES);
         const uint32_t d = tmem_base + acc * TILE_T;
-        for (int k = 0; k < nks; ++k)  // advance 16 fp16 = 32 bytes along K inside the swizzle atom
-          mma_f16_ss(d, adesc + 2 * k, bdesc + 2 * k, idesc, k > 0);
-        tc_commit(bar_t_full + 8 * acc);
+        if (elect_one()) {
+#pragma unroll
+          for (int k = 0; k < 4; ++k)  // advance 16 fp16 = 32 bytes along K inside the swizzle atom
+            if (k < nks) mma_f16_ss(d, adesc + 2 * k, bdesc + 2 * k, idesc, k > 0);
+          tc_commit(bar_t_full + 8 * acc);
+          if (m == gm - 1) tc_commit(bar_b_empty + 8 * st);
+        }
+        __syncwarp();
       }
-      tc_commit(bar_b_empty + 8 * st);
+    }
+  } else if (warp == TMA_WARP && lane == 0) {
+    // =========================================================================== bulk-copy producer (one thread)
+    const size_t row_bytes = (size_t)2 * p.nant;
+    const char *volt = reinterpret_cast<const char *>(p.volt);
+    int ag = 0, prev_c = -1, prev_g = -1;
+    Item it = decode_item(it0, nG, nTt);
+    for (int i = 0; i < n_items; ++i, next_item(it, nG, nTt)) {
+      if (it.c != prev_c || it.g != prev_g) {
+        // new (channel, beam group): its coefficient tiles (already the swizzled smem image) -> other A buffer
+        prev_c = it.c; prev_g = it.g;
+        const int ab = ag & 1;
+        mbar_wait(bar_a_empty + 8 * ab, ((ag >> 1) & 1) ^ 1);
+        const int gm = min(GROUP, nMt - it.g * GROUP);
+        const char *wsrc = reinterpret_cast<const char *>(p.wop) + ((size_t)it.c * nMt + (size_t)it.g * GROUP) * A_TILE_BYTES;
+        mbar_arrive_expect_tx(bar_a_full + 8 * ab, gm * A_TILE_BYTES);
+        bulk_g2s(sA + ab * GROUP * A_TILE_BYTES, wsrc, gm * A_TILE_BYTES, bar_a_full + 8 * ab);
+        ++ag;
+      }
+      const int rs = i % NRAW;
+      mbar_wait(bar_r_empty + 8 * rs, ((i / NRAW) & 1) ^ 1);
+      const int t_base = it.tt * TILE_T;
+      const int rows = min(TILE_T, p.nsamp - t_base);  // tail tile: the stale rest of the stage is finite
+      const uint32_t bytes = (uint32_t)(rows * row_bytes);  // int8 and only feeds bins >= nbin, never stored
+      mbar_arrive_expect_tx(bar_r_full + 8 * rs, bytes);
+      bulk_g2s(sR + rs * RAW_STAGE_BYTES, volt + ((size_t)it.c * p.nsamp + t_base) * row_bytes, bytes, bar_r_full + 8 * rs);
     }
   }
 
@@ -318,14 +337,14 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   if (warp == MMA_WARP) tmem_dealloc(tmem_base, 512);
 }
 
-template <int NINT_T, int GROUP, int NSTAGE, int CONV_WARPS>
+template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS>
 cudaError_t launch_k64(const BfParams &p, int sm_count, cudaStream_t st) {
   const int nG = (p.nMt + GROUP - 1) / GROUP;
   const int nTt = (p.nsamp + TILE_T - 1) / TILE_T;
   const long long total = (long long)p.nchan_run * nG * nTt;
   const int nks = (2 * p.nant + 15) / 16;
-  const size_t smem = 1024 + 2 * GROUP * A_TILE_BYTES + NSTAGE * B_STAGE_BYTES + 256;
-  auto kern = bf_umma_k64_kernel<NINT_T, GROUP, NSTAGE, CONV_WARPS>;
+  const size_t smem = 1024 + 2 * GROUP * A_TILE_BYTES + NSTAGE * B_STAGE_BYTES + NRAW * RAW_STAGE_BYTES + 256;
+  auto kern = bf_umma_k64_kernel<NINT_T, GROUP, NSTAGE, NRAW, CONV_WARPS>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   if (NINT_T == 0) {
@@ -333,14 +352,14 @@ cudaError_t launch_k64(const BfParams &p, int sm_count, cudaStream_t st) {
     if (e != cudaSuccess) return e;
   }
   const int grid = (int)(total < sm_count ? total : sm_count);
-  kern<<<grid, (EPI_WARPS + CONV_WARPS + 1) * 32, smem, st>>>(p, total, nG, nTt, nks);
+  kern<<<grid, (EPI_WARPS + CONV_WARPS + 2) * 32, smem, st>>>(p, total, nG, nTt, nks);
   return cudaGetLastError();
 }
 
 template <int NINT_T>
 cudaError_t launch_k64_nint(const BfParams &p, int sm_count, cudaStream_t st) {
-  if (p.nMt <= 2) return launch_k64<NINT_T, 2, 4, 8>(p, sm_count, st);
-  return launch_k64<NINT_T, 4, 3, 8>(p, sm_count, st);
+  if (p.nMt <= 2) return launch_k64<NINT_T, 2, 3, 4, 8>(p, sm_count, st);  // HBM/ingest-heavy: deep raw ring
+  return launch_k64<NINT_T, 4, 2, 2, 8>(p, sm_count, st);                  // many beams: MMA-bound, big A group
 }
 
 }  // namespace
@@ -349,8 +368,8 @@ bool bf_umma_supported(const bf_ctx *c, const char **why) {
   if (c->dtype != BF_CI8) { *why = "only complex int8 input so far"; return false; }
   if (c->nant % 8 != 0 || c->nant > 32) { *why = "needs nant in {8,16,24,32}"; return false; }
   const int I = c->nint;
-  const bool pow2_small = I <= 256 && (I & (I - 1)) == 0;
-  if (!pow2_small && I % 256 != 0) { *why = "needs nint a power of two <= 256 or a multiple of 256"; return false; }
+  const bool pow2_small = I <= 64 && (I & (I - 1)) == 0;
+  if (!pow2_small && I % 64 != 0) { *why = "needs nint a power of two <= 64 or a multiple of 64"; return false; }
   return true;
 }
 
@@ -364,8 +383,6 @@ cudaError_t bf_launch_umma(const BfParams &p, int dtype, int sm_count, cudaStrea
     case 16: return launch_k64_nint<16>(p, sm_count, st);
     case 32: return launch_k64_nint<32>(p, sm_count, st);
     case 64: return launch_k64_nint<64>(p, sm_count, st);
-    case 128: return launch_k64_nint<128>(p, sm_count, st);
-    case 256: return launch_k64_nint<256>(p, sm_count, st);
-    default: return launch_k64_nint<0>(p, sm_count, st);
+    default: return launch_k64_nint<0>(p, sm_count, st);  // multiples of 64: atomic partial sums
   }
 }

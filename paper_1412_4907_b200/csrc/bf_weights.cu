@@ -38,7 +38,7 @@ __global__ void bf_weights_kernel(const double *__restrict__ ant, const double *
     else           { a0 = (float)wim; a1 = (float)wre; }
   }
   int kb = (2 * n) / BF_KBLOCK, kk = (2 * n) % BF_KBLOCK;
-  size_t o = ((((size_t)c * nMt + mt) * nKb + kb) * BF_TILE_ROWS + r) * BF_KBLOCK + kk;
+  size_t o = (((size_t)c * nMt + mt) * nKb + kb) * (BF_TILE_ROWS * BF_KBLOCK) + bf_tile_off(r, kk);
   *reinterpret_cast<__half2 *>(wop + o) = __floats2half2_rn(a0, a1);
 }
 
@@ -63,9 +63,9 @@ __global__ void bf_decode_weights_kernel(const __half *__restrict__ wop, float *
   int c = (int)(t / nbeam);
   int mt = b / BF_TILE_BEAMS, bl = b % BF_TILE_BEAMS;
   int kb = (2 * n) / BF_KBLOCK, kk = (2 * n) % BF_KBLOCK;
-  size_t base = (((size_t)c * nMt + mt) * nKb + kb) * BF_TILE_ROWS;
-  float wre = __half2float(wop[(base + bf_beam_row(bl, 0)) * BF_KBLOCK + kk]);
-  float wim = __half2float(wop[(base + bf_beam_row(bl, 1)) * BF_KBLOCK + kk]);
+  size_t base = (((size_t)c * nMt + mt) * nKb + kb) * (BF_TILE_ROWS * BF_KBLOCK);
+  float wre = __half2float(wop[base + bf_tile_off(bf_beam_row(bl, 0), kk)]);
+  float wim = __half2float(wop[base + bf_tile_off(bf_beam_row(bl, 1), kk)]);
   out[2 * idx] = wre;
   out[2 * idx + 1] = wim;
 }
