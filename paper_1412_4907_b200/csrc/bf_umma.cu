@@ -272,37 +272,46 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   } else if (warp == MMA_WARP) {
     // =========================================================================== MMA issue
     // The whole warp walks the loop (all values warp-uniform); one elected lane issues tcgen05.
+    // This warp paces the tensor pipe (4 MMAs = 512 clk per accumulator tile), so its per-tile
+    // instruction path is kept minimal: wrap-around counters instead of div/mod, descriptors
+    // advanced by constant adds.
     constexpr uint32_t idesc = make_idesc_f16(BF_TILE_ROWS, TILE_T);
-    int ag = 0, prev_c = -1, prev_g = -1, ab = 0, u = 0;
+    const uint64_t adesc0 = make_sdesc_k_sw128(sA);
+    const uint64_t bdesc0 = make_sdesc_k_sw128(sB);
     Item it = decode_item(it0, nG, nTt);
-    for (int i = 0; i < n_items; ++i, next_item(it, nG, nTt)) {
-      if (it.c != prev_c || it.g != prev_g) {
+    int ag = 0, ab = 0;
+    int st = 0;                 // operand stage and the parity its "full" barrier completes next
+    uint32_t st_par = 0;
+    int acc = 0;                // accumulator stage; te_par bit a = parity of t_empty[a] to wait for
+    uint32_t te_par = 3;        // first use of a stage passes on the fresh barrier (parity 1)
+    int gm = min(GROUP, nMt - it.g * GROUP);
+    for (int i = 0; i < n_items; ++i) {
+      if (i == 0 || it.tt == 0) {  // (chan, beam group) changes exactly when the time tile wraps
         if (ag > 0 && elect_one()) tc_commit(bar_a_empty + 8 * ab);  // all MMAs so far have left the old buffer
-        __syncwarp();
-        prev_c = it.c; prev_g = it.g;
         ab = ag & 1;
+        gm = min(GROUP, nMt - it.g * GROUP);
         mbar_wait(bar_a_full + 8 * ab, (ag >> 1) & 1);
         ++ag;
       }
-      const int st = i % NSTAGE;
-      mbar_wait(bar_b_full + 8 * st, (i / NSTAGE) & 1);
-      const int gm = min(GROUP, nMt - it.g * GROUP);
-      const uint64_t bdesc = make_sdesc_k_sw128(sB + st * B_STAGE_BYTES);
-      for (int m = 0; m < gm; ++m, ++u) {
-        const int acc = u & 1;
-        mbar_wait(bar_t_empty + 8 * acc, ((u >> 1) & 1) ^ 1);
+      mbar_wait(bar_b_full + 8 * st, st_par);
+      const uint64_t bdesc = bdesc0 + (uint64_t)(st * (B_STAGE_BYTES >> 4));
+      for (int m = 0; m < gm; ++m) {
+        mbar_wait(bar_t_empty + 8 * acc, (te_par >> acc) & 1);
         tc_fence_after();
-        const uint64_t adesc = make_sdesc_k_sw128(sA + (ab * GROUP + m) * A_TILE_BYTES);
-        const uint32_t d = tmem_base + acc * TILE_T;
         if (elect_one()) {
+          const uint64_t adesc = adesc0 + (uint64_t)((ab * GROUP + m) * (A_TILE_BYTES >> 4));
+          const uint32_t d = tmem_base + acc * TILE_T;
 #pragma unroll
           for (int k = 0; k < 4; ++k)  // advance 16 fp16 = 32 bytes along K inside the swizzle atom
             if (k < nks) mma_f16_ss(d, adesc + 2 * k, bdesc + 2 * k, idesc, k > 0);
           tc_commit(bar_t_full + 8 * acc);
           if (m == gm - 1) tc_commit(bar_b_empty + 8 * st);
         }
-        __syncwarp();
+        te_par ^= 1u << acc;
+        acc ^= 1;
       }
+      if (++st == NSTAGE) { st = 0; st_par ^= 1; }
+      next_item(it, nG, nTt);
     }
   } else if (warp == TMA_WARP && lane == 0) {
     // =========================================================================== bulk-copy producer (one thread)
