@@ -66,7 +66,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE,
+                                          "-i", str(self.index), "-lms", "20"], stdout=subprocess.PIPE,
                                          stderr=subprocess.DEVNULL, text=True)
         except Exception:
             self.proc = None
@@ -101,7 +101,7 @@ class ClockSampler:
         return out
 
 
-def time_oracle_sample(w, v_host_fn, target_s=15.0, max_chan=64):
+def time_oracle_sample(w, v_host_fn, target_s=15.0, max_chan=1 << 30):
     """The oracle as it stands on the host cores, on whole channels of the workload; returns
     (TFLOP/s, cores, description).  v_host_fn(chan_list) -> numpy voltages of those channels."""
     import numpy as np
@@ -172,7 +172,7 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="medium")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
