@@ -67,3 +67,4 @@ cudaError_t bf_launch_decode_weights(const bf_ctx *c, float *d_out, cudaStream_t
 cudaError_t bf_launch_simt(const BfParams &p, int dtype, cudaStream_t st);
 bool bf_umma_supported(const bf_ctx *c, const char **why);
 cudaError_t bf_launch_umma(const BfParams &p, int dtype, int sm_count, cudaStream_t st);
+cudaError_t bf_launch_umma_kblock(const BfParams &p, int dtype, int sm_count, cudaStream_t st);

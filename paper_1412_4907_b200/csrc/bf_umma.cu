@@ -23,17 +23,13 @@
 // Pipelines (all mbarrier based): raw stages full/empty (TMA <-> convert), operand stages full/empty
 // (convert <-> MMA), coefficient buffers full/empty (TMA <-> MMA), TMEM accumulator stages full/empty
 // (MMA <-> epilogue).
-#include "bf_internal.h"
-#include "ptx.cuh"
+#include "bf_umma_common.cuh"
 
 namespace {
 
-constexpr int TILE_T = 256;                 // time samples per tile = UMMA N
-constexpr int EPI_WARPS = 16;
-constexpr int A_TILE_BYTES = BF_TILE_ROWS * 128;   // 128 rows x 64 fp16
-constexpr int B_STAGE_BYTES = TILE_T * 128;        // 256 rows x 64 fp16
+using namespace bfk;
+
 constexpr int MAX_INPUT_PIECES = TILE_T * 4;  // 16-byte input pieces per tile at nant = 32
-constexpr int RAW_STAGE_BYTES = TILE_T * 64;  // 256 time samples x 32 antennas x (re, im) int8
 
 struct Item { int c, g, tt; };
 
@@ -51,34 +47,6 @@ __device__ __forceinline__ void next_item(Item &it, int nG, int nTt) {
     it.tt = 0;
     if (++it.g == nG) { it.g = 0; ++it.c; }
   }
-}
-
-// int8 x4 (one 32-bit word) -> two half2, exact: 0x6400 | (x ^ 0x80) is the fp16 number 1024 + (x + 128)
-__device__ __forceinline__ void cvt_i8x4_f16x4(uint32_t w, uint32_t &lo, uint32_t &hi) {
-  const uint32_t u = w ^ 0x80808080u;
-  const uint32_t l = __byte_perm(u, 0x64646464u, 0x5140);
-  const uint32_t h = __byte_perm(u, 0x64646464u, 0x5342);
-  const __half2 bias = __halves2half2(__ushort_as_half(0x6480), __ushort_as_half(0x6480));  // 1152
-  __half2 a = __hsub2(*reinterpret_cast<const __half2 *>(&l), bias);
-  __half2 b = __hsub2(*reinterpret_cast<const __half2 *>(&h), bias);
-  lo = *reinterpret_cast<uint32_t *>(&a);
-  hi = *reinterpret_cast<uint32_t *>(&b);
-}
-
-__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
-  asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
-}
-__device__ __forceinline__ uint4 ld_shared_v4(uint32_t addr) {
-  uint4 r;
-  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
-  return r;
-}
-__device__ __forceinline__ uint4 ldg_nc_v4(const void *p) {
-  uint4 r;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
-               : "l"(p));
-  return r;
 }
 
 // NINT_T: integration length if it is a power of two <= 64; 0 = a larger multiple of 64 (each epilogue
@@ -135,16 +103,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     // The TMEM stage is handed back to the MMA thread as soon as this warp's last tcgen05.ld has
     // landed in registers -- the squaring of that last chunk, the shuffle and the store run in the
     // shadow of the next tile's MMAs.
-    constexpr int CPW = TILE_T / (EPI_WARPS / 4);                          // columns per warp (64)
-    constexpr int NCH = CPW / 32;                                          // 32-column chunks per warp
     const int quad = warp & 3, slot = warp >> 2;
-    const uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16) + slot * CPW;
-    constexpr int SUB = (NINT_T == 0 || NINT_T > 32) ? 32 : NINT_T;        // columns per partial sum
-    constexpr int NSUB = 32 / SUB;                                          // partial sums per chunk
-    constexpr int CPB = NINT_T == 0 ? NCH : (NINT_T <= 32 ? 1 : NINT_T / 32);  // chunks per bin
-    constexpr int BINS_PER_WARP = NINT_T == 0 ? 1 : CPW / NINT_T;
-    static_assert(NINT_T == 0 || (NINT_T <= CPW && CPW % NINT_T == 0), "bin must not straddle epilogue warps");
-    const bool vec_ok = (BINS_PER_WARP >= 4) && (p.nbin % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.pow) & 15) == 0);
     int u = 0;
     Item it = decode_item(it0, nG, nTt);
     for (int i = 0; i < n_items; ++i, next_item(it, nG, nTt)) {
@@ -153,72 +112,8 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         const int acc = u & 1;
         mbar_wait(bar_t_full + 8 * acc, (u >> 1) & 1);
         tc_fence_after();
-        const int mt = it.g * GROUP + m;
-        const int beam0 = mt * BF_TILE_BEAMS + quad * 16;
-        if (beam0 >= p.nbeam) {  // warp-uniform: this lane quadrant holds only padding rows
-          __syncwarp();
-          if (lane == 0) mbar_arrive(bar_t_empty + 8 * acc);
-          continue;
-        }
-        const int beam = beam0 + (lane & 15);
-        const bool writer = (lane < 16) && (beam < p.nbeam);
-        float *prow = p.pow + ((size_t)it.c * p.nbeam + beam) * p.nbin;
-        const int t_first = it.tt * TILE_T + slot * CPW;  // first time sample of this warp's columns
-        const int bin0 = NINT_T == 0 ? t_first / p.nint : t_first / (NINT_T == 0 ? 1 : NINT_T);
-        float binacc = 0.f;
-        float ob[4];
-#pragma unroll
-        for (int ch = 0; ch < NCH; ++ch) {
-          uint32_t v[32];
-          BF_TMEM_LD_32x32b_X32(t_lane + acc * TILE_T + 32 * ch, v);
-          tc_wait_ld();
-          if (ch == NCH - 1) {  // all of this warp's columns are in registers: release the stage
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar_t_empty + 8 * acc);
-          }
-#pragma unroll
-          for (int s = 0; s < NSUB; ++s) {
-            float sum;
-            if constexpr (SUB == 1) {
-              const float d = __uint_as_float(v[s]);
-              sum = d * d;
-            } else {
-              constexpr int NACC = SUB >= 8 ? 4 : SUB / 2;
-              float2 a[NACC];
-#pragma unroll
-              for (int q = 0; q < NACC; ++q) a[q] = make_float2(0.f, 0.f);
-#pragma unroll
-              for (int j = 0; j < SUB / 2; ++j) {
-                const float2 d = make_float2(__uint_as_float(v[s * SUB + 2 * j]), __uint_as_float(v[s * SUB + 2 * j + 1]));
-                a[j % NACC] = ffma2(d, d, a[j % NACC]);
-              }
-              sum = 0.f;
-#pragma unroll
-              for (int q = 0; q < NACC; ++q) sum += a[q].x + a[q].y;
-            }
-            if (CPB > 1) {
-              binacc += sum;
-              if ((ch + 1) % CPB != 0) continue;
-              sum = binacc;
-              binacc = 0.f;
-            }
-            const float tot = sum + __shfl_xor_sync(0xffffffffu, sum, 16);  // re^2 rows + im^2 rows
-            if (NINT_T == 0) {
-              if (writer && t_first < p.nsamp) atomicAdd(prow + bin0, tot);
-            } else {
-              const int jb = (ch / CPB) * NSUB + s;  // bin index inside this warp's columns (compile-time)
-              const int j = bin0 + jb;
-              if (vec_ok) {
-                ob[jb & 3] = tot;
-                if ((jb & 3) == 3 && writer && j < p.nbin)
-                  *reinterpret_cast<float4 *>(prow + j - 3) = make_float4(ob[0], ob[1], ob[2], ob[3]);
-              } else if (writer && j < p.nbin) {
-                prow[j] = tot;
-              }
-            }
-          }
-        }
+        epilogue_tile<NINT_T>(p, tmem_base, acc * TILE_T, quad, slot, lane, it.c, it.g * GROUP + m, it.tt,
+                              bar_t_empty + 8 * acc);
       }
     }
   } else if (warp < MMA_WARP) {
@@ -244,24 +139,10 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
       const int rs = i % NRAW;
       mbar_wait(bar_r_full + 8 * rs, (i / NRAW) & 1);
       uint4 x[PIECES];
-#pragma unroll
-      for (int k = 0; k < PIECES; ++k)
-        if (p_dst[k] != 0xffffffffu) x[k] = ld_shared_v4(sR + rs * RAW_STAGE_BYTES + 16 * (ctid + k * CONV_THREADS));
+      convert_load<PIECES, CONV_THREADS>(sR + rs * RAW_STAGE_BYTES, ctid, p_dst, x);
       const int st = i % NSTAGE;
       mbar_wait(bar_b_empty + 8 * st, ((i / NSTAGE) & 1) ^ 1);
-      const uint32_t sdst = sB + st * B_STAGE_BYTES;
-#pragma unroll
-      for (int k = 0; k < PIECES; ++k) {
-        if (p_dst[k] != 0xffffffffu) {
-          uint32_t h[8];
-          cvt_i8x4_f16x4(x[k].x, h[0], h[1]);
-          cvt_i8x4_f16x4(x[k].y, h[2], h[3]);
-          cvt_i8x4_f16x4(x[k].z, h[4], h[5]);
-          cvt_i8x4_f16x4(x[k].w, h[6], h[7]);
-          st_shared_v4(sdst + p_dst[k], h[0], h[1], h[2], h[3]);
-          st_shared_v4(sdst + (p_dst[k] ^ 16u), h[4], h[5], h[6], h[7]);
-        }
-      }
+      convert_store<PIECES>(sB + st * B_STAGE_BYTES, p_dst, x);
       fence_proxy_async_smem();
       __syncwarp();
       if (lane == 0) {
@@ -373,16 +254,24 @@ cudaError_t launch_k64_nint(const BfParams &p, int sm_count, cudaStream_t st) {
 
 }  // namespace
 
+static bool nint_ok(int I) { return (I <= 64 && (I & (I - 1)) == 0) || I % 64 == 0; }
+
+// which tensor-core kernel takes this shape: 1 = coefficients-resident (2*nant <= 64, int8), 2 = K-blocked
+static int umma_variant(int dtype, int nant) {
+  if (dtype == BF_CI8 && nant % 8 == 0 && nant <= 32) return 1;
+  if (dtype == BF_CI8 && nant % 8 == 0) return 2;   // TMA rows must be multiples of 16 bytes
+  if (dtype == BF_CF16 && nant % 4 == 0) return 2;
+  return 0;
+}
+
 bool bf_umma_supported(const bf_ctx *c, const char **why) {
-  if (c->dtype != BF_CI8) { *why = "only complex int8 input so far"; return false; }
-  if (c->nant % 8 != 0 || c->nant > 32) { *why = "needs nant in {8,16,24,32}"; return false; }
-  const int I = c->nint;
-  const bool pow2_small = I <= 64 && (I & (I - 1)) == 0;
-  if (!pow2_small && I % 64 != 0) { *why = "needs nint a power of two <= 64 or a multiple of 64"; return false; }
+  if (!umma_variant(c->dtype, c->nant)) { *why = "needs nant % 8 == 0 (int8) or nant % 4 == 0 (fp16)"; return false; }
+  if (!nint_ok(c->nint)) { *why = "needs nint a power of two <= 64 or a multiple of 64"; return false; }
   return true;
 }
 
 cudaError_t bf_launch_umma(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
+  if (umma_variant(dtype, p.nant) == 2) return bf_launch_umma_kblock(p, dtype, sm_count, st);
   if (dtype != BF_CI8) return cudaErrorNotSupported;
   switch (p.nint) {
     case 1: return launch_k64_nint<1>(p, sm_count, st);

@@ -1,0 +1,147 @@
+// bf_umma_common.cuh -- pieces shared by the two tensor-core kernels (bf_umma.cu: coefficients resident,
+// 2*nant <= 64; bf_umma_kblock.cu: K-blocked, any nant): the int8 -> fp16 converter and the fused
+// |.|^2 + integrate epilogue (hot-path rows a4, a5).
+#pragma once
+#include "bf_internal.h"
+#include "ptx.cuh"
+
+namespace bfk {
+
+constexpr int TILE_T = 256;                        // time samples per tile = UMMA N
+constexpr int EPI_WARPS = 16;
+constexpr int A_TILE_BYTES = BF_TILE_ROWS * 128;   // 128 rows x 64 fp16
+constexpr int B_STAGE_BYTES = TILE_T * 128;        // 256 rows x 64 fp16
+constexpr int RAW_STAGE_BYTES = TILE_T * 64;       // 256 time samples x 64 int8 (32 antennas x (re, im))
+
+// int8 x4 (one 32-bit word) -> two half2, exact: 0x6400 | (x ^ 0x80) is the fp16 number 1024 + (x + 128)
+__device__ __forceinline__ void cvt_i8x4_f16x4(uint32_t w, uint32_t &lo, uint32_t &hi) {
+  const uint32_t u = w ^ 0x80808080u;
+  const uint32_t l = __byte_perm(u, 0x64646464u, 0x5140);
+  const uint32_t h = __byte_perm(u, 0x64646464u, 0x5342);
+  const __half2 bias = __halves2half2(__ushort_as_half(0x6480), __ushort_as_half(0x6480));  // 1152
+  __half2 a = __hsub2(*reinterpret_cast<const __half2 *>(&l), bias);
+  __half2 b = __hsub2(*reinterpret_cast<const __half2 *>(&h), bias);
+  lo = *reinterpret_cast<uint32_t *>(&a);
+  hi = *reinterpret_cast<uint32_t *>(&b);
+}
+
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ uint4 ld_shared_v4(uint32_t addr) {
+  uint4 r;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
+  return r;
+}
+
+// raw int8 stage (256 rows x 64 bytes, compact) -> fp16 operand stage (256 rows x 128 bytes, 128-byte
+// swizzle).  PIECES 16-byte input pieces per thread; piece pc = tid + k*NTHREADS covers row pc/4,
+// bytes 16*(pc%4)..  p_dst[k] = byte offset of its first output chunk (0xffffffff = not mine).
+template <int PIECES, int NTHREADS>
+__device__ __forceinline__ void convert_load(uint32_t s_raw, int tid, const uint32_t (&p_dst)[PIECES], uint4 (&x)[PIECES]) {
+#pragma unroll
+  for (int k = 0; k < PIECES; ++k)
+    if (p_dst[k] != 0xffffffffu) x[k] = ld_shared_v4(s_raw + 16 * (tid + k * NTHREADS));
+}
+template <int PIECES>
+__device__ __forceinline__ void convert_store(uint32_t s_dst, const uint32_t (&p_dst)[PIECES], const uint4 (&x)[PIECES]) {
+#pragma unroll
+  for (int k = 0; k < PIECES; ++k) {
+    if (p_dst[k] != 0xffffffffu) {
+      uint32_t h[8];
+      cvt_i8x4_f16x4(x[k].x, h[0], h[1]);
+      cvt_i8x4_f16x4(x[k].y, h[2], h[3]);
+      cvt_i8x4_f16x4(x[k].z, h[4], h[5]);
+      cvt_i8x4_f16x4(x[k].w, h[6], h[7]);
+      st_shared_v4(s_dst + p_dst[k], h[0], h[1], h[2], h[3]);
+      st_shared_v4(s_dst + (p_dst[k] ^ 16u), h[4], h[5], h[6], h[7]);
+    }
+  }
+}
+
+// Epilogue of ONE accumulator tile (128 TMEM lanes x 256 columns at column `acc_col`) for ONE warp of
+// the 16: lanes 32*quad.., columns 64*slot...  Rows: lane l < 16 is the re row, lane l+16 the im row of
+// beam 64*mt + 16*quad + l.  The TMEM stage is handed back (arrive on bar_empty) as soon as this warp's
+// last tcgen05.ld has landed; squaring, shuffle and store run in the shadow of the next MMAs.
+// NINT_T: integration length if a power of two <= 64; 0 = a larger multiple of 64 (the partial sum of
+// the warp's 64 columns is added atomically into a zeroed output).
+template <int NINT_T>
+__device__ __forceinline__ void epilogue_tile(const BfParams &p, uint32_t tmem_base, uint32_t acc_col, int quad, int slot,
+                                              int lane, int c, int mt, int tt, uint32_t bar_empty) {
+  constexpr int CPW = TILE_T / (EPI_WARPS / 4);                          // columns per warp (64)
+  constexpr int NCH = CPW / 32;                                          // 32-column chunks per warp
+  constexpr int SUB = (NINT_T == 0 || NINT_T > 32) ? 32 : NINT_T;        // columns per partial sum
+  constexpr int NSUB = 32 / SUB;                                          // partial sums per chunk
+  constexpr int CPB = NINT_T == 0 ? NCH : (NINT_T <= 32 ? 1 : NINT_T / 32);  // chunks per bin
+  constexpr int BINS_PER_WARP = NINT_T == 0 ? 1 : CPW / NINT_T;
+  static_assert(NINT_T == 0 || (NINT_T <= CPW && CPW % (NINT_T == 0 ? 1 : NINT_T) == 0), "bin must not straddle epilogue warps");
+  const int beam0 = mt * BF_TILE_BEAMS + quad * 16;
+  if (beam0 >= p.nbeam) {  // warp-uniform: this lane quadrant holds only padding rows
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_empty);
+    return;
+  }
+  const bool vec_ok = (BINS_PER_WARP >= 4) && (p.nbin % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.pow) & 15) == 0);
+  const uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16) + acc_col + slot * CPW;
+  const int beam = beam0 + (lane & 15);
+  const bool writer = (lane < 16) && (beam < p.nbeam);
+  float *prow = p.pow + ((size_t)c * p.nbeam + beam) * p.nbin;
+  const int t_first = tt * TILE_T + slot * CPW;  // first time sample of this warp's columns
+  const int bin0 = NINT_T == 0 ? t_first / p.nint : t_first / (NINT_T == 0 ? 1 : NINT_T);
+  float binacc = 0.f;
+  float ob[4];
+#pragma unroll
+  for (int ch = 0; ch < NCH; ++ch) {
+    uint32_t v[32];
+    BF_TMEM_LD_32x32b_X32(t_lane + 32 * ch, v);
+    tc_wait_ld();
+    if (ch == NCH - 1) {  // all of this warp's columns are in registers: release the stage
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_empty);
+    }
+#pragma unroll
+    for (int s = 0; s < NSUB; ++s) {
+      float sum;
+      if constexpr (SUB == 1) {
+        const float d = __uint_as_float(v[s]);
+        sum = d * d;
+      } else {
+        constexpr int NACC = SUB >= 8 ? 4 : SUB / 2;
+        float2 a[NACC];
+#pragma unroll
+        for (int q = 0; q < NACC; ++q) a[q] = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int j = 0; j < SUB / 2; ++j) {
+          const float2 d = make_float2(__uint_as_float(v[s * SUB + 2 * j]), __uint_as_float(v[s * SUB + 2 * j + 1]));
+          a[j % NACC] = ffma2(d, d, a[j % NACC]);
+        }
+        sum = 0.f;
+#pragma unroll
+        for (int q = 0; q < NACC; ++q) sum += a[q].x + a[q].y;
+      }
+      if (CPB > 1) {
+        binacc += sum;
+        if ((ch + 1) % CPB != 0) continue;
+        sum = binacc;
+        binacc = 0.f;
+      }
+      const float tot = sum + __shfl_xor_sync(0xffffffffu, sum, 16);  // re^2 rows + im^2 rows
+      if (NINT_T == 0) {
+        if (writer && t_first < p.nsamp) atomicAdd(prow + bin0, tot);
+      } else {
+        const int jb = (ch / CPB) * NSUB + s;  // bin index inside this warp's columns (compile-time)
+        const int j = bin0 + jb;
+        if (vec_ok) {
+          ob[jb & 3] = tot;
+          if ((jb & 3) == 3 && writer && j < p.nbin)
+            *reinterpret_cast<float4 *>(prow + j - 3) = make_float4(ob[0], ob[1], ob[2], ob[3]);
+        } else if (writer && j < p.nbin) {
+          prow[j] = tot;
+        }
+      }
+    }
+  }
+}
+
+}  // namespace bfk

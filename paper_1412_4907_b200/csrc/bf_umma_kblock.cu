@@ -1,0 +1,276 @@
+// bf_umma_kblock.cu -- the fused tensor-core beamformer for larger arrays (any nant that is a multiple
+// of 8 (int8) / 4 (fp16)): hot-path rows a2..a5 with the contraction K-blocked.
+//
+// Per channel the contraction is a real GEMM  D[2B rows][T] = A[2B][K'] X'[T][K']^T, K' = 2*nant
+// (the (re, -im)/(im, re) row expansion is described in bf_internal.h).  Neither operand
+// fits in shared memory any more, so both stream in K-blocks of 64:
+//   * coefficient tiles (128 rows x 64, pre-swizzled in HBM) by cp.async.bulk, two M-tiles (128 beams)
+//     per stage -- every voltage K-block is used for both before it is released;
+//   * voltage K-blocks (256 samples x 64) by a 3-D TMA tensor copy: fp16 input lands directly in the
+//     128-byte-swizzled operand layout; int8 input lands raw and the convert warps rewrite it as fp16
+//     (the paper's in-kernel unpack).
+// The two accumulators (2 x 256 TMEM columns) are drained by the same fused |.|^2 + integrate
+// epilogue as the small-array kernel once the last K-block has been issued.
+//
+// Work item = (channel, time tile, beam-group of 128 beams), beam group fastest, so the same CTA reads
+// a voltage tile for consecutive beam groups while it is still in L2.
+#include <cuda.h>
+
+#include "bf_umma_common.cuh"
+
+namespace {
+
+using namespace bfk;
+
+constexpr int KB_GROUP = 2;                        // M-tiles (of 64 beams) per item
+constexpr int CONV_WARPS = 8;
+constexpr int CONV_THREADS = CONV_WARPS * 32;
+constexpr int MMA_WARP = EPI_WARPS + CONV_WARPS;
+constexpr int TMA_WARP = MMA_WARP + 1;
+constexpr int NTHREADS = (EPI_WARPS + CONV_WARPS + 2) * 32;
+constexpr int A_STAGE_BYTES = KB_GROUP * A_TILE_BYTES;
+
+struct KItem { int c, tt, g; };
+__device__ __forceinline__ KItem kdecode(long long idx, int nG, int nTt) {
+  KItem it;
+  it.g = (int)(idx % nG);
+  long long ct = idx / nG;
+  it.tt = (int)(ct % nTt);
+  it.c = (int)(ct / nTt);
+  return it;
+}
+__device__ __forceinline__ void knext(KItem &it, int nG, int nTt) {
+  if (++it.g == nG) {
+    it.g = 0;
+    if (++it.tt == nTt) { it.tt = 0; ++it.c; }
+  }
+}
+
+template <int NINT_T, bool IS_F16, int NA, int NB, int NR>
+__global__ void __launch_bounds__(NTHREADS, 1)
+bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, const long long total_items,
+                      const int nG, const int nTt) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sA = smem_base;                              // NA stages x 2 coefficient tiles
+  const uint32_t sB = sA + NA * A_STAGE_BYTES;                // NB fp16 operand stages
+  const uint32_t sR = sB + NB * B_STAGE_BYTES;                // NR raw int8 stages (int8 input only)
+  const uint32_t sBar = sR + NR * RAW_STAGE_BYTES;
+  const uint32_t bar_a_full = sBar, bar_a_empty = bar_a_full + 8 * NA;
+  const uint32_t bar_b_full = bar_a_empty + 8 * NA, bar_b_empty = bar_b_full + 8 * NB;
+  const uint32_t bar_r_full = bar_b_empty + 8 * NB, bar_r_empty = bar_r_full + 8 * (NR + 1);
+  const uint32_t bar_t_full = bar_r_empty + 8 * (NR + 1), bar_t_empty = bar_t_full + 16;
+  const uint32_t s_tmem = bar_t_empty + 16;
+
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < NA; ++s) { mbar_init(bar_a_full + 8 * s, 1); mbar_init(bar_a_empty + 8 * s, 1); }
+    for (int s = 0; s < NB; ++s) { mbar_init(bar_b_full + 8 * s, IS_F16 ? 1 : CONV_WARPS); mbar_init(bar_b_empty + 8 * s, 1); }
+    for (int s = 0; s < NR; ++s) { mbar_init(bar_r_full + 8 * s, 1); mbar_init(bar_r_empty + 8 * s, CONV_WARPS); }
+    for (int s = 0; s < 2; ++s) { mbar_init(bar_t_full + 8 * s, 1); mbar_init(bar_t_empty + 8 * s, EPI_WARPS); }
+    fence_barrier_init();
+  }
+  if (warp == MMA_WARP) tmem_alloc(s_tmem, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(s_tmem));
+  tmem_base = __shfl_sync(0xffffffffu, tmem_base, 0);
+
+  const long long it0 = total_items * blockIdx.x / gridDim.x;
+  const long long it1 = total_items * (blockIdx.x + 1) / gridDim.x;
+  const int n_items = (int)(it1 - it0);
+  const int nMt = p.nMt, nKb = p.nKb;
+
+  if (warp < EPI_WARPS) {
+    // =========================================================================== epilogue
+    const int quad = warp & 3, slot = warp >> 2;
+    KItem it = kdecode(it0, nG, nTt);
+    uint32_t tpar = 0;  // bit m: parity of the next completion of t_full[m] (an odd last group skips m = 1)
+    for (int i = 0; i < n_items; ++i, knext(it, nG, nTt)) {
+      const int gm = min(KB_GROUP, nMt - it.g * KB_GROUP);
+      for (int m = 0; m < gm; ++m) {
+        mbar_wait(bar_t_full + 8 * m, (tpar >> m) & 1);
+        tpar ^= 1u << m;
+        tc_fence_after();
+        epilogue_tile<NINT_T>(p, tmem_base, m * TILE_T, quad, slot, lane, it.c, it.g * KB_GROUP + m, it.tt,
+                              bar_t_empty + 8 * m);
+      }
+    }
+  } else if (warp < MMA_WARP) {
+    // =========================================================================== convert (int8 input only)
+    if (!IS_F16) {
+      constexpr int PIECES = (TILE_T * 4) / CONV_THREADS;
+      const int ctid = threadIdx.x - EPI_WARPS * 32;
+      uint32_t p_dst[PIECES];
+#pragma unroll
+      for (int k = 0; k < PIECES; ++k) {
+        const int pc = ctid + k * CONV_THREADS;
+        const int t = pc >> 2, q = pc & 3;
+        p_dst[k] = (uint32_t)((t >> 3) * 1024 + (t & 7) * 128 + (((2 * q) ^ (t & 7)) << 4));
+      }
+      const long long nblk = (long long)n_items * nKb;
+      int rs = 0, bs = 0;
+      uint32_t rpar = 0, bpar = 1;
+      for (long long j = 0; j < nblk; ++j) {
+        mbar_wait(bar_r_full + 8 * rs, rpar);
+        uint4 x[PIECES];
+        convert_load<PIECES, CONV_THREADS>(sR + rs * RAW_STAGE_BYTES, ctid, p_dst, x);
+        mbar_wait(bar_b_empty + 8 * bs, bpar);
+        convert_store<PIECES>(sB + bs * B_STAGE_BYTES, p_dst, x);
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(bar_r_empty + 8 * rs);
+          mbar_arrive(bar_b_full + 8 * bs);
+        }
+        if (++rs == NR) { rs = 0; rpar ^= 1; }
+        if (++bs == NB) { bs = 0; bpar ^= 1; }
+      }
+    }
+  } else if (warp == MMA_WARP) {
+    // =========================================================================== MMA issue
+    constexpr uint32_t idesc = make_idesc_f16(BF_TILE_ROWS, TILE_T);
+    const uint64_t adesc0 = make_sdesc_k_sw128(sA);
+    const uint64_t bdesc0 = make_sdesc_k_sw128(sB);
+    KItem it = kdecode(it0, nG, nTt);
+    int sa = 0, sb = 0;
+    uint32_t apar = 0, bpar = 0, tpar = 3;
+    for (int i = 0; i < n_items; ++i, knext(it, nG, nTt)) {
+      const int gm = min(KB_GROUP, nMt - it.g * KB_GROUP);
+      // the accumulators must have been drained (first use: fresh barriers pass on parity 1)
+      for (int m = 0; m < gm; ++m) { mbar_wait(bar_t_empty + 8 * m, (tpar >> m) & 1); tpar ^= 1u << m; }
+      tc_fence_after();
+      for (int kb = 0; kb < nKb; ++kb) {
+        mbar_wait(bar_a_full + 8 * sa, apar);
+        mbar_wait(bar_b_full + 8 * sb, bpar);
+        tc_fence_after();
+        if (elect_one()) {
+          const uint64_t bdesc = bdesc0 + (uint64_t)(sb * (B_STAGE_BYTES >> 4));
+          for (int m = 0; m < gm; ++m) {
+            const uint64_t adesc = adesc0 + (uint64_t)((sa * KB_GROUP + m) * (A_TILE_BYTES >> 4));
+            const uint32_t d = tmem_base + m * TILE_T;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) mma_f16_ss(d, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+          }
+          tc_commit(bar_a_empty + 8 * sa);
+          tc_commit(bar_b_empty + 8 * sb);
+          if (kb == nKb - 1)
+            for (int m = 0; m < gm; ++m) tc_commit(bar_t_full + 8 * m);
+        }
+        __syncwarp();
+        if (++sa == NA) { sa = 0; apar ^= 1; }
+        if (++sb == NB) { sb = 0; bpar ^= 1; }
+      }
+    }
+  } else if (warp == TMA_WARP && lane == 0) {
+    // =========================================================================== TMA producer (one thread)
+    tma_prefetch_desc(&tmap);
+    KItem it = kdecode(it0, nG, nTt);
+    int sa = 0, sv = 0;  // sv: voltage stage (operand stage for fp16, raw stage for int8)
+    uint32_t apar = 1, vpar = 1;
+    constexpr int NV = IS_F16 ? NB : NR;
+    constexpr uint32_t VBYTES = IS_F16 ? B_STAGE_BYTES : RAW_STAGE_BYTES;
+    const uint32_t sV = IS_F16 ? sB : sR;
+    const uint32_t bar_v_full = IS_F16 ? bar_b_full : bar_r_full, bar_v_empty = IS_F16 ? bar_b_empty : bar_r_empty;
+    for (int i = 0; i < n_items; ++i, knext(it, nG, nTt)) {
+      const int gm = min(KB_GROUP, nMt - it.g * KB_GROUP);
+      for (int kb = 0; kb < nKb; ++kb) {
+        mbar_wait(bar_a_empty + 8 * sa, apar);
+        mbar_arrive_expect_tx(bar_a_full + 8 * sa, gm * A_TILE_BYTES);
+        for (int m = 0; m < gm; ++m) {
+          const char *src = reinterpret_cast<const char *>(p.wop) +
+                            (((size_t)it.c * nMt + (size_t)(it.g * KB_GROUP + m)) * nKb + kb) * A_TILE_BYTES;
+          bulk_g2s(sA + (sa * KB_GROUP + m) * A_TILE_BYTES, src, A_TILE_BYTES, bar_a_full + 8 * sa);
+        }
+        mbar_wait(bar_v_empty + 8 * sv, vpar);
+        mbar_arrive_expect_tx(bar_v_full + 8 * sv, VBYTES);
+        tma_load_3d(sV + sv * VBYTES, &tmap, kb * BF_KBLOCK, it.tt * TILE_T, it.c, bar_v_full + 8 * sv);
+        if (++sa == NA) { sa = 0; apar ^= 1; }
+        if (++sv == NV) { sv = 0; vpar ^= 1; }
+      }
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == MMA_WARP) tmem_dealloc(tmem_base, 512);
+}
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+PFN_encodeTiled get_encode() {
+  static PFN_encodeTiled fn = nullptr;
+  if (!fn) {
+    void *ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<PFN_encodeTiled>(ptr);
+  }
+  return fn;
+}
+
+// 3-D view of the voltages: {K' elements, nsamp, nchan}, box {64, 256, 1}
+cudaError_t make_tmap(CUtensorMap *tm, const BfParams &p, int dtype) {
+  PFN_encodeTiled enc = get_encode();
+  if (!enc) return cudaErrorNotSupported;
+  const bool f16 = dtype == BF_CF16;
+  const cuuint64_t esz = f16 ? 2 : 1;
+  cuuint64_t dims[3] = {(cuuint64_t)2 * p.nant, (cuuint64_t)p.nsamp, (cuuint64_t)p.nchan_run};
+  cuuint64_t strides[2] = {dims[0] * esz, dims[0] * esz * (cuuint64_t)p.nsamp};
+  cuuint32_t box[3] = {BF_KBLOCK, (cuuint32_t)TILE_T, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = enc(tm, f16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8, 3,
+                   const_cast<void *>(p.volt), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   f16 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+template <int NINT_T, bool IS_F16>
+cudaError_t launch_kb(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
+  constexpr int NA = 3, NB = IS_F16 ? 3 : 2, NR = IS_F16 ? 0 : 3;
+  CUtensorMap tm;
+  cudaError_t e = make_tmap(&tm, p, dtype);
+  if (e != cudaSuccess) return e;
+  const int nG = (p.nMt + KB_GROUP - 1) / KB_GROUP;
+  const int nTt = (p.nsamp + TILE_T - 1) / TILE_T;
+  const long long total = (long long)p.nchan_run * nTt * nG;
+  const size_t smem = 1024 + NA * A_STAGE_BYTES + NB * B_STAGE_BYTES + NR * RAW_STAGE_BYTES + 512;
+  auto kern = bf_umma_kblock_kernel<NINT_T, IS_F16, NA, NB, NR>;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  if (NINT_T == 0) {
+    e = cudaMemsetAsync(p.pow, 0, (size_t)p.nchan_run * p.nbeam * p.nbin * sizeof(float), st);
+    if (e != cudaSuccess) return e;
+  }
+  const int grid = (int)(total < sm_count ? total : sm_count);
+  kern<<<grid, NTHREADS, smem, st>>>(p, tm, total, nG, nTt);
+  return cudaGetLastError();
+}
+
+template <bool IS_F16>
+cudaError_t launch_kb_nint(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
+  switch (p.nint) {
+    case 1: return launch_kb<1, IS_F16>(p, dtype, sm_count, st);
+    case 2: return launch_kb<2, IS_F16>(p, dtype, sm_count, st);
+    case 4: return launch_kb<4, IS_F16>(p, dtype, sm_count, st);
+    case 8: return launch_kb<8, IS_F16>(p, dtype, sm_count, st);
+    case 16: return launch_kb<16, IS_F16>(p, dtype, sm_count, st);
+    case 32: return launch_kb<32, IS_F16>(p, dtype, sm_count, st);
+    case 64: return launch_kb<64, IS_F16>(p, dtype, sm_count, st);
+    default: return launch_kb<0, IS_F16>(p, dtype, sm_count, st);
+  }
+}
+
+}  // namespace
+
+cudaError_t bf_launch_umma_kblock(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
+  if (dtype == BF_CF16) return launch_kb_nint<true>(p, dtype, sm_count, st);
+  return launch_kb_nint<false>(p, dtype, sm_count, st);
+}

@@ -40,6 +40,16 @@ BF_DEVI void bulk_g2s(uint32_t dst_smem, const void *src_gmem, uint32_t bytes, u
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(dst_smem), "l"(src_gmem), "r"(bytes), "r"(bar) : "memory");
 }
+// TMA tiled tensor copy (3-D): global -> shared through a CUtensorMap; out-of-bounds elements are
+// zero-filled, the full box is counted on the mbarrier.  SASS: UTMALDG.
+BF_DEVI void tma_load_3d(uint32_t dst_smem, const void *tmap, int x, int y, int z, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+      ::"r"(dst_smem), "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(bar) : "memory");
+}
+BF_DEVI void tma_prefetch_desc(const void *tmap) {
+  asm volatile("prefetch.tensormap [%0];" ::"l"(tmap) : "memory");
+}
 BF_DEVI bool mbar_try_wait(uint32_t bar, uint32_t parity) {
   uint32_t ok;
   asm volatile(
