@@ -18,7 +18,7 @@
 // Warp roles (one CTA per SM, persistent over a contiguous range of (chan, beam group, time tile)):
 //   warps 0-15  epilogue: warp w owns TMEM lanes 32*(w&3).. and columns 64*(w>>2).. of every tile
 //   warps 16..  convert (CONV_WARPS): raw int8 stage -> fp16 operand stage
-//   next warp   TMEM allocation + the single MMA-issuing thread
+//   next 2      MMA issue, one warp (one elected lane) per TMEM accumulator stage; TMEM allocation
 //   last warp   one thread issuing the bulk copies (voltage tiles; coefficient tiles on channel change)
 // Pipelines (all mbarrier based): raw stages full/empty (TMA <-> convert), operand stages full/empty
 // (convert <-> MMA), coefficient buffers full/empty (TMA <-> MMA), TMEM accumulator stages full/empty
@@ -52,12 +52,12 @@ __device__ __forceinline__ void next_item(Item &it, int nG, int nTt) {
 // NINT_T: integration length if it is a power of two <= 64; 0 = a larger multiple of 64 (each epilogue
 // warp adds the partial sum of its 64 columns atomically into a zeroed output).
 template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS>
-__global__ void __launch_bounds__((EPI_WARPS + CONV_WARPS + 2) * 32, 1)
+__global__ void __launch_bounds__((EPI_WARPS + CONV_WARPS + 3) * 32, 1)
 bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, const int nTt, const int nks) {
   extern __shared__ uint8_t smem_raw[];
   constexpr int CONV_THREADS = CONV_WARPS * 32;
   constexpr int MMA_WARP = EPI_WARPS + CONV_WARPS;
-  constexpr int TMA_WARP = MMA_WARP + 1;
+  constexpr int TMA_WARP = MMA_WARP + 2;  // two MMA-issuing warps, one per accumulator stage
 
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sA = smem_base;                                  // 2 buffers x GROUP coefficient tiles
@@ -75,10 +75,10 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < NSTAGE; ++s) { mbar_init(bar_b_full + 8 * s, CONV_WARPS); mbar_init(bar_b_empty + 8 * s, 1); }
+    for (int s = 0; s < NSTAGE; ++s) { mbar_init(bar_b_full + 8 * s, CONV_WARPS); mbar_init(bar_b_empty + 8 * s, 2); }
     for (int s = 0; s < NRAW; ++s) { mbar_init(bar_r_full + 8 * s, 1); mbar_init(bar_r_empty + 8 * s, CONV_WARPS); }
     for (int s = 0; s < 2; ++s) {
-      mbar_init(bar_a_full + 8 * s, 1); mbar_init(bar_a_empty + 8 * s, 1);
+      mbar_init(bar_a_full + 8 * s, 1); mbar_init(bar_a_empty + 8 * s, 2);
       mbar_init(bar_t_full + 8 * s, 1);          mbar_init(bar_t_empty + 8 * s, EPI_WARPS);
     }
     fence_barrier_init();
@@ -150,47 +150,55 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         mbar_arrive(bar_b_full + 8 * st);
       }
     }
-  } else if (warp == MMA_WARP) {
-    // =========================================================================== MMA issue
-    // The whole warp walks the loop (all values warp-uniform); one elected lane issues tcgen05.
-    // This warp paces the tensor pipe (4 MMAs = 512 clk per accumulator tile), so its per-tile
-    // instruction path is kept minimal: wrap-around counters instead of div/mod, descriptors
-    // advanced by constant adds.
+  } else if (warp < TMA_WARP) {
+    // =========================================================================== MMA issue (2 warps)
+    // tcgen05.mma issue is (nearly) blocking: measured, the issuing thread gets control back only
+    // ~160 clk before its 4 MMAs (512 clk) finish, so any bookkeeping + barrier wait longer than that
+    // between two tiles idles the tensor pipe.  Hence one issuing warp PER ACCUMULATOR STAGE: while
+    // warp 0 is blocked issuing into stage 0, warp 1 does its waits for stage 1 and queues behind it.
+    // The whole warp walks the loop (all values warp-uniform); one elected lane issues.
+    const int id = warp - MMA_WARP;  // = the accumulator stage this warp feeds
     constexpr uint32_t idesc = make_idesc_f16(BF_TILE_ROWS, TILE_T);
     const uint64_t adesc0 = make_sdesc_k_sw128(sA);
     const uint64_t bdesc0 = make_sdesc_k_sw128(sB);
+    const uint32_t d = tmem_base + id * TILE_T;
     Item it = decode_item(it0, nG, nTt);
     int ag = 0, ab = 0;
     int st = 0;                 // operand stage and the parity its "full" barrier completes next
     uint32_t st_par = 0;
-    int acc = 0;                // accumulator stage; te_par bit a = parity of t_empty[a] to wait for
-    uint32_t te_par = 3;        // first use of a stage passes on the fresh barrier (parity 1)
+    uint32_t te_par = 1;        // parity of t_empty[id] to wait for (first use passes on the fresh barrier)
+    int u = 0;                  // running accumulator-tile index; tile u goes to stage u & 1
     int gm = min(GROUP, nMt - it.g * GROUP);
     for (int i = 0; i < n_items; ++i) {
       if (i == 0 || it.tt == 0) {  // (chan, beam group) changes exactly when the time tile wraps
-        if (ag > 0 && elect_one()) tc_commit(bar_a_empty + 8 * ab);  // all MMAs so far have left the old buffer
+        if (ag > 0 && elect_one()) tc_commit(bar_a_empty + 8 * ab);  // my MMAs so far have left the old buffer
         ab = ag & 1;
         gm = min(GROUP, nMt - it.g * GROUP);
         mbar_wait(bar_a_full + 8 * ab, (ag >> 1) & 1);
         ++ag;
       }
-      mbar_wait(bar_b_full + 8 * st, st_par);
-      const uint64_t bdesc = bdesc0 + (uint64_t)(st * (B_STAGE_BYTES >> 4));
-      for (int m = 0; m < gm; ++m) {
-        mbar_wait(bar_t_empty + 8 * acc, (te_par >> acc) & 1);
-        tc_fence_after();
-        if (elect_one()) {
-          const uint64_t adesc = adesc0 + (uint64_t)((ab * GROUP + m) * (A_TILE_BYTES >> 4));
-          const uint32_t d = tmem_base + acc * TILE_T;
+      const int m0 = ((u & 1) == id) ? 0 : 1;  // my tiles of this item: m0, m0 + 2, ...
+      if (m0 < gm) {
+        mbar_wait(bar_b_full + 8 * st, st_par);
+        const uint64_t bdesc = bdesc0 + (uint64_t)(st * (B_STAGE_BYTES >> 4));
+        for (int m = m0; m < gm; m += 2) {
+          mbar_wait(bar_t_empty + 8 * id, te_par);
+          te_par ^= 1;
+          tc_fence_after();
+          if (elect_one()) {
+            const uint64_t adesc = adesc0 + (uint64_t)((ab * GROUP + m) * (A_TILE_BYTES >> 4));
 #pragma unroll
-          for (int k = 0; k < 4; ++k)  // advance 16 fp16 = 32 bytes along K inside the swizzle atom
-            if (k < nks) mma_f16_ss(d, adesc + 2 * k, bdesc + 2 * k, idesc, k > 0);
-          tc_commit(bar_t_full + 8 * acc);
-          if (m == gm - 1) tc_commit(bar_b_empty + 8 * st);
+            for (int k = 0; k < 4; ++k)  // advance 16 fp16 = 32 bytes along K inside the swizzle atom
+              if (k < nks) mma_f16_ss(d, adesc + 2 * k, bdesc + 2 * k, idesc, k > 0);
+            tc_commit(bar_t_full + 8 * id);
+            if (m + 2 >= gm) {
+              tc_commit(bar_b_empty + 8 * st);
+              if (gm == 1) tc_commit(bar_b_empty + 8 * st);  // the other warp has no tile in this item
+            }
+          }
         }
-        te_par ^= 1u << acc;
-        acc ^= 1;
       }
+      u += gm;
       if (++st == NSTAGE) { st = 0; st_par ^= 1; }
       next_item(it, nG, nTt);
     }
@@ -242,7 +250,7 @@ cudaError_t launch_k64(const BfParams &p, int sm_count, cudaStream_t st) {
     if (e != cudaSuccess) return e;
   }
   const int grid = (int)(total < sm_count ? total : sm_count);
-  kern<<<grid, (EPI_WARPS + CONV_WARPS + 2) * 32, smem, st>>>(p, total, nG, nTt, nks);
+  kern<<<grid, (EPI_WARPS + CONV_WARPS + 3) * 32, smem, st>>>(p, total, nG, nTt, nks);
   return cudaGetLastError();
 }
 

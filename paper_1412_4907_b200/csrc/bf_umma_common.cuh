@@ -88,8 +88,11 @@ __device__ __forceinline__ void epilogue_tile(const BfParams &p, uint32_t tmem_b
   float *prow = p.pow + ((size_t)c * p.nbeam + beam) * p.nbin;
   const int t_first = tt * TILE_T + slot * CPW;  // first time sample of this warp's columns
   const int bin0 = NINT_T == 0 ? t_first / p.nint : t_first / (NINT_T == 0 ? 1 : NINT_T);
-  float binacc = 0.f;
   float ob[4];
+  constexpr int NACC = SUB >= 8 ? 4 : (SUB >= 2 ? SUB / 2 : 1);
+  float2 a[NACC];  // packed running sums of squares; live across the chunks of one bin
+#pragma unroll
+  for (int q = 0; q < NACC; ++q) a[q] = make_float2(0.f, 0.f);
 #pragma unroll
   for (int ch = 0; ch < NCH; ++ch) {
     uint32_t v[32];
@@ -107,24 +110,15 @@ __device__ __forceinline__ void epilogue_tile(const BfParams &p, uint32_t tmem_b
         const float d = __uint_as_float(v[s]);
         sum = d * d;
       } else {
-        constexpr int NACC = SUB >= 8 ? 4 : SUB / 2;
-        float2 a[NACC];
-#pragma unroll
-        for (int q = 0; q < NACC; ++q) a[q] = make_float2(0.f, 0.f);
 #pragma unroll
         for (int j = 0; j < SUB / 2; ++j) {
           const float2 d = make_float2(__uint_as_float(v[s * SUB + 2 * j]), __uint_as_float(v[s * SUB + 2 * j + 1]));
           a[j % NACC] = ffma2(d, d, a[j % NACC]);
         }
+        if (CPB > 1 && (ch + 1) % CPB != 0) continue;  // bin continues in the next chunk
         sum = 0.f;
 #pragma unroll
-        for (int q = 0; q < NACC; ++q) sum += a[q].x + a[q].y;
-      }
-      if (CPB > 1) {
-        binacc += sum;
-        if ((ch + 1) % CPB != 0) continue;
-        sum = binacc;
-        binacc = 0.f;
+        for (int q = 0; q < NACC; ++q) { sum += a[q].x + a[q].y; a[q] = make_float2(0.f, 0.f); }
       }
       const float tot = sum + __shfl_xor_sync(0xffffffffu, sum, 16);  // re^2 rows + im^2 rows
       if (NINT_T == 0) {

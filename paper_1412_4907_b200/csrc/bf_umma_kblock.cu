@@ -26,8 +26,8 @@ constexpr int KB_GROUP = 2;                        // M-tiles (of 64 beams) per 
 constexpr int CONV_WARPS = 8;
 constexpr int CONV_THREADS = CONV_WARPS * 32;
 constexpr int MMA_WARP = EPI_WARPS + CONV_WARPS;
-constexpr int TMA_WARP = MMA_WARP + 1;
-constexpr int NTHREADS = (EPI_WARPS + CONV_WARPS + 2) * 32;
+constexpr int TMA_WARP = MMA_WARP + 2;  // two MMA-issuing warps, one per accumulator
+constexpr int NTHREADS = (EPI_WARPS + CONV_WARPS + 3) * 32;
 constexpr int A_STAGE_BYTES = KB_GROUP * A_TILE_BYTES;
 
 struct KItem { int c, tt, g; };
@@ -65,8 +65,8 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < NA; ++s) { mbar_init(bar_a_full + 8 * s, 1); mbar_init(bar_a_empty + 8 * s, 1); }
-    for (int s = 0; s < NB; ++s) { mbar_init(bar_b_full + 8 * s, IS_F16 ? 1 : CONV_WARPS); mbar_init(bar_b_empty + 8 * s, 1); }
+    for (int s = 0; s < NA; ++s) { mbar_init(bar_a_full + 8 * s, 1); mbar_init(bar_a_empty + 8 * s, 2); }
+    for (int s = 0; s < NB; ++s) { mbar_init(bar_b_full + 8 * s, IS_F16 ? 1 : CONV_WARPS); mbar_init(bar_b_empty + 8 * s, 2); }
     for (int s = 0; s < NR; ++s) { mbar_init(bar_r_full + 8 * s, 1); mbar_init(bar_r_empty + 8 * s, CONV_WARPS); }
     for (int s = 0; s < 2; ++s) { mbar_init(bar_t_full + 8 * s, 1); mbar_init(bar_t_empty + 8 * s, EPI_WARPS); }
     fence_barrier_init();
@@ -130,37 +130,38 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
         if (++bs == NB) { bs = 0; bpar ^= 1; }
       }
     }
-  } else if (warp == MMA_WARP) {
-    // =========================================================================== MMA issue
+  } else if (warp < TMA_WARP) {
+    // =========================================================================== MMA issue (2 warps)
+    // One issuing warp per accumulator (tcgen05.mma issue is nearly blocking, see bf_umma.cu): warp id
+    // feeds accumulator id = M-tile id of the item's beam group, for every K-block.
+    const int id = warp - MMA_WARP;
     constexpr uint32_t idesc = make_idesc_f16(BF_TILE_ROWS, TILE_T);
-    const uint64_t adesc0 = make_sdesc_k_sw128(sA);
+    const uint64_t adesc0 = make_sdesc_k_sw128(sA + id * A_TILE_BYTES);
     const uint64_t bdesc0 = make_sdesc_k_sw128(sB);
+    const uint32_t d = tmem_base + id * TILE_T;
     KItem it = kdecode(it0, nG, nTt);
     int sa = 0, sb = 0;
-    uint32_t apar = 0, bpar = 0, tpar = 3;
+    uint32_t apar = 0, bpar = 0, tpar = 1;
     for (int i = 0; i < n_items; ++i, knext(it, nG, nTt)) {
       const int gm = min(KB_GROUP, nMt - it.g * KB_GROUP);
-      // the accumulators must have been drained (first use: fresh barriers pass on parity 1)
-      for (int m = 0; m < gm; ++m) { mbar_wait(bar_t_empty + 8 * m, (tpar >> m) & 1); tpar ^= 1u << m; }
-      tc_fence_after();
+      const bool mine = id < gm;  // an odd last group has no second M-tile
+      if (mine) { mbar_wait(bar_t_empty + 8 * id, tpar); tpar ^= 1; tc_fence_after(); }
       for (int kb = 0; kb < nKb; ++kb) {
-        mbar_wait(bar_a_full + 8 * sa, apar);
-        mbar_wait(bar_b_full + 8 * sb, bpar);
-        tc_fence_after();
-        if (elect_one()) {
-          const uint64_t bdesc = bdesc0 + (uint64_t)(sb * (B_STAGE_BYTES >> 4));
-          for (int m = 0; m < gm; ++m) {
-            const uint64_t adesc = adesc0 + (uint64_t)((sa * KB_GROUP + m) * (A_TILE_BYTES >> 4));
-            const uint32_t d = tmem_base + m * TILE_T;
+        if (mine) {
+          mbar_wait(bar_a_full + 8 * sa, apar);
+          mbar_wait(bar_b_full + 8 * sb, bpar);
+          tc_fence_after();
+          if (elect_one()) {
+            const uint64_t bdesc = bdesc0 + (uint64_t)(sb * (B_STAGE_BYTES >> 4));
+            const uint64_t adesc = adesc0 + (uint64_t)(sa * (A_STAGE_BYTES >> 4));
 #pragma unroll
             for (int k = 0; k < 4; ++k) mma_f16_ss(d, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+            tc_commit(bar_a_empty + 8 * sa);
+            tc_commit(bar_b_empty + 8 * sb);
+            if (gm == 1) { tc_commit(bar_a_empty + 8 * sa); tc_commit(bar_b_empty + 8 * sb); }  // other warp idle
+            if (kb == nKb - 1) tc_commit(bar_t_full + 8 * id);
           }
-          tc_commit(bar_a_empty + 8 * sa);
-          tc_commit(bar_b_empty + 8 * sb);
-          if (kb == nKb - 1)
-            for (int m = 0; m < gm; ++m) tc_commit(bar_t_full + 8 * m);
         }
-        __syncwarp();
         if (++sa == NA) { sa = 0; apar ^= 1; }
         if (++sb == NB) { sb = 0; bpar ^= 1; }
       }
