@@ -53,6 +53,24 @@ def algorithmic_bytes(w):
     return w.in_bytes + w.nchan * w.nbeam * w.nant * 4 + w.out_bytes
 
 
+def rank_seed(base_seed: int, rank: int) -> int:
+    """Every replica beamforms its own buffer (weak scaling, no exchange between ranks)."""
+    return base_seed + 100 * rank
+
+
+def aggregate(total_ms_local: float, units_local: float, dist_mod=None, device=None):
+    """(max over ranks of the timed region, sum over ranks of the units processed).  With one
+    process this is the identity; with several it is two all-reduces (MAX, SUM) on `device`."""
+    if dist_mod is None:
+        return total_ms_local, units_local
+    import torch
+    t = torch.tensor([total_ms_local], dtype=torch.float64, device=device)
+    u = torch.tensor([units_local], dtype=torch.float64, device=device)
+    dist_mod.all_reduce(t, op=dist_mod.ReduceOp.MAX)
+    dist_mod.all_reduce(u, op=dist_mod.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -205,7 +223,7 @@ def main():
     W = max(3, args.warmup)
     K = max(1, args.steps)
     w = workload_for(args.config)
-    w.seed += 100 * rank  # every replica beamforms its own buffer
+    w.seed = rank_seed(w.seed, rank)
     peaks = load_peaks()
     kern = {"auto": bf.BF_KERNEL_AUTO, "simt": bf.BF_KERNEL_SIMT, "umma": bf.BF_KERNEL_UMMA}[args.kernel]
     dt = bf.BF_CI8 if w.dtype == "ci8" else bf.BF_CF16
@@ -240,12 +258,9 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     total_ms = ev[0].elapsed_time(ev[K])
     per_launch_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(K)]
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if dist:
-        td.all_reduce(t, op=td.ReduceOp.MAX)
-    total_ms_max = float(t.item())
     flop_step = 8.0 * w.cmac
-    value = world * flop_step * K / (total_ms_max * 1e-3) / 1e12
+    total_ms_max, flop_all = aggregate(total_ms, flop_step * K, td if dist else None, dev)
+    value = flop_all / (total_ms_max * 1e-3) / 1e12
     ms_per_step = total_ms_max / K
     avg_kernel_ms = statistics.mean(per_launch_ms)
 
@@ -297,11 +312,8 @@ def main():
         cs.synchronize(); xs.synchronize()
         barrier()
         e2e_ms = e0.elapsed_time(e1)
-        te = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-        if dist:
-            td.all_reduce(te, op=td.ReduceOp.MAX)
-        e2e_ms = float(te.item())
-        e2e = {"value": world * flop_step * Ke / (e2e_ms * 1e-3) / 1e12, "unit": UNIT,
+        e2e_ms, e2e_flop = aggregate(e2e_ms, flop_step * Ke, td if dist else None, dev)
+        e2e = {"value": e2e_flop / (e2e_ms * 1e-3) / 1e12, "unit": UNIT,
                "h2d_bytes_per_step": int(w.in_bytes), "d2h_bytes_per_step": int(w.out_bytes), "steps": Ke,
                "ms_per_step": e2e_ms / Ke, "h2d_gbs": w.in_bytes / (e2e_ms / Ke * 1e-3) / 1e9,
                "chan_per_chunk": cpc, "api": "bf_run_host (pinned host in/out, 2 streams)"}

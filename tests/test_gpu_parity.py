@@ -104,8 +104,13 @@ SMALL = [
     (64, 2, 33, 512, 32, "ci8"),
     (5, 2, 3, 77, 7, "ci8"),         # odd everything: generic kernel only
     (32, 2, 16, 256, 16, "cf16"),
-    (256, 1, 70, 512, 32, "cf16"),
-    (12, 2, 6, 200, 8, "cf16"),
+    (256, 1, 70, 512, 32, "cf16"),   # K-blocked kernel, 2 M-tiles, second one ragged
+    (12, 2, 6, 200, 8, "cf16"),      # K' = 24 < one K-block (TMA zero-fills the rest)
+    (40, 2, 20, 520, 8, "ci8"),      # K' = 80: second K-block only a quarter full
+    (64, 1, 130, 768, 64, "ci8"),    # three M-tiles: the last beam group has a single tile
+    (128, 1, 9, 512, 128, "ci8"),    # nint > 64: atomic partial sums, K-blocked
+    (96, 2, 64, 300, 4, "cf16"),     # ragged time tail, K' = 192
+    (1024, 1, 16, 256, 64, "ci8"),   # the streaming config's antenna count
 ]
 
 
@@ -184,9 +189,13 @@ def test_full_size_sampled_channels(bf, name, nbeam, nsample):
 
 
 # ------------------------------------------------------------------ host / streaming entry points
-def test_run_host_and_streaming_match_run(bf):
+@pytest.mark.parametrize("name", ["tiny", "kblock"])
+def test_run_host_and_streaming_match_run(bf, name):
     import torch
     w = synthetic.make_workload("tiny")
+    if name == "kblock":  # same sizes, 64 antennas -> the K-blocked kernel (TMA tensor map per launch)
+        w = synthetic.Workload("tiny64", 64, 64, 16, 1024, 16, "ci8", 7, synthetic.grid(8, 8, 3.0, 3.0),
+                               w.freqs, w.beam_dir, 16.0, [])
     blocks = [w.make_voltages(block=i) for i in range(3)]
     B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint)
     B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)

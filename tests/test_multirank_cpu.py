@@ -1,0 +1,61 @@
+"""N > 1 host logic on CPU: two gloo ranks.  The path shards with NO data-path collective (channels
+and replicas are independent); what the ranks share is the barrier + max-over-ranks timing
+and the sum of the units they processed (bench.py aggregate), and each rank draws its own buffer."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    import oracle
+    import synthetic
+    # each rank: its own seeded buffer, its own (oracle-computed) slab -- no exchange of data
+    w = synthetic.make_workload("tiny").sub(nchan=2, nsamp=64)
+    w.seed = bench.rank_seed(w.seed, rank)
+    v = w.make_voltages()
+    P = oracle.beamform(w.ant_xyz, w.freqs, w.beam_dir, v, w.nint)
+    local_ms = 10.0 + 5.0 * rank          # pretend timings: rank 1 is the slow one
+    units = float(w.cmac) * 8
+    dist.barrier()
+    t_max, u_sum = bench.aggregate(local_ms, units, dist, torch.device("cpu"))
+    out[rank] = (t_max, u_sum, float(P.sum()), int(v.astype(np.int64).sum()))
+    dist.destroy_process_group()
+
+
+def test_two_ranks_aggregate_and_shard():
+    world = 2
+    mgr = mp.Manager()
+    out = mgr.dict()
+    mp.spawn(_worker, args=(world, _free_port(), out), nprocs=world, join=True)
+    assert set(out.keys()) == {0, 1}
+    (t0, u0, p0, s0), (t1, u1, p1, s1) = out[0], out[1]
+    assert t0 == t1 == 15.0                       # max over ranks
+    assert u0 == u1 and u0 == 2 * 8 * 2 * 16 * 32 * 64  # sum over ranks of 8*C*B*N*T
+    assert s0 != s1 and p0 != p1                  # the replicas really beamformed different buffers
+
+
+def test_single_process_aggregate_is_identity():
+    import bench
+    assert bench.aggregate(3.5, 7.0) == (3.5, 7.0)
+    assert bench.rank_seed(1, 0) == 1 and bench.rank_seed(1, 3) == 301
