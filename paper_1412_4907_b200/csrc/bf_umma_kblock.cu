@@ -12,8 +12,11 @@
 // The two accumulators (2 x 256 TMEM columns) are drained by the same fused |.|^2 + integrate
 // epilogue as the small-array kernel once the last K-block has been issued.
 //
-// Work item = (channel, time tile, beam-group of 128 beams), beam group fastest, so the same CTA reads
-// a voltage tile for consecutive beam groups while it is still in L2.
+// Work item = (channel, time tile, beam-group of 128 beams), beam group fastest.  Items are dealt
+// round-robin to the persistent CTAs (item j -> CTA j mod grid), so at any moment the 148 CTAs work on
+// ~148 consecutive items = one or two channels: that channel's coefficients and voltages stay in the
+// 126 MB L2 while every CTA that needs them passes by (with contiguous ranges per CTA all channels
+// would be live at once and DRAM traffic was 3-14x the algorithmic bytes).
 #include <cuda.h>
 
 #include "bf_umma_common.cuh"
@@ -38,12 +41,6 @@ __device__ __forceinline__ KItem kdecode(long long idx, int nG, int nTt) {
   it.tt = (int)(ct % nTt);
   it.c = (int)(ct / nTt);
   return it;
-}
-__device__ __forceinline__ void knext(KItem &it, int nG, int nTt) {
-  if (++it.g == nG) {
-    it.g = 0;
-    if (++it.tt == nTt) { it.tt = 0; ++it.c; }
-  }
 }
 
 template <int NINT_T, bool IS_F16, int NA, int NB, int NR>
@@ -79,17 +76,16 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(s_tmem));
   tmem_base = __shfl_sync(0xffffffffu, tmem_base, 0);
 
-  const long long it0 = total_items * blockIdx.x / gridDim.x;
-  const long long it1 = total_items * (blockIdx.x + 1) / gridDim.x;
-  const int n_items = (int)(it1 - it0);
+  const long long it0 = blockIdx.x, it_step = gridDim.x;  // round-robin item assignment
+  const int n_items = (int)((total_items - it0 + it_step - 1) / it_step);
   const int nMt = p.nMt, nKb = p.nKb;
 
   if (warp < EPI_WARPS) {
     // =========================================================================== epilogue
     const int quad = warp & 3, slot = warp >> 2;
-    KItem it = kdecode(it0, nG, nTt);
     uint32_t tpar = 0;  // bit m: parity of the next completion of t_full[m] (an odd last group skips m = 1)
-    for (int i = 0; i < n_items; ++i, knext(it, nG, nTt)) {
+    for (int i = 0; i < n_items; ++i) {
+      const KItem it = kdecode(it0 + i * it_step, nG, nTt);
       const int gm = min(KB_GROUP, nMt - it.g * KB_GROUP);
       for (int m = 0; m < gm; ++m) {
         mbar_wait(bar_t_full + 8 * m, (tpar >> m) & 1);
@@ -139,10 +135,10 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
     const uint64_t adesc0 = make_sdesc_k_sw128(sA + id * A_TILE_BYTES);
     const uint64_t bdesc0 = make_sdesc_k_sw128(sB);
     const uint32_t d = tmem_base + id * TILE_T;
-    KItem it = kdecode(it0, nG, nTt);
     int sa = 0, sb = 0;
     uint32_t apar = 0, bpar = 0, tpar = 1;
-    for (int i = 0; i < n_items; ++i, knext(it, nG, nTt)) {
+    for (int i = 0; i < n_items; ++i) {
+      const KItem it = kdecode(it0 + i * it_step, nG, nTt);
       const int gm = min(KB_GROUP, nMt - it.g * KB_GROUP);
       const bool mine = id < gm;  // an odd last group has no second M-tile
       if (mine) { mbar_wait(bar_t_empty + 8 * id, tpar); tpar ^= 1; tc_fence_after(); }
@@ -169,14 +165,14 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
   } else if (warp == TMA_WARP && lane == 0) {
     // =========================================================================== TMA producer (one thread)
     tma_prefetch_desc(&tmap);
-    KItem it = kdecode(it0, nG, nTt);
     int sa = 0, sv = 0;  // sv: voltage stage (operand stage for fp16, raw stage for int8)
     uint32_t apar = 1, vpar = 1;
     constexpr int NV = IS_F16 ? NB : NR;
     constexpr uint32_t VBYTES = IS_F16 ? B_STAGE_BYTES : RAW_STAGE_BYTES;
     const uint32_t sV = IS_F16 ? sB : sR;
     const uint32_t bar_v_full = IS_F16 ? bar_b_full : bar_r_full, bar_v_empty = IS_F16 ? bar_b_empty : bar_r_empty;
-    for (int i = 0; i < n_items; ++i, knext(it, nG, nTt)) {
+    for (int i = 0; i < n_items; ++i) {
+      const KItem it = kdecode(it0 + i * it_step, nG, nTt);
       const int gm = min(KB_GROUP, nMt - it.g * KB_GROUP);
       for (int kb = 0; kb < nKb; ++kb) {
         mbar_wait(bar_a_empty + 8 * sa, apar);
