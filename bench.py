@@ -298,25 +298,41 @@ def main():
         del v
         torch.cuda.empty_cache()
         Ke = min(K, 10)
+        if w.name == "streaming":
+            # BASELINE.json config 5: continuous blocks from pinned host memory, H2D on a side stream
+            # overlapped with compute (bf_run_streaming, double-buffered staging); 2 distinct blocks cycled
+            hv2 = torch.empty(hv.shape, dtype=hv.dtype, pin_memory=True)
+            hv2.copy_(torch.roll(hv, 1, dims=1))
+            nblk = 8
+            blocks = [hv if (i % 2 == 0) else hv2 for i in range(nblk)]
+            Pb = torch.empty((nblk,) + tuple(P.shape), dtype=torch.float32, device=dev)
+            run_e2e = lambda: B.run_streaming(blocks, Pb, cs, xs)
+            steps_per_call, api = nblk, "bf_run_streaming (8 pinned host blocks per call, 2 streams, powers stay on device)"
+            d2h = 0
+        else:
+            run_e2e = lambda: B.run_host(hv, hp, cpc, cs, xs)
+            steps_per_call, api = 1, "bf_run_host (pinned host in/out, 2 streams)"
+            d2h = int(w.out_bytes)
         for _ in range(2):
-            B.run_host(hv, hp, cpc, cs, xs)
+            run_e2e()
         cs.synchronize(); xs.synchronize()
         barrier()
-        t0 = time.perf_counter()
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
         e0.record(cs)
         for _ in range(Ke):
-            B.run_host(hv, hp, cpc, cs, xs)
+            run_e2e()
         cs.wait_stream(xs)
         e1.record(cs)
         cs.synchronize(); xs.synchronize()
         barrier()
+        Ke *= steps_per_call
         e2e_ms = e0.elapsed_time(e1)
         e2e_ms, e2e_flop = aggregate(e2e_ms, flop_step * Ke, td if dist else None, dev)
         e2e = {"value": e2e_flop / (e2e_ms * 1e-3) / 1e12, "unit": UNIT,
-               "h2d_bytes_per_step": int(w.in_bytes), "d2h_bytes_per_step": int(w.out_bytes), "steps": Ke,
+               "h2d_bytes_per_step": int(w.in_bytes), "d2h_bytes_per_step": d2h, "steps": Ke,
                "ms_per_step": e2e_ms / Ke, "h2d_gbs": w.in_bytes / (e2e_ms / Ke * 1e-3) / 1e9,
-               "chan_per_chunk": cpc, "api": "bf_run_host (pinned host in/out, 2 streams)"}
+               "ant_samples_per_s": world * w.nchan * w.nsamp * w.nant * Ke / (e2e_ms * 1e-3),
+               "chan_per_chunk": cpc, "api": api}
         sample_src = hv
     else:
         sample_src = v

@@ -51,13 +51,16 @@ __device__ __forceinline__ void next_item(Item &it, int nG, int nTt) {
 
 // NINT_T: integration length if it is a power of two <= 64; 0 = a larger multiple of 64 (each epilogue
 // warp adds the partial sum of its 64 columns atomically into a zeroed output).
-template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS>
-__global__ void __launch_bounds__((EPI_WARPS + CONV_WARPS + 3) * 32, 1)
+// SPREAD: with <= 64 beams only the first TMEM lane quadrants hold real rows, and a quadrant can only be
+// read by warps w with w % 4 == quadrant -- which all sit on SM sub-partition `quadrant`.  For <= 16
+// beams the whole epilogue therefore lands on sub-partition 0; SPREAD launches 32 warps and puts the
+// convert / MMA / TMA warps on sub-partitions 1-3 only, so that sub-partition 0 does nothing else.
+template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD>
+__global__ void __launch_bounds__(SPREAD ? 1024 : (EPI_WARPS + CONV_WARPS + 3) * 32, 1)
 bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, const int nTt, const int nks) {
   extern __shared__ uint8_t smem_raw[];
   constexpr int CONV_THREADS = CONV_WARPS * 32;
-  constexpr int MMA_WARP = EPI_WARPS + CONV_WARPS;
-  constexpr int TMA_WARP = MMA_WARP + 2;  // two MMA-issuing warps, one per accumulator stage
+  static_assert(CONV_WARPS == 8, "role table below assumes 8 convert warps");
 
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sA = smem_base;                                  // 2 buffers x GROUP coefficient tiles
@@ -73,6 +76,19 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   // warp index through a shuffle so that the compiler knows it is warp-uniform (role code then
   // runs on the uniform datapath: descriptors in uniform registers, no per-lane waterfall loops)
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
+  // role table: cw = convert-warp index (0..7) or -1, mw = MMA-warp index (0/1) or -1
+  int cw = -1, mw = -1;
+  bool is_tma = false;
+  if (!SPREAD) {  // warps 16-23 convert, 24/25 MMA, 26 TMA
+    if (warp >= EPI_WARPS && warp < EPI_WARPS + 8) cw = warp - EPI_WARPS;
+    else if (warp == EPI_WARPS + 8 || warp == EPI_WARPS + 9) mw = warp - (EPI_WARPS + 8);
+    else if (warp == EPI_WARPS + 10) is_tma = true;
+  } else if (warp >= EPI_WARPS && (warp & 3) != 0) {  // 32 warps; nothing but epilogue on sub-partition 0
+    const int r = (warp - EPI_WARPS) >> 2, q = warp & 3;   // r = 0..3, q = 1..3
+    if (r < 3) { const int k = r * 3 + (q - 1); if (k < 8) cw = k; }   // 17,18,19,21,22,23,25,26
+    else if (q < 3) mw = q - 1;                                        // 29, 30
+    else is_tma = true;                                                // 31
+  }
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < NSTAGE; ++s) { mbar_init(bar_b_full + 8 * s, CONV_WARPS); mbar_init(bar_b_empty + 8 * s, 2); }
@@ -83,7 +99,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     }
     fence_barrier_init();
   }
-  if (warp == MMA_WARP) tmem_alloc(s_tmem, 512);
+  if (mw == 0) tmem_alloc(s_tmem, 512);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -116,10 +132,10 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
                               bar_t_empty + 8 * acc);
       }
     }
-  } else if (warp < MMA_WARP) {
+  } else if (cw >= 0) {
     // =========================================================================== convert
     constexpr int PIECES = MAX_INPUT_PIECES / CONV_THREADS;  // 16-byte input pieces per thread per tile
-    const int ctid = threadIdx.x - EPI_WARPS * 32;
+    const int ctid = cw * 32 + lane;
     const int npr = p.nant / 8;                  // 16-byte pieces per time sample (int8: 2*nant bytes)
     const int npieces = TILE_T * npr;
     // zero the operand stages once: K' columns beyond 2*nant must read as 0, never as stale NaN patterns
@@ -150,14 +166,14 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         mbar_arrive(bar_b_full + 8 * st);
       }
     }
-  } else if (warp < TMA_WARP) {
+  } else if (mw >= 0) {
     // =========================================================================== MMA issue (2 warps)
     // tcgen05.mma issue is (nearly) blocking: measured, the issuing thread gets control back only
     // ~160 clk before its 4 MMAs (512 clk) finish, so any bookkeeping + barrier wait longer than that
     // between two tiles idles the tensor pipe.  Hence one issuing warp PER ACCUMULATOR STAGE: while
     // warp 0 is blocked issuing into stage 0, warp 1 does its waits for stage 1 and queues behind it.
     // The whole warp walks the loop (all values warp-uniform); one elected lane issues.
-    const int id = warp - MMA_WARP;  // = the accumulator stage this warp feeds
+    const int id = mw;  // = the accumulator stage this warp feeds
     constexpr uint32_t idesc = make_idesc_f16(BF_TILE_ROWS, TILE_T);
     const uint64_t adesc0 = make_sdesc_k_sw128(sA);
     const uint64_t bdesc0 = make_sdesc_k_sw128(sB);
@@ -202,7 +218,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
       if (++st == NSTAGE) { st = 0; st_par ^= 1; }
       next_item(it, nG, nTt);
     }
-  } else if (warp == TMA_WARP && lane == 0) {
+  } else if (is_tma && lane == 0) {
     // =========================================================================== bulk-copy producer (one thread)
     const size_t row_bytes = (size_t)2 * p.nant;
     const char *volt = reinterpret_cast<const char *>(p.volt);
@@ -232,17 +248,17 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
 
   tc_fence_before();
   __syncthreads();
-  if (warp == MMA_WARP) tmem_dealloc(tmem_base, 512);
+  if (mw == 0) tmem_dealloc(tmem_base, 512);
 }
 
-template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS>
+template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD>
 cudaError_t launch_k64(const BfParams &p, int sm_count, cudaStream_t st) {
   const int nG = (p.nMt + GROUP - 1) / GROUP;
   const int nTt = (p.nsamp + TILE_T - 1) / TILE_T;
   const long long total = (long long)p.nchan_run * nG * nTt;
   const int nks = (2 * p.nant + 15) / 16;
   const size_t smem = 1024 + 2 * GROUP * A_TILE_BYTES + NSTAGE * B_STAGE_BYTES + NRAW * RAW_STAGE_BYTES + 256;
-  auto kern = bf_umma_k64_kernel<NINT_T, GROUP, NSTAGE, NRAW, CONV_WARPS>;
+  auto kern = bf_umma_k64_kernel<NINT_T, GROUP, NSTAGE, NRAW, CONV_WARPS, SPREAD>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   if (NINT_T == 0) {
@@ -250,14 +266,18 @@ cudaError_t launch_k64(const BfParams &p, int sm_count, cudaStream_t st) {
     if (e != cudaSuccess) return e;
   }
   const int grid = (int)(total < sm_count ? total : sm_count);
-  kern<<<grid, (EPI_WARPS + CONV_WARPS + 3) * 32, smem, st>>>(p, total, nG, nTt, nks);
+  kern<<<grid, SPREAD ? 1024 : (EPI_WARPS + CONV_WARPS + 3) * 32, smem, st>>>(p, total, nG, nTt, nks);
   return cudaGetLastError();
 }
 
 template <int NINT_T>
 cudaError_t launch_k64_nint(const BfParams &p, int sm_count, cudaStream_t st) {
-  if (p.nMt <= 2) return launch_k64<NINT_T, 2, 3, 4, 8>(p, sm_count, st);  // HBM/ingest-heavy: deep raw ring
-  return launch_k64<NINT_T, 4, 2, 2, 8>(p, sm_count, st);                  // many beams: MMA-bound, big A group
+  // <= 64 beams: HBM-bound.  A raw slot is held for the whole HBM latency plus the conversion (~3 us
+  // measured), so the bytes in flight per SM decide the bandwidth: 8 raw slots of 16 KiB.
+  if (p.nbeam <= 32) return launch_k64<NINT_T, 1, 2, 8, 8, true>(p, sm_count, st);   // rows only in lane quadrants 0-1
+  if (p.nMt == 1) return launch_k64<NINT_T, 1, 2, 8, 8, false>(p, sm_count, st);
+  if (p.nMt <= 2) return launch_k64<NINT_T, 2, 3, 4, 8, false>(p, sm_count, st);
+  return launch_k64<NINT_T, 4, 2, 2, 8, false>(p, sm_count, st);                  // many beams: MMA-bound, big A group
 }
 
 }  // namespace
