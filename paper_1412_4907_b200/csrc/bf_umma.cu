@@ -119,17 +119,45 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     // The TMEM stage is handed back to the MMA thread as soon as this warp's last tcgen05.ld has
     // landed in registers -- the squaring of that last chunk, the shuffle and the store run in the
     // shadow of the next tile's MMAs.
+    // 16 warps: warp w owns TMEM lanes 32*(w&3).. and columns 64*(w>>2).. of EVERY accumulator tile.
+    // Everything that does not change from tile to tile is computed here, once.
+    constexpr int BPW = NINT_T == 0 ? 1 : 64 / NINT_T;       // bins per warp and tile
+    constexpr int BPT = NINT_T == 0 ? 0 : TILE_T / NINT_T;   // bins per tile
     const int quad = warp & 3, slot = warp >> 2;
-    int u = 0;
+    const bool lane0 = lane == 0;
+    uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16) + slot * 64;
+    uint32_t b_full = bar_t_full, b_empty = bar_t_empty;
+    asm volatile("" : "+r"(t_lane), "+r"(b_full), "+r"(b_empty));  // keep in registers, do not rematerialise
+    const int bl = quad * 16 + (lane & 15);                  // this lane's beam inside an M-tile
+    const size_t mstride = (size_t)BF_TILE_BEAMS * p.nbin;   // output distance between M-tiles
+    const bool vec_ok = (p.nbin % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.pow) & 15) == 0);
     Item it = decode_item(it0, nG, nTt);
+    int u = 0, gm = 0, beam_g = 0;
+    float *base = nullptr;                                   // this lane's row of the group's first M-tile
     for (int i = 0; i < n_items; ++i, next_item(it, nG, nTt)) {
-      const int gm = min(GROUP, nMt - it.g * GROUP);
+      if (i == 0 || it.tt == 0) {                            // new (chan, beam group)
+        gm = min(GROUP, nMt - it.g * GROUP);
+        beam_g = it.g * GROUP * BF_TILE_BEAMS + bl;
+        base = p.pow + ((size_t)it.c * p.nbeam + beam_g) * p.nbin + slot * BPW;
+      }
       for (int m = 0; m < gm; ++m, ++u) {
         const int acc = u & 1;
-        mbar_wait(bar_t_full + 8 * acc, (u >> 1) & 1);
+        mbar_wait(b_full + 8 * acc, (u >> 1) & 1);
         tc_fence_after();
-        epilogue_tile<NINT_T>(p, tmem_base, acc * TILE_T, quad, slot, lane, it.c, it.g * GROUP + m, it.tt,
-                              bar_t_empty + 8 * acc);
+        const int beam = beam_g + m * BF_TILE_BEAMS;
+        if (beam - (lane & 15) >= p.nbeam) {                 // warp-uniform: only padding rows in this quadrant
+          epilogue_skip(b_empty + 8 * acc, lane0);
+          continue;
+        }
+        const bool writer = (lane < 16) && (beam < p.nbeam);
+        if (NINT_T == 0) {
+          const int t_first = it.tt * TILE_T + slot * 64;    // first time sample of this warp's columns
+          epilogue_tile<NINT_T>(t_lane + acc * TILE_T, base - slot * BPW + m * mstride + t_first / p.nint, writer,
+                                t_first < p.nsamp ? 1 : 0, false, b_empty + 8 * acc, lane0);
+        } else {
+          epilogue_tile<NINT_T>(t_lane + acc * TILE_T, base + m * mstride + it.tt * BPT, writer,
+                                p.nbin - (it.tt * BPT + slot * BPW), vec_ok, b_empty + 8 * acc, lane0);
+        }
       }
     }
   } else if (cw >= 0) {

@@ -59,35 +59,25 @@ __device__ __forceinline__ void convert_store(uint32_t s_dst, const uint32_t (&p
   }
 }
 
-// Epilogue of ONE accumulator tile (128 TMEM lanes x 256 columns at column `acc_col`) for ONE warp of
-// the 16: lanes 32*quad.., columns 64*slot...  Rows: lane l < 16 is the re row, lane l+16 the im row of
-// beam 64*mt + 16*quad + l.  The TMEM stage is handed back (arrive on bar_empty) as soon as this warp's
-// last tcgen05.ld has landed; squaring, shuffle and store run in the shadow of the next MMAs.
-// NINT_T: integration length if a power of two <= 64; 0 = a larger multiple of 64 (the partial sum of
-// the warp's 64 columns is added atomically into a zeroed output).
+// Epilogue of ONE accumulator tile for ONE warp of the 16: TMEM lanes 32*quad.., 64 columns starting at
+// `taddr` (lane and column already folded in).  Rows: lane l < 16 is the re row, lane l+16 the im row of
+// one beam.  The TMEM stage is handed back (arrive on bar_empty) as soon as this warp's last tcgen05.ld
+// has landed; squaring, shuffle and store run in the shadow of the next MMAs.  `out` points at this
+// lane's first output bin of the tile, `nvalid` = how many bins from there exist (tail tiles), `writer`
+// = this lane holds a real beam and is a re lane.  All per-tile address arithmetic is the caller's, so
+// that it can be hoisted out of the tile loop.
+// NINT_T: integration length if a power of two <= 64; 0 = a larger multiple of 64: the partial sum of
+// the warp's 64 columns is added atomically into the (zeroed) bin `out` points at.
 template <int NINT_T>
-__device__ __forceinline__ void epilogue_tile(const BfParams &p, uint32_t tmem_base, uint32_t acc_col, int quad, int slot,
-                                              int lane, int c, int mt, int tt, uint32_t bar_empty) {
+__device__ __forceinline__ void epilogue_tile(uint32_t taddr, float *out, bool writer, int nvalid, bool vec_ok,
+                                              uint32_t bar_empty, bool lane0) {
   constexpr int CPW = TILE_T / (EPI_WARPS / 4);                          // columns per warp (64)
   constexpr int NCH = CPW / 32;                                          // 32-column chunks per warp
   constexpr int SUB = (NINT_T == 0 || NINT_T > 32) ? 32 : NINT_T;        // columns per partial sum
   constexpr int NSUB = 32 / SUB;                                          // partial sums per chunk
   constexpr int CPB = NINT_T == 0 ? NCH : (NINT_T <= 32 ? 1 : NINT_T / 32);  // chunks per bin
-  constexpr int BINS_PER_WARP = NINT_T == 0 ? 1 : CPW / NINT_T;
+  constexpr int NBIN = NINT_T == 0 ? 1 : CPW / NINT_T;                   // bins per warp and tile
   static_assert(NINT_T == 0 || (NINT_T <= CPW && CPW % (NINT_T == 0 ? 1 : NINT_T) == 0), "bin must not straddle epilogue warps");
-  const int beam0 = mt * BF_TILE_BEAMS + quad * 16;
-  if (beam0 >= p.nbeam) {  // warp-uniform: this lane quadrant holds only padding rows
-    __syncwarp();
-    if (lane == 0) mbar_arrive(bar_empty);
-    return;
-  }
-  const bool vec_ok = (BINS_PER_WARP >= 4) && (p.nbin % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.pow) & 15) == 0);
-  const uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16) + acc_col + slot * CPW;
-  const int beam = beam0 + (lane & 15);
-  const bool writer = (lane < 16) && (beam < p.nbeam);
-  float *prow = p.pow + ((size_t)c * p.nbeam + beam) * p.nbin;
-  const int t_first = tt * TILE_T + slot * CPW;  // first time sample of this warp's columns
-  const int bin0 = NINT_T == 0 ? t_first / p.nint : t_first / (NINT_T == 0 ? 1 : NINT_T);
   float ob[4];
   constexpr int NACC = SUB >= 8 ? 4 : (SUB >= 2 ? SUB / 2 : 1);
   float2 a[NACC];  // packed running sums of squares; live across the chunks of one bin
@@ -96,12 +86,12 @@ __device__ __forceinline__ void epilogue_tile(const BfParams &p, uint32_t tmem_b
 #pragma unroll
   for (int ch = 0; ch < NCH; ++ch) {
     uint32_t v[32];
-    BF_TMEM_LD_32x32b_X32(t_lane + 32 * ch, v);
+    BF_TMEM_LD_32x32b_X32(taddr + 32 * ch, v);
     tc_wait_ld();
     if (ch == NCH - 1) {  // all of this warp's columns are in registers: release the stage
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(bar_empty);
+      if (lane0) mbar_arrive(bar_empty);
     }
 #pragma unroll
     for (int s = 0; s < NSUB; ++s) {
@@ -116,26 +106,34 @@ __device__ __forceinline__ void epilogue_tile(const BfParams &p, uint32_t tmem_b
           a[j % NACC] = ffma2(d, d, a[j % NACC]);
         }
         if (CPB > 1 && (ch + 1) % CPB != 0) continue;  // bin continues in the next chunk
-        sum = 0.f;
 #pragma unroll
-        for (int q = 0; q < NACC; ++q) { sum += a[q].x + a[q].y; a[q] = make_float2(0.f, 0.f); }
+        for (int w = NACC / 2; w >= 1; w >>= 1)        // packed add tree
+#pragma unroll
+          for (int q = 0; q < w; ++q) a[q] = fadd2(a[q], a[q + w]);
+        sum = a[0].x + a[0].y;
+#pragma unroll
+        for (int q = 0; q < NACC; ++q) a[q] = make_float2(0.f, 0.f);
       }
       const float tot = sum + __shfl_xor_sync(0xffffffffu, sum, 16);  // re^2 rows + im^2 rows
       if (NINT_T == 0) {
-        if (writer && t_first < p.nsamp) atomicAdd(prow + bin0, tot);
+        if (writer && nvalid > 0) atomicAdd(out, tot);
       } else {
         const int jb = (ch / CPB) * NSUB + s;  // bin index inside this warp's columns (compile-time)
-        const int j = bin0 + jb;
-        if (vec_ok) {
+        if (NBIN >= 4 && vec_ok) {
           ob[jb & 3] = tot;
-          if ((jb & 3) == 3 && writer && j < p.nbin)
-            *reinterpret_cast<float4 *>(prow + j - 3) = make_float4(ob[0], ob[1], ob[2], ob[3]);
-        } else if (writer && j < p.nbin) {
-          prow[j] = tot;
+          if ((jb & 3) == 3 && writer && jb < nvalid)
+            *reinterpret_cast<float4 *>(out + jb - 3) = make_float4(ob[0], ob[1], ob[2], ob[3]);
+        } else if (writer && jb < nvalid) {
+          out[jb] = tot;
         }
       }
     }
   }
+}
+// a lane quadrant that holds only padding rows just hands the stage back
+__device__ __forceinline__ void epilogue_skip(uint32_t bar_empty, bool lane0) {
+  __syncwarp();
+  if (lane0) mbar_arrive(bar_empty);
 }
 
 }  // namespace bfk

@@ -82,17 +82,33 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
 
   if (warp < EPI_WARPS) {
     // =========================================================================== epilogue
+    constexpr int BPW = NINT_T == 0 ? 1 : 64 / NINT_T;       // bins per warp and tile
+    constexpr int BPT = NINT_T == 0 ? 0 : TILE_T / NINT_T;   // bins per tile
     const int quad = warp & 3, slot = warp >> 2;
+    const bool lane0 = lane == 0;
+    const uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16) + slot * 64;
+    const int bl = quad * 16 + (lane & 15);
+    const bool vec_ok = (p.nbin % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.pow) & 15) == 0);
     uint32_t tpar = 0;  // bit m: parity of the next completion of t_full[m] (an odd last group skips m = 1)
     for (int i = 0; i < n_items; ++i) {
       const KItem it = kdecode(it0 + i * it_step, nG, nTt);
       const int gm = min(KB_GROUP, nMt - it.g * KB_GROUP);
+      const int t_first = it.tt * TILE_T + slot * 64;
       for (int m = 0; m < gm; ++m) {
         mbar_wait(bar_t_full + 8 * m, (tpar >> m) & 1);
         tpar ^= 1u << m;
         tc_fence_after();
-        epilogue_tile<NINT_T>(p, tmem_base, m * TILE_T, quad, slot, lane, it.c, it.g * KB_GROUP + m, it.tt,
-                              bar_t_empty + 8 * m);
+        const int beam = (it.g * KB_GROUP + m) * BF_TILE_BEAMS + bl;
+        if (beam - (lane & 15) >= p.nbeam) { epilogue_skip(bar_t_empty + 8 * m, lane0); continue; }
+        const bool writer = (lane < 16) && (beam < p.nbeam);
+        float *row = p.pow + ((size_t)it.c * p.nbeam + beam) * p.nbin;
+        if (NINT_T == 0) {
+          epilogue_tile<NINT_T>(t_lane + m * TILE_T, row + t_first / p.nint, writer, t_first < p.nsamp ? 1 : 0, false,
+                                bar_t_empty + 8 * m, lane0);
+        } else {
+          const int bin0 = it.tt * BPT + slot * BPW;
+          epilogue_tile<NINT_T>(t_lane + m * TILE_T, row + bin0, writer, p.nbin - bin0, vec_ok, bar_t_empty + 8 * m, lane0);
+        }
       }
     }
   } else if (warp < MMA_WARP) {

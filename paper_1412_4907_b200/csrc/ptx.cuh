@@ -146,6 +146,14 @@ __host__ __device__ constexpr uint32_t make_idesc_f16(uint32_t M, uint32_t N) {
                  "=r"(r[30]), "=r"(r[31])                                                          \
                : "r"(taddr))
 
+// packed fp32x2 add
+BF_DEVI float2 fadd2(float2 a, float2 b) {
+  float2 d;
+  asm("add.rn.f32x2 %0, %1, %2;"
+      : "=l"(reinterpret_cast<uint64_t &>(d))
+      : "l"(reinterpret_cast<uint64_t &>(a)), "l"(reinterpret_cast<uint64_t &>(b)));
+  return d;
+}
 // packed fp32x2 FMA (FFMA2): d = a * b + c on both halves of a 64-bit register pair
 BF_DEVI float2 ffma2(float2 a, float2 b, float2 c) {
   float2 d;
