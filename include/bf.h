@@ -103,6 +103,18 @@ int bf_set_geometry(bf_ctx *ctx, const double *ant_xyz_m, const double *chan_fre
                     const double *beam_dir, void *stream);
 
 /*
+ * Per-antenna complex gains folded into the weights: W'[c][b][n] = g[c][n] * W[c][b][n].  This is the
+ * paper's sub-arraying "antenna mask in the kernel" (g = 0 drops an antenna) and the gain
+ * calibration its X-engine provides -- free in the beamforming kernel because only the
+ * coefficients change.
+ *   gains  HOST fp64, (re, im) pairs: [nant][2] if per_channel == 0, else [nchan][nant][2];
+ *          NULL resets all gains to 1.
+ * If a geometry is already set the weights are regenerated on `stream`; otherwise the gains take effect
+ * at the next bf_set_geometry.  BF_EINVAL: non-finite gain.  BF_ENOGEOM: no workspace yet.
+ */
+int bf_set_antenna_gains(bf_ctx *ctx, const double *gains, int per_channel, void *stream);
+
+/*
  * Copy the generated weights back as fp32 (re, im) pairs, HOST [nchan][nbeam][nant][2] -- the values
  * the kernels actually use (after rounding to the operand type).  Synchronises `stream`.
  */

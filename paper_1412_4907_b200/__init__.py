@@ -33,6 +33,7 @@ SYMBOLS = {
     "bf_workspace_bytes": (_sz, [_vp]),
     "bf_set_workspace": (_i, [_vp, _vp, _sz]),
     "bf_set_geometry": (_i, [_vp, _dp, _dp, _dp, _vp]),
+    "bf_set_antenna_gains": (_i, [_vp, _dp, _i, _vp]),
     "bf_get_weights": (_i, [_vp, _vp, _vp]),
     "bf_run": (_i, [_vp, _vp, _vp, _vp]),
     "bf_staging_bytes": (_sz, [_vp, _i]),
@@ -132,6 +133,16 @@ def bf_set_geometry(ctx, ant_xyz_m, chan_freq_hz, beam_dir, stream=None):
     return lib().bf_set_geometry(ctx, pa, pf, pd, _stream(stream))
 
 
+def bf_set_antenna_gains(ctx, gains, per_channel=False, stream=None):
+    """gains: complex array [nant] (or [nchan][nant] with per_channel), or None to reset to 1."""
+    import numpy as np
+
+    if gains is None:
+        return lib().bf_set_antenna_gains(ctx, None, 0, _stream(stream))
+    g = np.ascontiguousarray(np.asarray(gains, dtype=np.complex128))
+    return lib().bf_set_antenna_gains(ctx, g.view(np.float64).ctypes.data_as(_dp), 1 if per_channel else 0, _stream(stream))
+
+
 def bf_get_weights(ctx, host_out, stream=None):
     return lib().bf_get_weights(ctx, _ptr(host_out), _stream(stream))
 
@@ -197,6 +208,9 @@ class Beamformer:
 
     def set_geometry(self, ant_xyz_m, chan_freq_hz, beam_dir, stream=None):
         self._check(bf_set_geometry(self.ctx, ant_xyz_m, chan_freq_hz, beam_dir, stream))
+
+    def set_antenna_gains(self, gains, per_channel=False, stream=None):
+        self._check(bf_set_antenna_gains(self.ctx, gains, per_channel, stream))
 
     def weights(self):
         import numpy as np

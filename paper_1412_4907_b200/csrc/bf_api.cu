@@ -34,7 +34,8 @@ size_t bf_wop_bytes_per_chan(const bf_ctx *c) {
   return (size_t)c->nMt * c->nKb * BF_TILE_ROWS * BF_KBLOCK * sizeof(__half);
 }
 static size_t geom_bytes(const bf_ctx *c) {
-  return align_up(sizeof(double) * (3 * (size_t)c->nant + c->nchan + 3 * (size_t)c->nbeam), BF_ALIGN);
+  return align_up(sizeof(double) * (3 * (size_t)c->nant + c->nchan + 3 * (size_t)c->nbeam +
+                                    2 * (size_t)c->nchan * c->nant), BF_ALIGN);
 }
 
 extern "C" const char *bf_version(void) { return "paper_1412_4907_b200 0.1 (sm_100a)"; }
@@ -54,6 +55,7 @@ extern "C" bf_ctx *bf_create(int nant, int nchan, int nbeam, int nsamp, int nint
   c->ws = nullptr; c->ws_bytes = 0;
   c->d_ant = c->d_freq = c->d_dir = nullptr; c->d_wop = nullptr;
   c->have_geom = false;
+  c->d_gain = nullptr; c->have_gains = false;
   c->launches = 0;
   c->sm_count = 0; c->device_ok = -1;
   c->have_events = false;
@@ -130,6 +132,7 @@ extern "C" int bf_set_workspace(bf_ctx *c, void *dev_ptr, size_t bytes) {
   c->d_ant = (double *)p;
   c->d_freq = c->d_ant + 3 * (size_t)c->nant;
   c->d_dir = c->d_freq + c->nchan;
+  c->d_gain = c->d_dir + 3 * (size_t)c->nbeam;
   c->d_wop = (__half *)(p + geom_bytes(c));
   c->have_geom = false;
   return BF_OK;
@@ -157,10 +160,42 @@ extern "C" int bf_set_geometry(bf_ctx *c, const double *ant, const double *freq,
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e = cudaMemcpyAsync(c->d_ant, c->h_geom.data(), (na + nf + nd) * sizeof(double), cudaMemcpyHostToDevice, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "geometry H2D copy");
+  if (c->have_gains) {
+    e = cudaMemcpyAsync(c->d_gain, c->h_gain.data(), c->h_gain.size() * sizeof(double), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "gain H2D copy");
+  }
   e = bf_launch_weights(c, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "weight generator launch");
   c->launches += 1;
   c->have_geom = true;
+  return BF_OK;
+}
+
+extern "C" int bf_set_antenna_gains(bf_ctx *c, const double *gains, int per_channel, void *stream) {
+  if (!c) return BF_EINVAL;
+  if (!gains) {
+    c->have_gains = false;
+    c->h_gain.clear();
+  } else {
+    const size_t n = 2 * (size_t)c->nant * (per_channel ? c->nchan : 1);
+    for (size_t i = 0; i < n; ++i)
+      if (!isfinite(gains[i])) return fail(c, BF_EINVAL, "antenna gain %zu is not finite", i / 2);
+    c->h_gain.resize(2 * (size_t)c->nant * c->nchan);
+    for (int ch = 0; ch < c->nchan; ++ch)
+      memcpy(c->h_gain.data() + 2 * (size_t)ch * c->nant, gains + (per_channel ? 2 * (size_t)ch * c->nant : 0),
+             2 * (size_t)c->nant * sizeof(double));
+    c->have_gains = true;
+  }
+  if (!c->have_geom) {
+    if (!c->ws) return fail(c, BF_ENOGEOM, "bf_set_workspace must be called before bf_set_antenna_gains");
+    return BF_OK;  // takes effect at the next bf_set_geometry
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e = cudaSuccess;
+  if (c->have_gains) e = cudaMemcpyAsync(c->d_gain, c->h_gain.data(), c->h_gain.size() * sizeof(double), cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = bf_launch_weights(c, st);
+  if (e != cudaSuccess) return cuda_fail(c, e, "weight regeneration");
+  c->launches += 1;
   return BF_OK;
 }
 

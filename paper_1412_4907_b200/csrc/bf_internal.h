@@ -47,6 +47,9 @@ struct bf_ctx {
   void *ws;
   size_t ws_bytes;
   double *d_ant, *d_freq, *d_dir;
+  double *d_gain;          // [nchan][nant][2] complex gains (always per channel on the device)
+  bool have_gains;         // false = all ones (d_gain not read)
+  std::vector<double> h_gain;
   __half *d_wop;
   bool have_geom;
   std::vector<double> h_geom;

@@ -11,7 +11,8 @@
 #define BF_C0 299792458.0
 
 __global__ void bf_weights_kernel(const double *__restrict__ ant, const double *__restrict__ freq,
-                                  const double *__restrict__ dir, __half *__restrict__ wop, int nant,
+                                  const double *__restrict__ dir, const double *__restrict__ gain,
+                                  __half *__restrict__ wop, int nant,
                                   int nchan, int nbeam, int nMt, int nKb) {
   // one thread per (chan, mt, row, n-slot) where n-slot covers the padded K' / 2
   const int npad = nKb * (BF_KBLOCK / 2);
@@ -34,6 +35,11 @@ __global__ void bf_weights_kernel(const double *__restrict__ ant, const double *
     double s, co;
     sincospi(2.0 * turns, &s, &co);
     double wre = co, wim = -s;  // e^{-i phi}
+    if (gain) {  // W' = g W: antenna mask / gain calibration folded into the coefficients
+      const double gre = gain[2 * ((size_t)c * nant + n)], gim = gain[2 * ((size_t)c * nant + n) + 1];
+      const double tre = gre * wre - gim * wim, tim = gre * wim + gim * wre;
+      wre = tre; wim = tim;
+    }
     if (part == 0) { a0 = (float)wre; a1 = (float)(-wim); }
     else           { a0 = (float)wim; a1 = (float)wre; }
   }
@@ -46,7 +52,8 @@ cudaError_t bf_launch_weights(const bf_ctx *c, cudaStream_t st) {
   long long total = (long long)c->nchan * c->nMt * BF_TILE_ROWS * c->nKb * (BF_KBLOCK / 2);
   int threads = 256;
   long long blocks = (total + threads - 1) / threads;
-  bf_weights_kernel<<<(unsigned)blocks, threads, 0, st>>>(c->d_ant, c->d_freq, c->d_dir, c->d_wop, c->nant,
+  bf_weights_kernel<<<(unsigned)blocks, threads, 0, st>>>(c->d_ant, c->d_freq, c->d_dir,
+                                                          c->have_gains ? c->d_gain : nullptr, c->d_wop, c->nant,
                                                           c->nchan, c->nbeam, c->nMt, c->nKb);
   return cudaGetLastError();
 }

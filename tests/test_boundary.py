@@ -68,6 +68,9 @@ def test_argument_errors_without_gpu(bf):
     assert bf.bf_set_geometry(ctx, r, f_bad, s) == bf.BF_EINVAL
     r_bad = r.copy(); r_bad[0, 0] = np.inf
     assert bf.bf_set_geometry(ctx, r_bad, f, s) == bf.BF_EINVAL
+    assert bf.bf_set_antenna_gains(ctx, np.ones(32, dtype=complex)) == bf.BF_ENOGEOM  # no workspace yet
+    gbad = np.ones(32, dtype=complex); gbad[5] = np.nan
+    assert bf.bf_set_antenna_gains(ctx, gbad) == bf.BF_EINVAL
     assert bf.bf_staging_bytes(ctx, 2) >= 2 * (2 * 256 * 32 * 2 + 2 * 16 * 16 * 4)
     assert bf.bf_launch_count(ctx) == 0
     bf.bf_destroy(ctx)

@@ -188,6 +188,45 @@ def test_full_size_sampled_channels(bf, name, nbeam, nsample):
     B.close()
 
 
+# ------------------------------------------------------------------ f2: antenna mask / complex gains in the weights
+@pytest.mark.parametrize("kernel", ["simt", "auto"])
+@pytest.mark.parametrize("mode", ["mask", "per_antenna", "per_channel"])
+def test_antenna_gains(bf, mode, kernel):
+    """W' = g W (PAPER.md:180 sub-arraying mask, PAPER.md:50 gain calibration).  The oracle knows nothing about
+    gains: it is handed the pre-scaled voltages g_n x_n in complex128 -- the same sum by linearity."""
+    import torch
+    w = synthetic.make_workload("tiny").sub(nchan=4, nsamp=512)
+    v = w.make_voltages()
+    rng = np.random.default_rng(3)
+    if mode == "mask":
+        g = (rng.random(w.nant) < 0.5).astype(np.complex128)      # drop about half the antennas
+        g[0] = 1.0
+        gfull = np.broadcast_to(g, (w.nchan, w.nant))
+    elif mode == "per_antenna":
+        g = rng.uniform(0.5, 1.5, w.nant) * np.exp(2j * np.pi * rng.random(w.nant))
+        gfull = np.broadcast_to(g, (w.nchan, w.nant))
+    else:
+        g = rng.uniform(0.5, 1.5, (w.nchan, w.nant)) * np.exp(2j * np.pi * rng.random((w.nchan, w.nant)))
+        gfull = g
+    x = (v[..., 0].astype(np.float64) + 1j * v[..., 1]) * gfull[:, None, :]
+    ref = oracle.beamform(w.ant_xyz, w.freqs, w.beam_dir, np.ascontiguousarray(x), w.nint)
+    B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint,
+                      kernel=bf.BF_KERNEL_SIMT if kernel == "simt" else bf.BF_KERNEL_AUTO)
+    B.set_antenna_gains(g, per_channel=(mode == "per_channel"))   # before the geometry: applied by set_geometry
+    B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
+    vd = torch.from_numpy(v).cuda()
+    out = B.run(vd).cpu().numpy()
+    check_rows(out, ref)
+    # resetting the gains on a live context regenerates the plain weights
+    B.set_antenna_gains(None)
+    out1 = B.run(vd).cpu().numpy()
+    check_rows(out1, oracle.beamform(w.ant_xyz, w.freqs, w.beam_dir, v, w.nint))
+    # and setting them after the geometry works too
+    B.set_antenna_gains(g, per_channel=(mode == "per_channel"))
+    np.testing.assert_array_equal(B.run(vd).cpu().numpy(), out)
+    B.close()
+
+
 # ------------------------------------------------------------------ host / streaming entry points
 @pytest.mark.parametrize("name", ["tiny", "kblock"])
 def test_run_host_and_streaming_match_run(bf, name):
