@@ -226,7 +226,7 @@ def main():
     w.seed = rank_seed(w.seed, rank)
     peaks = load_peaks()
     kern = {"auto": bf.BF_KERNEL_AUTO, "simt": bf.BF_KERNEL_SIMT, "umma": bf.BF_KERNEL_UMMA}[args.kernel]
-    dt = bf.BF_CI8 if w.dtype == "ci8" else bf.BF_CF16
+    dt = {"ci8": bf.BF_CI8, "cf16": bf.BF_CF16, "ci4": bf.BF_CI4}[w.dtype]
 
     B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint, dtype=dt, kernel=kern, device=dev)
     B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)

@@ -49,7 +49,9 @@ enum bf_status {
 
 enum bf_dtype {
   BF_CI8 = 0, /* complex int8, interleaved (re, im): 2 bytes per antenna-sample (BASELINE.json configs) */
-  BF_CF16 = 1 /* complex IEEE fp16, interleaved (re, im): 4 bytes per antenna-sample */
+  BF_CF16 = 1, /* complex IEEE fp16, interleaved (re, im): 4 bytes per antenna-sample */
+  BF_CI4 = 2   /* the paper's F-engine format: 4-bit + 4-bit two's complement in ONE byte per
+                  antenna-sample, high nibble real, low nibble imaginary; layout [nchan][nsamp][nant] bytes */
 };
 
 enum bf_kernel {
@@ -122,7 +124,7 @@ int bf_get_weights(bf_ctx *ctx, float *host_out, void *stream);
 
 /*
  * The hot path.  voltages: DEVICE, [nchan][nsamp][nant][2] (re, im interleaved) of the context's
- * dtype, 16-byte aligned.  powers: DEVICE fp32 [nchan][nbeam][nsamp/nint], fully overwritten.
+ * dtype ([nchan][nsamp][nant] bytes for BF_CI4), 16-byte aligned.  powers: DEVICE fp32 [nchan][nbeam][nsamp/nint], fully overwritten.
  * Enqueues on `stream` and returns.  BF_ENOGEOM before bf_set_geometry.
  */
 int bf_run(bf_ctx *ctx, const void *voltages, float *powers, void *stream);

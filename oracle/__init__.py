@@ -20,7 +20,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "bf_oracle.c")
 _LIB = os.path.join(_HERE, "libbf_oracle.so")
 
-CI8, CF16, C128 = 0, 1, 2
+CI8, CF16, C128, CI4 = 0, 1, 2, 3
 _lib = None
 
 
@@ -61,9 +61,12 @@ def _geom(ant_xyz, chan_freq_hz, beam_dir):
 
 
 def _volt(voltages, nchan, nant):
-    """Accept int8 [C][T][N][2], float16 [C][T][N][2], or complex128 [C][T][N]."""
+    """Accept int8 [C][T][N][2], float16 [C][T][N][2], complex128 [C][T][N], or uint8 [C][T][N]
+    (4+4-bit packed complex, high nibble real: PAPER.md:102)."""
     v = np.ascontiguousarray(voltages)
-    if v.dtype == np.int8:
+    if v.dtype == np.uint8:
+        dt = CI4
+    elif v.dtype == np.int8:
         dt = CI8
     elif v.dtype == np.float16:
         dt = CF16
@@ -71,7 +74,7 @@ def _volt(voltages, nchan, nant):
         dt = C128
     else:
         raise TypeError(f"unsupported voltage dtype {v.dtype}")
-    if dt == C128:
+    if dt in (C128, CI4):
         if v.ndim != 3 or v.shape[0] != nchan or v.shape[2] != nant:
             raise ValueError(f"bad voltage shape {v.shape}")
     else:

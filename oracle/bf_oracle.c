@@ -37,7 +37,7 @@
 
 #define ORACLE_C0 299792458.0 /* speed of light, m/s (exact SI value) */
 
-enum { ORACLE_CI8 = 0, ORACLE_CF16 = 1, ORACLE_C128 = 2 };
+enum { ORACLE_CI8 = 0, ORACLE_CF16 = 1, ORACLE_C128 = 2, ORACLE_CI4 = 3 };
 
 int oracle_num_threads(void) {
 #ifdef _OPENMP
@@ -89,6 +89,15 @@ static inline void load_sample(const void *volt, int dtype, size_t idx, double *
   } else if (dtype == ORACLE_CF16) {
     const _Float16 *p = (const _Float16 *)volt;
     *xr = (double)p[2 * idx]; *xi = (double)p[2 * idx + 1];
+  } else if (dtype == ORACLE_CI4) {
+    /* the paper's F-engine format: "4-bit, two's complement, complex voltages ... each antenna value as
+     * a single byte".  Nibble order is not stated: high nibble = real, low nibble =
+     * imaginary (reading A20).  Written out with plain integer arithmetic. */
+    const uint8_t b = ((const uint8_t *)volt)[idx];
+    int re = b >> 4, im = b & 15;
+    if (re >= 8) re -= 16;
+    if (im >= 8) im -= 16;
+    *xr = (double)re; *xi = (double)im;
   } else {
     const double *p = (const double *)volt;
     *xr = p[2 * idx]; *xi = p[2 * idx + 1];
@@ -106,7 +115,7 @@ int oracle_beamform(int nant, int nchan, int nbeam, int nsamp, int nint, int dty
                     double *powers, int chan_stride) {
   if (nant <= 0 || nchan <= 0 || nbeam <= 0 || nsamp <= 0 || nint <= 0) return -1;
   if (nsamp % nint != 0 || chan_stride <= 0) return -1;
-  if (dtype != ORACLE_CI8 && dtype != ORACLE_CF16 && dtype != ORACLE_C128) return -1;
+  if (dtype != ORACLE_CI8 && dtype != ORACLE_CF16 && dtype != ORACLE_C128 && dtype != ORACLE_CI4) return -1;
   const int nbin = nsamp / nint;
   int err = 0;
 #pragma omp parallel for schedule(dynamic, 1)

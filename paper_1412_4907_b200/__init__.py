@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libbf.so")
 
 BF_OK, BF_EINVAL, BF_ENOGEOM, BF_ECUDA, BF_EUNSUPPORTED, BF_ENOMEM = 0, -1, -2, -3, -4, -5
-BF_CI8, BF_CF16 = 0, 1
+BF_CI8, BF_CF16, BF_CI4 = 0, 1, 2
 BF_KERNEL_AUTO, BF_KERNEL_SIMT, BF_KERNEL_UMMA = 0, 1, 2
 
 # every symbol include/bf.h declares: name -> (restype, argtypes)
@@ -252,7 +252,7 @@ class Beamformer:
 
     def run_streaming(self, host_blocks, powers, compute_stream, copy_stream):
         nant, nchan, nbeam, nsamp, nint = self.shape
-        in_bytes = nchan * nsamp * nant * (2 if self.dtype == BF_CI8 else 4)
+        in_bytes = nchan * nsamp * nant * {BF_CI8: 2, BF_CF16: 4, BF_CI4: 1}[self.dtype]
         nbytes = 2 * ((in_bytes + 1023) // 1024 * 1024)
         st = self._get_staging(nbytes)
         self._check(bf_run_streaming(self.ctx, host_blocks, powers, st, nbytes, compute_stream, copy_stream))

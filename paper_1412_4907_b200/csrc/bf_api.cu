@@ -28,7 +28,7 @@ static int cuda_fail(bf_ctx *c, cudaError_t e, const char *what) {
 }
 
 size_t bf_in_bytes_per_chan(const bf_ctx *c) {
-  return (size_t)c->nsamp * c->nant * (c->dtype == BF_CI8 ? 2 : 4);
+  return (size_t)c->nsamp * c->nant * (c->dtype == BF_CI8 ? 2 : c->dtype == BF_CI4 ? 1 : 4);
 }
 size_t bf_wop_bytes_per_chan(const bf_ctx *c) {
   return (size_t)c->nMt * c->nKb * BF_TILE_ROWS * BF_KBLOCK * sizeof(__half);
@@ -74,7 +74,7 @@ extern "C" const char *bf_last_error(const bf_ctx *c) { return c ? c->err : "nul
 
 extern "C" int bf_set_dtype(bf_ctx *c, int dtype) {
   if (!c) return BF_EINVAL;
-  if (dtype != BF_CI8 && dtype != BF_CF16) return fail(c, BF_EINVAL, "unknown dtype %d", dtype);
+  if (dtype != BF_CI8 && dtype != BF_CF16 && dtype != BF_CI4) return fail(c, BF_EINVAL, "unknown dtype %d", dtype);
   c->dtype = dtype;
   return BF_OK;
 }

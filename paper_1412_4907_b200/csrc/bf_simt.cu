@@ -19,6 +19,9 @@ __device__ __forceinline__ float2 load_volt(const void *volt, size_t idx) {
   if (DTYPE == BF_CI8) {
     char2 v = reinterpret_cast<const char2 *>(volt)[idx];
     return make_float2((float)v.x, (float)v.y);
+  } else if (DTYPE == BF_CI4) {  // 4+4-bit two's complement, high nibble real
+    const int b = reinterpret_cast<const unsigned char *>(volt)[idx];
+    return make_float2((float)(((b >> 4) ^ 8) - 8), (float)(((b & 15) ^ 8) - 8));
   } else {
     __half2 v = reinterpret_cast<const __half2 *>(volt)[idx];
     return __half22float2(v);
@@ -100,7 +103,8 @@ cudaError_t bf_launch_simt(const BfParams &p, int dtype, cudaStream_t st) {
   dim3 grid((p.nsamp + samples_per_block - 1) / samples_per_block, (p.nbeam + SIMT_BEAMS - 1) / SIMT_BEAMS,
             p.nchan_run);
   if (grid.z > 65535 || grid.y > 65535) return cudaErrorInvalidConfiguration;
-  if (dtype == BF_CI8) bf_simt_kernel<BF_CI8><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
-  else                 bf_simt_kernel<BF_CF16><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
+  if (dtype == BF_CI8)      bf_simt_kernel<BF_CI8><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
+  else if (dtype == BF_CI4) bf_simt_kernel<BF_CI4><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
+  else                      bf_simt_kernel<BF_CF16><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
   return cudaGetLastError();
 }

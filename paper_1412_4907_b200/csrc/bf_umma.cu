@@ -55,7 +55,7 @@ __device__ __forceinline__ void next_item(Item &it, int nG, int nTt) {
 // read by warps w with w % 4 == quadrant -- which all sit on SM sub-partition `quadrant`.  For <= 16
 // beams the whole epilogue therefore lands on sub-partition 0; SPREAD launches 32 warps and puts the
 // convert / MMA / TMA warps on sub-partitions 1-3 only, so that sub-partition 0 does nothing else.
-template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD>
+template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD, int IN>
 __global__ void __launch_bounds__(SPREAD ? 1024 : (EPI_WARPS + CONV_WARPS + 3) * 32, 1)
 bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, const int nTt, const int nks) {
   extern __shared__ uint8_t smem_raw[];
@@ -162,9 +162,11 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     }
   } else if (cw >= 0) {
     // =========================================================================== convert
-    constexpr int PIECES = MAX_INPUT_PIECES / CONV_THREADS;  // 16-byte input pieces per thread per tile
+    // 16-byte input pieces per thread per tile: int8 rows are 2*nant bytes, 4-bit rows nant bytes
+    constexpr int PIECES = (IN == BF_CI4 ? MAX_INPUT_PIECES / 2 : MAX_INPUT_PIECES) / CONV_THREADS;
+    constexpr int CPP = IN == BF_CI4 ? 4 : 2;    // 16-byte fp16 output chunks per input piece
     const int ctid = cw * 32 + lane;
-    const int npr = p.nant / 8;                  // 16-byte pieces per time sample (int8: 2*nant bytes)
+    const int npr = IN == BF_CI4 ? p.nant / 16 : p.nant / 8;   // pieces per time sample
     const int npieces = TILE_T * npr;
     // zero the operand stages once: K' columns beyond 2*nant must read as 0, never as stale NaN patterns
     for (int o = ctid * 16; o < NSTAGE * B_STAGE_BYTES; o += CONV_THREADS * 16) st_shared_v4(sB + o, 0, 0, 0, 0);
@@ -177,7 +179,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     for (int k = 0; k < PIECES; ++k) {
       const int pc = ctid + k * CONV_THREADS;
       const int t = pc / npr, q = pc - t * npr;
-      p_dst[k] = pc < npieces ? (uint32_t)((t >> 3) * 1024 + (t & 7) * 128 + (((2 * q) ^ (t & 7)) << 4)) : 0xffffffffu;
+      p_dst[k] = pc < npieces ? (uint32_t)((t >> 3) * 1024 + (t & 7) * 128 + (((CPP * q) ^ (t & 7)) << 4)) : 0xffffffffu;
     }
     for (int i = 0; i < n_items; ++i) {
       const int rs = i % NRAW;
@@ -186,7 +188,8 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
       convert_load<PIECES, CONV_THREADS>(sR + rs * RAW_STAGE_BYTES, ctid, p_dst, x);
       const int st = i % NSTAGE;
       mbar_wait(bar_b_empty + 8 * st, ((i / NSTAGE) & 1) ^ 1);
-      convert_store<PIECES>(sB + st * B_STAGE_BYTES, p_dst, x);
+      if (IN == BF_CI4) convert_store_ci4<PIECES>(sB + st * B_STAGE_BYTES, p_dst, x);
+      else convert_store<PIECES>(sB + st * B_STAGE_BYTES, p_dst, x);
       fence_proxy_async_smem();
       __syncwarp();
       if (lane == 0) {
@@ -248,7 +251,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     }
   } else if (is_tma && lane == 0) {
     // =========================================================================== bulk-copy producer (one thread)
-    const size_t row_bytes = (size_t)2 * p.nant;
+    const size_t row_bytes = IN == BF_CI4 ? (size_t)p.nant : (size_t)2 * p.nant;
     const char *volt = reinterpret_cast<const char *>(p.volt);
     int ag = 0, prev_c = -1, prev_g = -1;
     Item it = decode_item(it0, nG, nTt);
@@ -279,14 +282,14 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   if (mw == 0) tmem_dealloc(tmem_base, 512);
 }
 
-template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD>
+template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD, int IN>
 cudaError_t launch_k64(const BfParams &p, int sm_count, cudaStream_t st) {
   const int nG = (p.nMt + GROUP - 1) / GROUP;
   const int nTt = (p.nsamp + TILE_T - 1) / TILE_T;
   const long long total = (long long)p.nchan_run * nG * nTt;
   const int nks = (2 * p.nant + 15) / 16;
   const size_t smem = 1024 + 2 * GROUP * A_TILE_BYTES + NSTAGE * B_STAGE_BYTES + NRAW * RAW_STAGE_BYTES + 256;
-  auto kern = bf_umma_k64_kernel<NINT_T, GROUP, NSTAGE, NRAW, CONV_WARPS, SPREAD>;
+  auto kern = bf_umma_k64_kernel<NINT_T, GROUP, NSTAGE, NRAW, CONV_WARPS, SPREAD, IN>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   if (NINT_T == 0) {
@@ -298,45 +301,52 @@ cudaError_t launch_k64(const BfParams &p, int sm_count, cudaStream_t st) {
   return cudaGetLastError();
 }
 
-template <int NINT_T>
+template <int NINT_T, int IN>
 cudaError_t launch_k64_nint(const BfParams &p, int sm_count, cudaStream_t st) {
   // <= 64 beams: HBM-bound.  A raw slot is held for the whole HBM latency plus the conversion (~3 us
   // measured), so the bytes in flight per SM decide the bandwidth: 8 raw slots of 16 KiB.
-  if (p.nbeam <= 32) return launch_k64<NINT_T, 1, 2, 8, 8, true>(p, sm_count, st);   // rows only in lane quadrants 0-1
-  if (p.nMt == 1) return launch_k64<NINT_T, 1, 2, 8, 8, false>(p, sm_count, st);
-  if (p.nMt <= 2) return launch_k64<NINT_T, 2, 3, 4, 8, false>(p, sm_count, st);
-  return launch_k64<NINT_T, 4, 2, 2, 8, false>(p, sm_count, st);                  // many beams: MMA-bound, big A group
+  if (p.nbeam <= 32) return launch_k64<NINT_T, 1, 2, 8, 8, true, IN>(p, sm_count, st);   // rows only in lane quadrants 0-1
+  if (p.nMt == 1) return launch_k64<NINT_T, 1, 2, 8, 8, false, IN>(p, sm_count, st);
+  if (p.nMt <= 2) return launch_k64<NINT_T, 2, 3, 4, 8, false, IN>(p, sm_count, st);
+  return launch_k64<NINT_T, 4, 2, 2, 8, false, IN>(p, sm_count, st);                  // many beams: MMA-bound, big A group
 }
 
 }  // namespace
 
 static bool nint_ok(int I) { return (I <= 64 && (I & (I - 1)) == 0) || I % 64 == 0; }
 
-// which tensor-core kernel takes this shape: 1 = coefficients-resident (2*nant <= 64, int8), 2 = K-blocked
+// which tensor-core kernel takes this shape: 1 = coefficients-resident (2*nant <= 64), 2 = K-blocked
 static int umma_variant(int dtype, int nant) {
   if (dtype == BF_CI8 && nant % 8 == 0 && nant <= 32) return 1;
+  if (dtype == BF_CI4 && nant % 16 == 0 && nant <= 32) return 1;  // bulk copies need rows of 16 bytes
   if (dtype == BF_CI8 && nant % 8 == 0) return 2;   // TMA rows must be multiples of 16 bytes
   if (dtype == BF_CF16 && nant % 4 == 0) return 2;
   return 0;
 }
 
 bool bf_umma_supported(const bf_ctx *c, const char **why) {
-  if (!umma_variant(c->dtype, c->nant)) { *why = "needs nant % 8 == 0 (int8) or nant % 4 == 0 (fp16)"; return false; }
+  if (!umma_variant(c->dtype, c->nant)) { *why = "needs nant % 8 == 0 (int8), % 4 == 0 (fp16), or 16 / 32 (4-bit)"; return false; }
   if (!nint_ok(c->nint)) { *why = "needs nint a power of two <= 64 or a multiple of 64"; return false; }
   return true;
 }
 
-cudaError_t bf_launch_umma(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
-  if (umma_variant(dtype, p.nant) == 2) return bf_launch_umma_kblock(p, dtype, sm_count, st);
-  if (dtype != BF_CI8) return cudaErrorNotSupported;
+template <int IN>
+static cudaError_t launch_k64_in(const BfParams &p, int sm_count, cudaStream_t st) {
   switch (p.nint) {
-    case 1: return launch_k64_nint<1>(p, sm_count, st);
-    case 2: return launch_k64_nint<2>(p, sm_count, st);
-    case 4: return launch_k64_nint<4>(p, sm_count, st);
-    case 8: return launch_k64_nint<8>(p, sm_count, st);
-    case 16: return launch_k64_nint<16>(p, sm_count, st);
-    case 32: return launch_k64_nint<32>(p, sm_count, st);
-    case 64: return launch_k64_nint<64>(p, sm_count, st);
-    default: return launch_k64_nint<0>(p, sm_count, st);  // multiples of 64: atomic partial sums
+    case 1: return launch_k64_nint<1, IN>(p, sm_count, st);
+    case 2: return launch_k64_nint<2, IN>(p, sm_count, st);
+    case 4: return launch_k64_nint<4, IN>(p, sm_count, st);
+    case 8: return launch_k64_nint<8, IN>(p, sm_count, st);
+    case 16: return launch_k64_nint<16, IN>(p, sm_count, st);
+    case 32: return launch_k64_nint<32, IN>(p, sm_count, st);
+    case 64: return launch_k64_nint<64, IN>(p, sm_count, st);
+    default: return launch_k64_nint<0, IN>(p, sm_count, st);  // multiples of 64: atomic partial sums
   }
+}
+
+cudaError_t bf_launch_umma(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
+  const int v = umma_variant(dtype, p.nant);
+  if (v == 2) return bf_launch_umma_kblock(p, dtype, sm_count, st);
+  if (v != 1) return cudaErrorNotSupported;
+  return dtype == BF_CI4 ? launch_k64_in<BF_CI4>(p, sm_count, st) : launch_k64_in<BF_CI8>(p, sm_count, st);
 }

@@ -25,6 +25,24 @@ __device__ __forceinline__ void cvt_i8x4_f16x4(uint32_t w, uint32_t &lo, uint32_
   hi = *reinterpret_cast<uint32_t *>(&b);
 }
 
+// 4+4-bit packed complex (high nibble re, low nibble im), 4 antennas in one 32-bit word
+// -> four half2 (re, im), exact.  Per antenna: PRMT builds [b, 0x64, b, 0x64]; one LOP3 flips the two
+// sign bits and masks the nibbles, leaving the halves 0x6400|(re_u<<4) = 1024 + 16 re_u and
+// 0x6400|im_u = 1024 + im_u (re_u = re + 8, im_u = im + 8); one HFMA2 with per-half constants
+// (x/16 - 72, x - 1032) gives (re, im).
+__device__ __forceinline__ void cvt_i4x8_f16x8(uint32_t w, uint32_t (&h)[4]) {
+  const uint32_t c64 = 0x64646464u, flip = 0x00080080u, mask = 0xFF0FFFF0u;
+  const __half2 scale = __halves2half2(__ushort_as_half(0x2C00), __ushort_as_half(0x3C00));   // (1/16, 1)
+  const __half2 off = __halves2half2(__ushort_as_half(0xD480), __ushort_as_half(0xE408));     // (-72, -1032)
+#pragma unroll
+  for (int a = 0; a < 4; ++a) {
+    const uint32_t p = __byte_perm(w, c64, 0x4040 | a | (a << 8));  // [b_a, 0x64, b_a, 0x64]
+    const uint32_t m = (p ^ flip) & mask;
+    const __half2 r = __hfma2(*reinterpret_cast<const __half2 *>(&m), scale, off);
+    h[a] = *reinterpret_cast<const uint32_t *>(&r);
+  }
+}
+
 __device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
 }
@@ -55,6 +73,24 @@ __device__ __forceinline__ void convert_store(uint32_t s_dst, const uint32_t (&p
       cvt_i8x4_f16x4(x[k].w, h[6], h[7]);
       st_shared_v4(s_dst + p_dst[k], h[0], h[1], h[2], h[3]);
       st_shared_v4(s_dst + (p_dst[k] ^ 16u), h[4], h[5], h[6], h[7]);
+    }
+  }
+}
+
+// 4-bit input: raw stage rows are nant bytes; a 16-byte piece = 16 antennas = 4 output chunks of 16 bytes
+// (chunk (4q + j) ^ (t & 7) = first chunk ^ j, since 4q has its two low bits clear)
+template <int PIECES>
+__device__ __forceinline__ void convert_store_ci4(uint32_t s_dst, const uint32_t (&p_dst)[PIECES], const uint4 (&x)[PIECES]) {
+#pragma unroll
+  for (int k = 0; k < PIECES; ++k) {
+    if (p_dst[k] != 0xffffffffu) {
+      const uint32_t w[4] = {x[k].x, x[k].y, x[k].z, x[k].w};
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        uint32_t h[4];
+        cvt_i4x8_f16x8(w[j], h);
+        st_shared_v4(s_dst + (p_dst[k] ^ (uint32_t)(j << 4)), h[0], h[1], h[2], h[3]);
+      }
     }
   }
 }

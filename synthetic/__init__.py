@@ -98,6 +98,29 @@ def voltages_ci8(rng: np.random.Generator, nchan: int, nsamp: int, nant: int, si
     return out
 
 
+def pack_ci4(re, im) -> np.ndarray:
+    """Two's-complement nibbles, high nibble real, low nibble imaginary (reading A20). re, im in [-8, 7]."""
+    return (((np.asarray(re).astype(np.int16) & 15) << 4) | (np.asarray(im).astype(np.int16) & 15)).astype(np.uint8)
+
+
+def voltages_ci4(rng: np.random.Generator, nchan: int, nsamp: int, nant: int, sigma: float = 2.0,
+                 sources=None, ant_xyz=None, freqs=None) -> np.ndarray:
+    """4+4-bit packed complex voltages [C][T][N] uint8 (the paper's F-engine format):
+    Gaussian sigma per component + optional sources, clip(rint(.), -7, 7) (-8 never occurs)."""
+    out = np.empty((nchan, nsamp, nant), dtype=np.uint8)
+    for c in range(nchan):
+        z = rng.standard_normal((nsamp, nant, 2), dtype=np.float32).astype(np.float64) * sigma
+        if sources:
+            for (sdir, amp) in sources:
+                ph = rng.uniform(0.0, 2.0 * np.pi, size=(1, nsamp))
+                s = _source_term(ant_xyz, freqs[c:c + 1], sdir, amp, ph)[0]
+                z[..., 0] += s.real
+                z[..., 1] += s.imag
+        q = np.clip(np.rint(z), -7, 7).astype(np.int16)
+        out[c] = pack_ci4(q[..., 0], q[..., 1])
+    return out
+
+
 def voltages_cf16(rng: np.random.Generator, nchan: int, nsamp: int, nant: int, sigma: float = 1.0,
                   sources=None, ant_xyz=None, freqs=None) -> np.ndarray:
     """Complex fp16 voltages [C][T][N][2] (Gaussian sigma per component + sources, rounded RN)."""
@@ -137,7 +160,7 @@ class Workload:
 
     @property
     def in_bytes(self) -> int:
-        return self.nchan * self.nsamp * self.nant * (2 if self.dtype == "ci8" else 4)
+        return self.nchan * self.nsamp * self.nant * {"ci8": 2, "cf16": 4, "ci4": 1}[self.dtype]
 
     @property
     def out_bytes(self) -> int:
@@ -155,7 +178,7 @@ class Workload:
         nsamp = self.nsamp if nsamp is None else nsamp
         rng = np.random.default_rng([self.seed, chan0, block])
         f = self.freqs[chan0:chan0 + nchan]
-        fn = voltages_ci8 if self.dtype == "ci8" else voltages_cf16
+        fn = {"ci8": voltages_ci8, "cf16": voltages_cf16, "ci4": voltages_ci4}[self.dtype]
         return fn(rng, nchan, nsamp, self.nant, self.sigma, self.sources, self.ant_xyz, f)
 
     def sub(self, nchan: Optional[int] = None, nsamp: Optional[int] = None, nbeam: Optional[int] = None,
@@ -195,6 +218,10 @@ def make_workload(name: str, nbeam: Optional[int] = None) -> Workload:
         s = lm_grid(16, 8, 0.06, 0.03)
         (ib,) = _src_at_beam(s, 1)
         return Workload(name, N, C, B, T, I, "ci8", 1, r, chan_centres(400e6, 16e6, C), s, 16.0, [(s[ib].copy(), 8.0)])
+    if name == "medium-ci4":
+        # the medium geometry with the paper's own 4+4-bit wire format
+        w = make_workload("medium")
+        return dataclasses.replace(w, name=name, dtype="ci4", sigma=2.0, sources=[(w.sources[0][0], 1.0)])
     if name == "sweep":
         N, C, T, I = 32, 512, 16384, 16
         B = 64 if nbeam is None else nbeam
@@ -227,8 +254,9 @@ def fill_voltages_torch(w: Workload, device, chunk_chan: int = 16):
 
     g = torch.Generator(device=device)
     g.manual_seed(1000 + w.seed)
-    dt = torch.int8 if w.dtype == "ci8" else torch.float16
-    out = torch.empty((w.nchan, w.nsamp, w.nant, 2), dtype=dt, device=device)
+    dt = {"ci8": torch.int8, "cf16": torch.float16, "ci4": torch.uint8}[w.dtype]
+    shape = (w.nchan, w.nsamp, w.nant) if w.dtype == "ci4" else (w.nchan, w.nsamp, w.nant, 2)
+    out = torch.empty(shape, dtype=dt, device=device)
     r = torch.as_tensor(w.ant_xyz, device=device)
     for c0 in range(0, w.nchan, chunk_chan):
         c1 = min(w.nchan, c0 + chunk_chan)
@@ -243,6 +271,9 @@ def fill_voltages_torch(w: Workload, device, chunk_chan: int = 16):
             z[..., 1] += (amp * torch.sin(ph)).float()
         if w.dtype == "ci8":
             out[c0:c1] = torch.clamp(torch.round(z), -127, 127).to(torch.int8)
+        elif w.dtype == "ci4":
+            q = torch.clamp(torch.round(z), -7, 7).to(torch.int16)
+            out[c0:c1] = (((q[..., 0] & 15) << 4) | (q[..., 1] & 15)).to(torch.uint8)
         else:
             out[c0:c1] = z.to(torch.float16)
     return out

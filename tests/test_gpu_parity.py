@@ -42,9 +42,13 @@ def check_rows(P_gpu, P_ref, tol=TOL):
     return worst
 
 
+def bf_dtype(bf, w):
+    return {"ci8": bf.BF_CI8, "cf16": bf.BF_CF16, "ci4": bf.BF_CI4}[w.dtype]
+
+
 def run_gpu(bf, w, v_host, kernel):
     import torch
-    dt = bf.BF_CI8 if w.dtype == "ci8" else bf.BF_CF16
+    dt = bf_dtype(bf, w)
     B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint, dtype=dt, kernel=kernel)
     B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
     v = torch.from_numpy(v_host).cuda()
@@ -67,7 +71,7 @@ def kernels(bf):
 def test_weights_match_oracle(bf, name):
     w = synthetic.make_workload(name)
     w = w.sub(chan_idx=[0, w.nchan // 2, w.nchan - 1])
-    dt = bf.BF_CI8 if w.dtype == "ci8" else bf.BF_CF16
+    dt = bf_dtype(bf, w)
     B = bf.Beamformer(w.nant, w.nchan, w.nbeam, 64, 16, dtype=dt)
     B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
     Wg = B.weights()
@@ -111,6 +115,10 @@ SMALL = [
     (128, 1, 9, 512, 128, "ci8"),    # nint > 64: atomic partial sums, K-blocked
     (96, 2, 64, 300, 4, "cf16"),     # ragged time tail, K' = 192
     (1024, 1, 16, 256, 64, "ci8"),   # the streaming config's antenna count
+    (32, 2, 16, 1000, 8, "ci4"),     # the paper's 4+4-bit format, BEST-2's 32 antennas, ragged tail
+    (32, 1, 130, 512, 64, "ci4"),
+    (16, 2, 5, 256, 1, "ci4"),       # K' = 32: half a K-block
+    (24, 2, 7, 128, 16, "ci4"),      # rows of 24 bytes: generic kernel only
 ]
 
 
@@ -122,8 +130,8 @@ def test_small_shapes(bf, shape, kernel):
     r = rng.uniform(-40, 40, size=(N, 3)); r[:, 2] *= 0.05
     f = np.linspace(380e6, 420e6, C) if C > 1 else np.array([408e6])
     s = rng.normal(size=(B, 3)); s[:, 2] = np.abs(s[:, 2]) + 1.5; s /= np.linalg.norm(s, axis=1, keepdims=True)
-    w = synthetic.Workload("small", N, C, B, T, I, dtype, 0, r, f, s, 16.0 if dtype == "ci8" else 1.0,
-                           [(s[B // 2].copy(), 4.0 if dtype == "ci8" else 0.5)])
+    sig, amp = {"ci8": (16.0, 4.0), "cf16": (1.0, 0.5), "ci4": (2.0, 1.0)}[dtype]
+    w = synthetic.Workload("small", N, C, B, T, I, dtype, 0, r, f, s, sig, [(s[B // 2].copy(), amp)])
     v = w.make_voltages()
     ref = oracle.beamform(r, f, s, v, I)
     out, used = run_gpu(bf, w, v, bf.BF_KERNEL_SIMT if kernel == "simt" else bf.BF_KERNEL_AUTO)
@@ -157,7 +165,7 @@ def test_coherent_gain_property(bf):
 
 
 # ------------------------------------------------------------------ full BASELINE.json sizes, sampled channels
-FULL = [("medium", None, 4), ("sweep", 1, 4), ("sweep", 16, 4), ("sweep", 256, 2), ("sweep", 1024, 1),
+FULL = [("medium", None, 4), ("medium-ci4", None, 4), ("sweep", 1, 4), ("sweep", 16, 4), ("sweep", 256, 2), ("sweep", 1024, 1),
         ("large-N", None, 2), ("streaming", None, 1)]
 
 
@@ -168,7 +176,7 @@ def test_full_size_sampled_channels(bf, name, nbeam, nsample):
     import torch
     w = synthetic.make_workload(name, nbeam=nbeam)
     v = synthetic.fill_voltages_torch(w, "cuda")
-    dt = bf.BF_CI8 if w.dtype == "ci8" else bf.BF_CF16
+    dt = bf_dtype(bf, w)
     B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint, dtype=dt)
     B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
     P = B.empty_powers(); P.fill_(float("nan"))

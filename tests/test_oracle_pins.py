@@ -246,6 +246,20 @@ def test_fp16_and_int8_inputs_agree_on_common_values():
     np.testing.assert_array_equal(oracle.beamform(r, f, s, v8, 4), oracle.beamform(r, f, s, v16, 4))
 
 
+def test_ci4_decode_by_hand_and_against_int8():
+    """4+4-bit two's complement, one byte per antenna, high nibble real (reading A20)."""
+    # 0x7F = (+7, -1), 0x80 = (-8, 0), 0x19 = (+1, -7), 0xF0 = (-1, 0)
+    v = np.array([[[0x7F], [0x80], [0x19], [0xF0]]], dtype=np.uint8)  # [C=1][T=4][N=1]
+    P = oracle.beamform([[0, 0, 0]], [100e6], [[0, 0, 1.0]], v, nint=1)
+    np.testing.assert_allclose(P[0, 0], [49 + 1, 64 + 0, 1 + 49, 1 + 0], rtol=1e-14)
+    rng = np.random.default_rng(4)
+    re = rng.integers(-8, 8, size=(2, 32, 8)); im = rng.integers(-8, 8, size=(2, 32, 8))
+    v4 = synthetic.pack_ci4(re, im)
+    v8 = np.stack([re, im], axis=-1).astype(np.int8)
+    r = synthetic.grid(4, 2, 2.0, 2.0); s = synthetic.lm_grid(3, 2, 0.4, 0.3); f = [70e6, 333e6]
+    np.testing.assert_array_equal(oracle.beamform(r, f, s, v4, 8), oracle.beamform(r, f, s, v8, 8))
+
+
 def test_rejects_bad_nint():
     w = synthetic.make_workload("tiny").sub(nchan=1, nsamp=32)
     with pytest.raises(ValueError):
