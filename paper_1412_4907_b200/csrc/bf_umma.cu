@@ -23,6 +23,8 @@
 // Pipelines (all mbarrier based): raw stages full/empty (TMA <-> convert), operand stages full/empty
 // (convert <-> MMA), coefficient buffers full/empty (TMA <-> MMA), TMEM accumulator stages full/empty
 // (MMA <-> epilogue).
+#include <type_traits>
+
 #include "bf_umma_common.cuh"
 
 namespace {
@@ -116,49 +118,78 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   if (warp < EPI_WARPS) {
     // =========================================================================== epilogue
     // 16 warps: warp w owns TMEM lanes 32*(w&3).. and columns 64*(w>>2).. of EVERY accumulator tile.
-    // The TMEM stage is handed back to the MMA thread as soon as this warp's last tcgen05.ld has
+    // The TMEM stage is handed back to the MMA warp as soon as this warp's last tcgen05.ld has
     // landed in registers -- the squaring of that last chunk, the shuffle and the store run in the
-    // shadow of the next tile's MMAs.
-    // 16 warps: warp w owns TMEM lanes 32*(w&3).. and columns 64*(w>>2).. of EVERY accumulator tile.
-    // Everything that does not change from tile to tile is computed here, once.
+    // shadow of the next tile's MMAs.  The kernel is bound by instruction issue around the tensor
+    // pipe (profiles/), so everything that does not change from tile to tile is computed once per
+    // (chan, beam group) run and the accumulator stage of a tile is a compile-time constant:
+    // tile m of an item uses stage m & 1 (GROUP even), item i uses stage i & 1 (GROUP == 1).
     constexpr int BPW = NINT_T == 0 ? 1 : 64 / NINT_T;       // bins per warp and tile
     constexpr int BPT = NINT_T == 0 ? 0 : TILE_T / NINT_T;   // bins per tile
     const int quad = warp & 3, slot = warp >> 2;
     const bool lane0 = lane == 0;
     uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16) + slot * 64;
-    uint32_t b_full = bar_t_full, b_empty = bar_t_empty;
-    asm volatile("" : "+r"(t_lane), "+r"(b_full), "+r"(b_empty));  // keep in registers, do not rematerialise
+    uint32_t b_full = bar_t_full;
+    asm volatile("" : "+r"(t_lane), "+r"(b_full));           // keep in registers, do not rematerialise
     const int bl = quad * 16 + (lane & 15);                  // this lane's beam inside an M-tile
-    const size_t mstride = (size_t)BF_TILE_BEAMS * p.nbin;   // output distance between M-tiles
-    const bool vec_ok = (p.nbin % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.pow) & 15) == 0);
+    const int nbeam = p.nbeam, nbin = p.nbin;
+    const size_t mstride = (size_t)BF_TILE_BEAMS * nbin;     // output distance between M-tiles
+    const bool vec_ok = (nbin % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.pow) & 15) == 0);
+    const bool ragged = (p.nsamp % TILE_T) != 0;             // the last time tile of a channel is partial
     Item it = decode_item(it0, nG, nTt);
-    int u = 0, gm = 0, beam_g = 0;
-    float *base = nullptr;                                   // this lane's row of the group's first M-tile
-    for (int i = 0; i < n_items; ++i, next_item(it, nG, nTt)) {
-      if (i == 0 || it.tt == 0) {                            // new (chan, beam group)
-        gm = min(GROUP, nMt - it.g * GROUP);
-        beam_g = it.g * GROUP * BF_TILE_BEAMS + bl;
-        base = p.pow + ((size_t)it.c * p.nbeam + beam_g) * p.nbin + slot * BPW;
+    uint32_t par0 = 0, par1 = 0;                             // parity of the next completion of t_full[0/1]
+    int i = 0;
+    while (i < n_items) {
+      // ---- one run: the items of one (chan, beam group) inside my range; time tiles it.tt ..
+      const int run = min(n_items - i, nTt - it.tt);
+      const int gm = min(GROUP, nMt - it.g * GROUP);
+      const int beam0 = it.g * GROUP * BF_TILE_BEAMS + bl;
+      uint32_t rows = 0, wr = 0;                             // bit m: quadrant holds real rows / this lane stores
+#pragma unroll
+      for (int m = 0; m < GROUP; ++m) {
+        const int beam = beam0 + m * BF_TILE_BEAMS;
+        if (m < gm && beam - (lane & 15) < nbeam) rows |= 1u << m;
+        if (m < gm && lane < 16 && beam < nbeam) wr |= 1u << m;
       }
-      for (int m = 0; m < gm; ++m, ++u) {
-        const int acc = u & 1;
-        mbar_wait(b_full + 8 * acc, (u >> 1) & 1);
-        tc_fence_after();
-        const int beam = beam_g + m * BF_TILE_BEAMS;
-        if (beam - (lane & 15) >= p.nbeam) {                 // warp-uniform: only padding rows in this quadrant
-          epilogue_skip(b_empty + 8 * acc, lane0);
-          continue;
-        }
-        const bool writer = (lane < 16) && (beam < p.nbeam);
+      float *ptr = p.pow + ((size_t)it.c * nbeam + beam0) * nbin + (NINT_T == 0 ? 0 : it.tt * BPT + slot * BPW);
+      int tt = it.tt;
+      for (int k = 0; k < run; ++k, ++i, ++tt, ptr += BPT) {
+        int nvalid = 1 << 30;
+        float *out = ptr;
         if (NINT_T == 0) {
-          const int t_first = it.tt * TILE_T + slot * 64;    // first time sample of this warp's columns
-          epilogue_tile<NINT_T>(t_lane + acc * TILE_T, base - slot * BPW + m * mstride + t_first / p.nint, writer,
-                                t_first < p.nsamp ? 1 : 0, false, b_empty + 8 * acc, lane0);
+          const int t_first = tt * TILE_T + slot * 64;       // first time sample of this warp's columns
+          out = ptr + t_first / p.nint;
+          nvalid = t_first < p.nsamp ? 1 : 0;
+        } else if (ragged && tt == nTt - 1) {
+          nvalid = nbin - (tt * BPT + slot * BPW);
+        }
+        auto one = [&](auto acc_c, int m) {
+          constexpr int ACC = decltype(acc_c)::value;
+          uint32_t &par = ACC ? par1 : par0;
+          mbar_wait(b_full + 8 * ACC, par);
+          par ^= 1;
+          tc_fence_after();
+          if (!((rows >> m) & 1)) {                          // warp-uniform: only padding rows in this quadrant
+            epilogue_skip(b_full + 16 + 8 * ACC, lane0);
+            return;
+          }
+          epilogue_tile<NINT_T>(t_lane + ACC * TILE_T, out + m * mstride, (wr >> m) & 1, nvalid, NINT_T != 0 && vec_ok,
+                                b_full + 16 + 8 * ACC, lane0);
+        };
+        if constexpr (GROUP == 1) {
+          if (i & 1) one(std::integral_constant<int, 1>{}, 0);
+          else one(std::integral_constant<int, 0>{}, 0);
         } else {
-          epilogue_tile<NINT_T>(t_lane + acc * TILE_T, base + m * mstride + it.tt * BPT, writer,
-                                p.nbin - (it.tt * BPT + slot * BPW), vec_ok, b_empty + 8 * acc, lane0);
+#pragma unroll
+          for (int m = 0; m < GROUP; ++m)
+            if (m < gm) {
+              if (m & 1) one(std::integral_constant<int, 1>{}, m);
+              else one(std::integral_constant<int, 0>{}, m);
+            }
         }
       }
+      it.tt = 0;
+      if (++it.g == nG) { it.g = 0; ++it.c; }
     }
   } else if (cw >= 0) {
     // =========================================================================== convert
@@ -181,20 +212,71 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
       const int t = pc / npr, q = pc - t * npr;
       p_dst[k] = pc < npieces ? (uint32_t)((t >> 3) * 1024 + (t & 7) * 128 + (((CPP * q) ^ (t & 7)) << 4)) : 0xffffffffu;
     }
-    for (int i = 0; i < n_items; ++i) {
-      const int rs = i % NRAW;
-      mbar_wait(bar_r_full + 8 * rs, (i / NRAW) & 1);
-      uint4 x[PIECES];
-      convert_load<PIECES, CONV_THREADS>(sR + rs * RAW_STAGE_BYTES, ctid, p_dst, x);
-      const int st = i % NSTAGE;
-      mbar_wait(bar_b_empty + 8 * st, ((i / NSTAGE) & 1) ^ 1);
-      if (IN == BF_CI4) convert_store_ci4<PIECES>(sB + st * B_STAGE_BYTES, p_dst, x);
-      else convert_store<PIECES>(sB + st * B_STAGE_BYTES, p_dst, x);
-      fence_proxy_async_smem();
-      __syncwarp();
-      if (lane == 0) {
-        mbar_arrive(bar_r_empty + 8 * rs);  // raw bytes are in registers / converted: slot may be refilled
-        mbar_arrive(bar_b_full + 8 * st);
+    int rs = 0, st = 0;              // raw slot / operand stage of the current item
+    uint32_t rpar = 0, bpar = 1;     // parities to wait for on r_full[rs] / b_empty[st]
+    if (npieces == PIECES * CONV_THREADS) {
+      // ---- full rows (nant = 32): every thread owns PIECES pieces, piece k sits KSTEP bytes after
+      // piece 0 in the operand stage and 16 * CONV_THREADS bytes after it in the raw slot, so all
+      // shared-memory accesses are [register + immediate]
+      constexpr int FULL_NPR = IN == BF_CI4 ? 2 : 4;
+      constexpr uint32_t KSTEP = (CONV_THREADS / FULL_NPR / 8) * 1024;
+      uint32_t raw = sR + 16 * ctid, dst = sB + p_dst[0];
+      for (int i = 0; i < n_items; ++i) {
+        mbar_wait(bar_r_full + 8 * rs, rpar);
+        uint4 x[PIECES];
+#pragma unroll
+        for (int k = 0; k < PIECES; ++k) x[k] = ld_shared_v4(raw + k * (16 * CONV_THREADS));
+        mbar_wait(bar_b_empty + 8 * st, bpar);
+        if (IN == BF_CI4) {
+          const uint32_t d1 = dst ^ 16u, d2 = dst ^ 32u, d3 = dst ^ 48u;
+#pragma unroll
+          for (int k = 0; k < PIECES; ++k) {
+            uint32_t h[4];
+            cvt_i4x8_f16x8(x[k].x, h); st_shared_v4(dst + k * KSTEP, h[0], h[1], h[2], h[3]);
+            cvt_i4x8_f16x8(x[k].y, h); st_shared_v4(d1 + k * KSTEP, h[0], h[1], h[2], h[3]);
+            cvt_i4x8_f16x8(x[k].z, h); st_shared_v4(d2 + k * KSTEP, h[0], h[1], h[2], h[3]);
+            cvt_i4x8_f16x8(x[k].w, h); st_shared_v4(d3 + k * KSTEP, h[0], h[1], h[2], h[3]);
+          }
+        } else {
+          const uint32_t d1 = dst ^ 16u;
+#pragma unroll
+          for (int k = 0; k < PIECES; ++k) {
+            uint32_t h[8];
+            cvt_i8x4_f16x4(x[k].x, h[0], h[1]);
+            cvt_i8x4_f16x4(x[k].y, h[2], h[3]);
+            cvt_i8x4_f16x4(x[k].z, h[4], h[5]);
+            cvt_i8x4_f16x4(x[k].w, h[6], h[7]);
+            st_shared_v4(dst + k * KSTEP, h[0], h[1], h[2], h[3]);
+            st_shared_v4(d1 + k * KSTEP, h[4], h[5], h[6], h[7]);
+          }
+        }
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(bar_r_empty + 8 * rs);  // raw bytes are converted: slot may be refilled
+          mbar_arrive(bar_b_full + 8 * st);
+        }
+        raw += RAW_STAGE_BYTES; dst += B_STAGE_BYTES;
+        if (++rs == NRAW) { rs = 0; rpar ^= 1; raw -= NRAW * RAW_STAGE_BYTES; }
+        if (++st == NSTAGE) { st = 0; bpar ^= 1; dst -= NSTAGE * B_STAGE_BYTES; }
+      }
+    } else {
+      // ---- short rows (nant < 32): generic piece table
+      for (int i = 0; i < n_items; ++i) {
+        mbar_wait(bar_r_full + 8 * rs, rpar);
+        uint4 x[PIECES];
+        convert_load<PIECES, CONV_THREADS>(sR + rs * RAW_STAGE_BYTES, ctid, p_dst, x);
+        mbar_wait(bar_b_empty + 8 * st, bpar);
+        if (IN == BF_CI4) convert_store_ci4<PIECES>(sB + st * B_STAGE_BYTES, p_dst, x);
+        else convert_store<PIECES>(sB + st * B_STAGE_BYTES, p_dst, x);
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(bar_r_empty + 8 * rs);  // raw bytes are in registers / converted: slot may be refilled
+          mbar_arrive(bar_b_full + 8 * st);
+        }
+        if (++rs == NRAW) { rs = 0; rpar ^= 1; }
+        if (++st == NSTAGE) { st = 0; bpar ^= 1; }
       }
     }
   } else if (mw >= 0) {
@@ -205,6 +287,8 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     // warp 0 is blocked issuing into stage 0, warp 1 does its waits for stage 1 and queues behind it.
     // The whole warp walks the loop (all values warp-uniform); one elected lane issues.
     const int id = mw;  // = the accumulator stage this warp feeds
+    // stage of a tile (the epilogue uses the same compile-time rule): GROUP even -> tile m of an item
+    // goes to stage m & 1; GROUP == 1 -> item i goes to stage i & 1
     constexpr uint32_t idesc = make_idesc_f16(BF_TILE_ROWS, TILE_T);
     const uint64_t adesc0 = make_sdesc_k_sw128(sA);
     const uint64_t bdesc0 = make_sdesc_k_sw128(sB);
@@ -214,7 +298,6 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     int st = 0;                 // operand stage and the parity its "full" barrier completes next
     uint32_t st_par = 0;
     uint32_t te_par = 1;        // parity of t_empty[id] to wait for (first use passes on the fresh barrier)
-    int u = 0;                  // running accumulator-tile index; tile u goes to stage u & 1
     int gm = min(GROUP, nMt - it.g * GROUP);
     for (int i = 0; i < n_items; ++i) {
       if (i == 0 || it.tt == 0) {  // (chan, beam group) changes exactly when the time tile wraps
@@ -224,11 +307,11 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         mbar_wait(bar_a_full + 8 * ab, (ag >> 1) & 1);
         ++ag;
       }
-      const int m0 = ((u & 1) == id) ? 0 : 1;  // my tiles of this item: m0, m0 + 2, ...
-      if (m0 < gm) {
+      const bool mine = GROUP == 1 ? ((i & 1) == id) : (id < gm);
+      if (mine) {
         mbar_wait(bar_b_full + 8 * st, st_par);
         const uint64_t bdesc = bdesc0 + (uint64_t)(st * (B_STAGE_BYTES >> 4));
-        for (int m = m0; m < gm; m += 2) {
+        for (int m = (GROUP == 1 ? 0 : id); m < gm; m += 2) {
           mbar_wait(bar_t_empty + 8 * id, te_par);
           te_par ^= 1;
           tc_fence_after();
@@ -245,7 +328,6 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
           }
         }
       }
-      u += gm;
       if (++st == NSTAGE) { st = 0; st_par ^= 1; }
       next_item(it, nG, nTt);
     }
