@@ -45,6 +45,8 @@ def _load():
         lib.oracle_beamform.argtypes = [ctypes.c_int] * 6 + [dp, dp, dp, ctypes.c_void_p, dp, ctypes.c_int]
         lib.oracle_beams.restype = ctypes.c_int
         lib.oracle_beams.argtypes = [ctypes.c_int] * 5 + [dp, dp, dp, ctypes.c_void_p, dp]
+        lib.oracle_incoherent.restype = ctypes.c_int
+        lib.oracle_incoherent.argtypes = [ctypes.c_int] * 5 + [ctypes.c_void_p, dp]
         _lib = lib
     return _lib
 
@@ -120,4 +122,18 @@ def beams(ant_xyz, chan_freq_hz, beam_dir, voltages) -> np.ndarray:
                               v.ctypes.data_as(ctypes.c_void_p), _dp(out.view(np.float64)))
     if rc != 0:
         raise ValueError(f"oracle_beams failed rc={rc}")
+    return out
+
+
+def incoherent(voltages, nint: int) -> np.ndarray:
+    """Incoherent beam P_inc[c][j] = sum over the bin and over antennas of |x|^2, fp64."""
+    v = np.ascontiguousarray(voltages)
+    nchan, nant = v.shape[0], v.shape[2]
+    v, dt, nsamp = _volt(v, nchan, nant)
+    if nint <= 0 or nsamp % nint != 0:
+        raise ValueError("nsamp must be a positive multiple of nint")
+    out = np.empty((nchan, nsamp // nint), dtype=np.float64)
+    rc = _load().oracle_incoherent(nant, nchan, nsamp, nint, dt, v.ctypes.data_as(ctypes.c_void_p), _dp(out))
+    if rc != 0:
+        raise ValueError(f"oracle_incoherent failed rc={rc}")
     return out

@@ -21,7 +21,7 @@
  * time summed in plain t order, no blocking, no fusion, no normalisation (reading A6).
  * OpenMP splits the channel loop only (channels are independent).
  *
- * Pins (tests/test_oracle_pins.py): Eq. 1 closed forms for a linear and a grid array,
+ * Pins (tests/test_oracle_pins.py; incoherent and voltage beams: tests/test_oracle_pins_modes.py): Eq. 1 closed forms for a linear and a grid array,
  * N^2 A^2 coherent gain, incoherent N level, a Parseval identity on a DFT beam grid, hand
  * cases with N=1 and N=2, algebraic invariants, and an independent numpy einsum.
  * Unpinned: value-level agreement with the paper itself -- it prints no beam powers
@@ -173,5 +173,30 @@ int oracle_beams(int nant, int nchan, int nbeam, int nsamp, int dtype, const dou
       }
   }
   free(wr); free(wi);
+  return 0;
+}
+
+/*
+ * Incoherent beam: "Squaring and adding the signals of all the elements together is the process of
+ * incoherent beamforming" -- the wide-field, low-sensitivity alternative the paper names
+ * next to coherent beams.  No weights, no geometry:
+ *     P_inc[c][j] = sum_{t=jI}^{(j+1)I-1} sum_n |x[c][t][n]|^2
+ * out: [nchan][nsamp/nint] fp64.  Plain t, n order, fp64, no normalisation (reading A6).
+ */
+int oracle_incoherent(int nant, int nchan, int nsamp, int nint, int dtype, const void *voltages, double *out) {
+  if (nant <= 0 || nchan <= 0 || nsamp <= 0 || nint <= 0 || nsamp % nint != 0) return -1;
+  if (dtype != ORACLE_CI8 && dtype != ORACLE_CF16 && dtype != ORACLE_C128 && dtype != ORACLE_CI4) return -1;
+  const int nbin = nsamp / nint;
+  for (int c = 0; c < nchan; ++c)
+    for (int j = 0; j < nbin; ++j) {
+      double acc = 0.0;
+      for (int t = j * nint; t < (j + 1) * nint; ++t)
+        for (int n = 0; n < nant; ++n) {
+          double xr, xi;
+          load_sample(voltages, dtype, ((size_t)c * nsamp + t) * nant + n, &xr, &xi);
+          acc += xr * xr + xi * xi;
+        }
+      out[(size_t)c * nbin + j] = acc;
+    }
   return 0;
 }
