@@ -105,6 +105,25 @@ int bf_set_geometry(bf_ctx *ctx, const double *ant_xyz_m, const double *chan_fre
                     const double *beam_dir, void *stream);
 
 /*
+ * Tracking beams.  The paper recomputes the coefficients between pipeline
+ * iterations so that "beam pointings [can] change dynamically during pipeline execution, which is useful
+ * for tracking observations" (stationary and tracking beams: PAPER.md:180).  With two
+ * weight buffers the regeneration overlaps the beamforming of the current block:
+ *   bf_set_weight_buffers(ctx, 2)   before bf_workspace_bytes / bf_set_workspace (the workspace doubles)
+ *   bf_update_geometry(...)         same arguments and validation as bf_set_geometry, but the new weights are
+ *                                   generated into the buffer the kernels are NOT reading, on `update_stream`
+ *                                   (any stream; it may differ from the run stream).  Calls to bf_run* that
+ *                                   were enqueued before keep the old weights; the NEXT bf_run* call waits (on
+ *                                   the device, through an event) for the generator and switches over.  The
+ *                                   library also orders a later update behind the last run that still reads
+ *                                   the buffer it is about to overwrite, so no host synchronisation is needed.
+ * BF_EINVAL without two buffers; BF_ENOGEOM before the first bf_set_geometry.
+ */
+int bf_set_weight_buffers(bf_ctx *ctx, int n);
+int bf_update_geometry(bf_ctx *ctx, const double *ant_xyz_m, const double *chan_freq_hz,
+                       const double *beam_dir, void *update_stream);
+
+/*
  * Per-antenna complex gains folded into the weights: W'[c][b][n] = g[c][n] * W[c][b][n].  This is the
  * paper's sub-arraying "antenna mask in the kernel" (g = 0 drops an antenna) and the gain
  * calibration its X-engine provides -- free in the beamforming kernel because only the
@@ -128,6 +147,27 @@ int bf_get_weights(bf_ctx *ctx, float *host_out, void *stream);
  * Enqueues on `stream` and returns.  BF_ENOGEOM before bf_set_geometry.
  */
 int bf_run(bf_ctx *ctx, const void *voltages, float *powers, void *stream);
+
+/*
+ * Voltage-beam output: the raw complex beams y[c][b][t] = sum_n W x, with no
+ * detection and no integration -- the S-engine's "electric-field ... beams ... output as 16-bit
+ * complex-valued words" for downstream coherent processing.  Same contraction, same kernels,
+ * a different epilogue.
+ *   beams  DEVICE fp16 (re, im) pairs, [nchan][nbeam][nsamp][2], 4-byte aligned (16-byte aligned and
+ *          nsamp % 4 == 0 for vector stores), fully overwritten with fp16(scale * y)
+ *   scale  finite, non-zero; choose it so that scale * |y| stays below 65504 (|y| <= nant * max|x|)
+ * nint is ignored.  BF_ENOGEOM before bf_set_geometry.
+ */
+int bf_run_beams(bf_ctx *ctx, const void *voltages, void *beams, float scale, void *stream);
+
+/*
+ * Incoherent beam: "squaring and adding the signals of all the elements together"
+ * (PAPER.md:21), the wide-field alternative to coherent beams:
+ *   powers[c][j] = sum_{t=j*nint}^{(j+1)*nint-1} sum_n |x[c][t][n]|^2     DEVICE fp32 [nchan][nsamp/nint]
+ * Needs neither geometry nor workspace (there are no weights).  Integer inputs are summed exactly and
+ * rounded once to fp32.
+ */
+int bf_run_incoherent(bf_ctx *ctx, const void *voltages, float *powers, void *stream);
 
 /*
  * End-to-end variant with HOST buffers (the paper's PCIe concern: "this data overhead

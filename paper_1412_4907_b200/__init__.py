@@ -36,6 +36,10 @@ SYMBOLS = {
     "bf_set_antenna_gains": (_i, [_vp, _dp, _i, _vp]),
     "bf_get_weights": (_i, [_vp, _vp, _vp]),
     "bf_run": (_i, [_vp, _vp, _vp, _vp]),
+    "bf_run_beams": (_i, [_vp, _vp, _vp, ctypes.c_float, _vp]),
+    "bf_run_incoherent": (_i, [_vp, _vp, _vp, _vp]),
+    "bf_set_weight_buffers": (_i, [_vp, _i]),
+    "bf_update_geometry": (_i, [_vp, _dp, _dp, _dp, _vp]),
     "bf_staging_bytes": (_sz, [_vp, _i]),
     "bf_run_host": (_i, [_vp, _vp, _vp, _vp, _sz, _i, _vp, _vp]),
     "bf_run_streaming": (_i, [_vp, ctypes.POINTER(_vp), _i, _vp, _vp, _sz, _vp, _vp]),
@@ -133,6 +137,20 @@ def bf_set_geometry(ctx, ant_xyz_m, chan_freq_hz, beam_dir, stream=None):
     return lib().bf_set_geometry(ctx, pa, pf, pd, _stream(stream))
 
 
+def bf_set_weight_buffers(ctx, n):
+    return lib().bf_set_weight_buffers(ctx, int(n))
+
+
+def bf_update_geometry(ctx, ant_xyz_m, chan_freq_hz, beam_dir, update_stream=None):
+    import numpy as np
+
+    a = np.ascontiguousarray(ant_xyz_m, dtype=np.float64)
+    f = np.ascontiguousarray(chan_freq_hz, dtype=np.float64)
+    d = np.ascontiguousarray(beam_dir, dtype=np.float64)
+    return lib().bf_update_geometry(ctx, a.ctypes.data_as(_dp), f.ctypes.data_as(_dp), d.ctypes.data_as(_dp),
+                                    _stream(update_stream))
+
+
 def bf_set_antenna_gains(ctx, gains, per_channel=False, stream=None):
     """gains: complex array [nant] (or [nchan][nant] with per_channel), or None to reset to 1."""
     import numpy as np
@@ -149,6 +167,14 @@ def bf_get_weights(ctx, host_out, stream=None):
 
 def bf_run(ctx, voltages, powers, stream=None):
     return lib().bf_run(ctx, _ptr(voltages), _ptr(powers), _stream(stream))
+
+
+def bf_run_beams(ctx, voltages, beams, scale=1.0, stream=None):
+    return lib().bf_run_beams(ctx, _ptr(voltages), _ptr(beams), float(scale), _stream(stream))
+
+
+def bf_run_incoherent(ctx, voltages, powers, stream=None):
+    return lib().bf_run_incoherent(ctx, _ptr(voltages), _ptr(powers), _stream(stream))
 
 
 def bf_staging_bytes(ctx, chan_per_chunk):
@@ -181,7 +207,8 @@ def bf_version():
 class Beamformer:
     """Owns a bf_ctx plus its device workspace (a torch uint8 tensor)."""
 
-    def __init__(self, nant, nchan, nbeam, nsamp, nint, dtype=BF_CI8, kernel=BF_KERNEL_AUTO, device="cuda:0"):
+    def __init__(self, nant, nchan, nbeam, nsamp, nint, dtype=BF_CI8, kernel=BF_KERNEL_AUTO, device="cuda:0",
+                 weight_buffers=1):
         import torch
 
         self.shape = (nant, nchan, nbeam, nsamp, nint)
@@ -190,6 +217,7 @@ class Beamformer:
             raise BfError(BF_EINVAL, "bf_create rejected the sizes (all > 0, nsamp % nint == 0)")
         self._check(bf_set_dtype(self.ctx, dtype))
         self._check(bf_set_kernel(self.ctx, kernel))
+        self._check(bf_set_weight_buffers(self.ctx, weight_buffers))
         self.dtype = dtype
         self.device = torch.device(device)
         nbytes = bf_workspace_bytes(self.ctx)
@@ -208,6 +236,10 @@ class Beamformer:
 
     def set_geometry(self, ant_xyz_m, chan_freq_hz, beam_dir, stream=None):
         self._check(bf_set_geometry(self.ctx, ant_xyz_m, chan_freq_hz, beam_dir, stream))
+
+    def update_geometry(self, ant_xyz_m, chan_freq_hz, beam_dir, update_stream=None):
+        """Tracking beams: regenerate the weights into the inactive buffer on `update_stream`."""
+        self._check(bf_update_geometry(self.ctx, ant_xyz_m, chan_freq_hz, beam_dir, update_stream))
 
     def set_antenna_gains(self, gains, per_channel=False, stream=None):
         self._check(bf_set_antenna_gains(self.ctx, gains, per_channel, stream))
@@ -234,6 +266,30 @@ class Beamformer:
         if stream is None:
             stream = torch.cuda.current_stream(self.device)
         self._check(bf_run(self.ctx, voltages, powers, stream))
+        return powers
+
+    def run_beams(self, voltages, beams=None, scale=1.0, stream=None):
+        """Voltage beams y[c][b][t] as fp16 (re, im): tensor [nchan][nbeam][nsamp][2]."""
+        import torch
+
+        nant, nchan, nbeam, nsamp, nint = self.shape
+        if beams is None:
+            beams = torch.empty((nchan, nbeam, nsamp, 2), dtype=torch.float16, device=self.device)
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        self._check(bf_run_beams(self.ctx, voltages, beams, scale, stream))
+        return beams
+
+    def run_incoherent(self, voltages, powers=None, stream=None):
+        """Incoherent beam sum_n |x_n|^2 integrated over nint: tensor [nchan][nsamp // nint] fp32."""
+        import torch
+
+        nant, nchan, nbeam, nsamp, nint = self.shape
+        if powers is None:
+            powers = torch.empty((nchan, nsamp // nint), dtype=torch.float32, device=self.device)
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        self._check(bf_run_incoherent(self.ctx, voltages, powers, stream))
         return powers
 
     def _get_staging(self, nbytes):

@@ -59,6 +59,9 @@ extern "C" bf_ctx *bf_create(int nant, int nchan, int nbeam, int nsamp, int nint
   c->launches = 0;
   c->sm_count = 0; c->device_ok = -1;
   c->have_events = false;
+  c->nwbuf = 1; c->active = 0; c->pending = -1;
+  c->geom_buf[0] = c->geom_buf[1] = nullptr; c->wop_buf[0] = c->wop_buf[1] = nullptr;
+  c->have_wevents = false; c->used[0] = c->used[1] = false;
   c->err[0] = 0;
   return c;
 }
@@ -67,6 +70,7 @@ extern "C" void bf_destroy(bf_ctx *c) {
   if (!c) return;
   if (c->have_events)
     for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_copied[i]); cudaEventDestroy(c->ev_done[i]); }
+  if (c->have_wevents) { cudaEventDestroy(c->ev_upd); cudaEventDestroy(c->ev_use[0]); cudaEventDestroy(c->ev_use[1]); }
   delete c;
 }
 
@@ -96,9 +100,29 @@ extern "C" int bf_selected_kernel(const bf_ctx *c) {
 
 extern "C" long long bf_launch_count(const bf_ctx *c) { return c ? c->launches : 0; }
 
+static size_t wop_bytes(const bf_ctx *c) { return align_up((size_t)c->nchan * bf_wop_bytes_per_chan(c), BF_ALIGN); }
+
 extern "C" size_t bf_workspace_bytes(const bf_ctx *c) {
   if (!c) return 0;
-  return geom_bytes(c) + align_up((size_t)c->nchan * bf_wop_bytes_per_chan(c), BF_ALIGN);
+  return (size_t)c->nwbuf * (geom_bytes(c) + wop_bytes(c));
+}
+
+extern "C" int bf_set_weight_buffers(bf_ctx *c, int n) {
+  if (!c) return BF_EINVAL;
+  if (n != 1 && n != 2) return fail(c, BF_EINVAL, "weight buffers must be 1 or 2");
+  if (c->ws) return fail(c, BF_EINVAL, "bf_set_weight_buffers must be called before bf_set_workspace");
+  c->nwbuf = n;
+  return BF_OK;
+}
+
+// point the generator / the kernels at (geometry, weight operand) buffer i
+static void select_buffer(bf_ctx *c, int i) {
+  char *p = c->geom_buf[i];
+  c->d_ant = (double *)p;
+  c->d_freq = c->d_ant + 3 * (size_t)c->nant;
+  c->d_dir = c->d_freq + c->nchan;
+  c->d_gain = c->d_dir + 3 * (size_t)c->nbeam;
+  c->d_wop = c->wop_buf[i];
 }
 
 // no fallback: the device must be Blackwell (compute capability 10.x)
@@ -129,17 +153,17 @@ extern "C" int bf_set_workspace(bf_ctx *c, void *dev_ptr, size_t bytes) {
   c->ws = dev_ptr;
   c->ws_bytes = bytes;
   char *p = (char *)dev_ptr;
-  c->d_ant = (double *)p;
-  c->d_freq = c->d_ant + 3 * (size_t)c->nant;
-  c->d_dir = c->d_freq + c->nchan;
-  c->d_gain = c->d_dir + 3 * (size_t)c->nbeam;
-  c->d_wop = (__half *)(p + geom_bytes(c));
+  for (int i = 0; i < c->nwbuf; ++i) {
+    c->geom_buf[i] = p + (size_t)i * geom_bytes(c);
+    c->wop_buf[i] = (__half *)(p + (size_t)c->nwbuf * geom_bytes(c) + (size_t)i * wop_bytes(c));
+  }
+  c->active = 0; c->pending = -1; c->used[0] = c->used[1] = false;
+  select_buffer(c, 0);
   c->have_geom = false;
   return BF_OK;
 }
 
-extern "C" int bf_set_geometry(bf_ctx *c, const double *ant, const double *freq, const double *dir, void *stream) {
-  if (!c) return BF_EINVAL;
+static int check_geometry(bf_ctx *c, const double *ant, const double *freq, const double *dir) {
   if (!ant || !freq || !dir) return fail(c, BF_EINVAL, "geometry pointer is NULL");
   for (int i = 0; i < 3 * c->nant; ++i)
     if (!isfinite(ant[i])) return fail(c, BF_EINVAL, "antenna position %d is not finite", i / 3);
@@ -149,15 +173,16 @@ extern "C" int bf_set_geometry(bf_ctx *c, const double *ant, const double *freq,
     double n2 = dir[3 * b] * dir[3 * b] + dir[3 * b + 1] * dir[3 * b + 1] + dir[3 * b + 2] * dir[3 * b + 2];
     if (!isfinite(n2) || fabs(sqrt(n2) - 1.0) > 1e-6) return fail(c, BF_EINVAL, "beam direction %d is not a unit vector", b);
   }
-  if (!c->ws) return fail(c, BF_ENOGEOM, "bf_set_workspace must be called before bf_set_geometry");
-  int rc = probe_device(c);
-  if (rc != BF_OK) return rc;
+  return BF_OK;
+}
+
+// copy the geometry (+ gains) into the currently selected buffer and generate its weights on `st`
+static int upload_and_generate(bf_ctx *c, const double *ant, const double *freq, const double *dir, cudaStream_t st) {
   size_t na = 3 * (size_t)c->nant, nf = c->nchan, nd = 3 * (size_t)c->nbeam;
   c->h_geom.resize(na + nf + nd);
   memcpy(c->h_geom.data(), ant, na * sizeof(double));
   memcpy(c->h_geom.data() + na, freq, nf * sizeof(double));
   memcpy(c->h_geom.data() + na + nf, dir, nd * sizeof(double));
-  cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e = cudaMemcpyAsync(c->d_ant, c->h_geom.data(), (na + nf + nd) * sizeof(double), cudaMemcpyHostToDevice, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "geometry H2D copy");
   if (c->have_gains) {
@@ -167,7 +192,54 @@ extern "C" int bf_set_geometry(bf_ctx *c, const double *ant, const double *freq,
   e = bf_launch_weights(c, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "weight generator launch");
   c->launches += 1;
+  return BF_OK;
+}
+
+extern "C" int bf_set_geometry(bf_ctx *c, const double *ant, const double *freq, const double *dir, void *stream) {
+  if (!c) return BF_EINVAL;
+  int rc = check_geometry(c, ant, freq, dir);
+  if (rc != BF_OK) return rc;
+  if (!c->ws) return fail(c, BF_ENOGEOM, "bf_set_workspace must be called before bf_set_geometry");
+  if ((rc = probe_device(c)) != BF_OK) return rc;
+  if (c->pending >= 0) {  // an update in flight is superseded: this call defines the weights of the next run
+    c->active = c->pending; c->pending = -1;
+    cudaStreamWaitEvent((cudaStream_t)stream, c->ev_upd, 0);
+  }
+  select_buffer(c, c->active);
+  if ((rc = upload_and_generate(c, ant, freq, dir, (cudaStream_t)stream)) != BF_OK) return rc;
   c->have_geom = true;
+  return BF_OK;
+}
+
+static int ensure_wevents(bf_ctx *c) {
+  if (c->have_wevents) return BF_OK;
+  cudaError_t e = cudaEventCreateWithFlags(&c->ev_upd, cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_use[0], cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_use[1], cudaEventDisableTiming);
+  if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventCreate");
+  c->have_wevents = true;
+  return BF_OK;
+}
+
+// Tracking beams (row f3): new pointings are generated into the buffer the kernels are
+// NOT reading, on the caller's update stream, while bf_run keeps using the active one.
+extern "C" int bf_update_geometry(bf_ctx *c, const double *ant, const double *freq, const double *dir, void *update_stream) {
+  if (!c) return BF_EINVAL;
+  if (c->nwbuf != 2) return fail(c, BF_EINVAL, "bf_update_geometry needs bf_set_weight_buffers(ctx, 2)");
+  int rc = check_geometry(c, ant, freq, dir);
+  if (rc != BF_OK) return rc;
+  if (!c->have_geom) return fail(c, BF_ENOGEOM, "bf_set_geometry must be called once before bf_update_geometry");
+  if ((rc = ensure_wevents(c)) != BF_OK) return rc;
+  cudaStream_t us = (cudaStream_t)update_stream;
+  const int target = 1 - c->active;  // a second update before any run overwrites the same (unused) buffer
+  // runs that read `target` before the last switch may still be executing on the run stream
+  if (c->used[target]) cudaStreamWaitEvent(us, c->ev_use[target], 0);
+  select_buffer(c, target);
+  rc = upload_and_generate(c, ant, freq, dir, us);
+  select_buffer(c, c->active);
+  if (rc != BF_OK) return rc;
+  cudaEventRecord(c->ev_upd, us);
+  c->pending = target;
   return BF_OK;
 }
 
@@ -192,6 +264,11 @@ extern "C" int bf_set_antenna_gains(bf_ctx *c, const double *gains, int per_chan
   }
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e = cudaSuccess;
+  if (c->pending >= 0) {  // regenerate the weights the next run will use
+    c->active = c->pending; c->pending = -1;
+    cudaStreamWaitEvent(st, c->ev_upd, 0);
+    select_buffer(c, c->active);
+  }
   if (c->have_gains) e = cudaMemcpyAsync(c->d_gain, c->h_gain.data(), c->h_gain.size() * sizeof(double), cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) e = bf_launch_weights(c, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "weight regeneration");
@@ -204,6 +281,11 @@ extern "C" int bf_get_weights(bf_ctx *c, float *host_out, void *stream) {
   if (!host_out) return fail(c, BF_EINVAL, "output pointer is NULL");
   if (!c->have_geom) return fail(c, BF_ENOGEOM, "no geometry set");
   cudaStream_t st = (cudaStream_t)stream;
+  if (c->pending >= 0) {  // report the weights the next run will use
+    cudaStreamWaitEvent(st, c->ev_upd, 0);
+    c->active = c->pending; c->pending = -1;
+    select_buffer(c, c->active);
+  }
   size_t bytes = (size_t)c->nchan * c->nbeam * c->nant * 2 * sizeof(float);
   float *d = nullptr;  // verification helper: the one place the library allocates device memory itself
   cudaError_t e = cudaMalloc(&d, bytes);
@@ -216,17 +298,23 @@ extern "C" int bf_get_weights(bf_ctx *c, float *host_out, void *stream) {
   return BF_OK;
 }
 
-// launch the selected kernel over channels [chan0, chan0 + nchan_run)
-static int launch_range(bf_ctx *c, const void *volt, float *pow, int chan0, int nchan_run, cudaStream_t st) {
+// launch the selected kernel over channels [chan0, chan0 + nchan_run); mode BF_MODE_POWER writes `out` as
+// fp32 powers, BF_MODE_BEAMS as fp16 (re, im) voltage beams scaled by `scale`
+static int launch_range(bf_ctx *c, const void *volt, void *out, int chan0, int nchan_run, cudaStream_t st,
+                        int mode = BF_MODE_POWER, float scale = 1.f) {
   BfParams p;
   p.nant = c->nant; p.nbeam = c->nbeam; p.nsamp = c->nsamp; p.nint = c->nint; p.nbin = c->nbin;
   p.nMt = c->nMt; p.nKb = c->nKb;
   p.nchan_run = nchan_run;
-  p.volt = volt; p.pow = pow;
+  p.volt = volt;
+  p.pow = mode == BF_MODE_POWER ? (float *)out : nullptr;
+  p.beams = mode == BF_MODE_BEAMS ? out : nullptr;
+  p.beam_scale = scale;
+  p.mode = mode;
   p.wop = c->d_wop + (size_t)chan0 * (bf_wop_bytes_per_chan(c) / sizeof(__half));
   int k = c->kernel_forced;
   const char *why = "";
-  bool umma_ok = bf_umma_supported(c, &why);
+  bool umma_ok = mode == BF_MODE_BEAMS ? bf_umma_shape_supported(c, &why) : bf_umma_supported(c, &why);
   if (k == BF_KERNEL_AUTO) k = umma_ok ? BF_KERNEL_UMMA : BF_KERNEL_SIMT;
   if (k == BF_KERNEL_UMMA && !umma_ok) return fail(c, BF_EUNSUPPORTED, "tensor-core kernel cannot run this shape: %s", why);
   cudaError_t e = (k == BF_KERNEL_UMMA) ? bf_launch_umma(p, c->dtype, c->sm_count, st) : bf_launch_simt(p, c->dtype, st);
@@ -242,11 +330,54 @@ static int check_run(bf_ctx *c, const void *volt, const void *pow) {
   return probe_device(c);
 }
 
+// tracking beams (row f3): switch to freshly generated weights once their generator has finished
+static void begin_run(bf_ctx *c, cudaStream_t st) {
+  if (c->pending >= 0) {
+    cudaStreamWaitEvent(st, c->ev_upd, 0);
+    c->active = c->pending;
+    c->pending = -1;
+    select_buffer(c, c->active);
+  }
+}
+// ... and remember when the last reader of the active buffer is done, for the next update of it
+static void end_run(bf_ctx *c, cudaStream_t st) {
+  if (c->nwbuf == 2 && ensure_wevents(c) == BF_OK) {
+    cudaEventRecord(c->ev_use[c->active], st);
+    c->used[c->active] = true;
+  }
+}
+
 extern "C" int bf_run(bf_ctx *c, const void *voltages, float *powers, void *stream) {
   int rc = check_run(c, voltages, powers);
   if (rc != BF_OK) return rc;
   if (((uintptr_t)voltages) % 16) return fail(c, BF_EINVAL, "voltages must be 16-byte aligned");
-  return launch_range(c, voltages, powers, 0, c->nchan, (cudaStream_t)stream);
+  begin_run(c, (cudaStream_t)stream);
+  rc = launch_range(c, voltages, powers, 0, c->nchan, (cudaStream_t)stream);
+  end_run(c, (cudaStream_t)stream);
+  return rc;
+}
+
+extern "C" int bf_run_beams(bf_ctx *c, const void *voltages, void *beams, float scale, void *stream) {
+  int rc = check_run(c, voltages, beams);
+  if (rc != BF_OK) return rc;
+  if (((uintptr_t)voltages) % 16) return fail(c, BF_EINVAL, "voltages must be 16-byte aligned");
+  if (((uintptr_t)beams) % 4) return fail(c, BF_EINVAL, "beams must be 4-byte aligned");
+  if (!isfinite(scale) || scale == 0.f) return fail(c, BF_EINVAL, "scale must be finite and non-zero");
+  begin_run(c, (cudaStream_t)stream);
+  rc = launch_range(c, voltages, beams, 0, c->nchan, (cudaStream_t)stream, BF_MODE_BEAMS, scale);
+  end_run(c, (cudaStream_t)stream);
+  return rc;
+}
+
+extern "C" int bf_run_incoherent(bf_ctx *c, const void *voltages, float *powers, void *stream) {
+  if (!c) return BF_EINVAL;
+  if (!voltages || !powers) return fail(c, BF_EINVAL, "voltages / powers pointer is NULL");
+  int rc = probe_device(c);  // needs neither geometry nor workspace: there are no weights
+  if (rc != BF_OK) return rc;
+  cudaError_t e = bf_launch_incoherent(c, voltages, powers, (cudaStream_t)stream);
+  if (e != cudaSuccess) return cuda_fail(c, e, "incoherent-beam kernel launch");
+  c->launches += 1;
+  return BF_OK;
 }
 
 static int ensure_events(bf_ctx *c) {
@@ -285,6 +416,7 @@ extern "C" int bf_run_host(bf_ctx *c, const void *host_volt, float *host_pow, vo
   char *out[2] = {(char *)staging + 2 * in_buf, (char *)staging + 2 * in_buf + out_buf};
   cudaError_t e;
   int k = 0;
+  begin_run(c, cs);
   for (int c0 = 0; c0 < c->nchan; c0 += chan_per_chunk, ++k) {
     int n = c->nchan - c0 < chan_per_chunk ? c->nchan - c0 : chan_per_chunk;
     int b = k & 1;
@@ -302,6 +434,7 @@ extern "C" int bf_run_host(bf_ctx *c, const void *host_volt, float *host_pow, vo
   // the next call on this context must not overwrite staging that is still in flight
   cudaStreamWaitEvent(xs, c->ev_done[0], 0);
   if (k > 1) cudaStreamWaitEvent(xs, c->ev_done[1], 0);
+  end_run(c, cs);
   return BF_OK;
 }
 
@@ -321,6 +454,7 @@ extern "C" int bf_run_streaming(bf_ctx *c, const void *const *host_blocks, int n
   const size_t out_elems = (size_t)c->nchan * c->nbeam * c->nbin;
   char *in[2] = {(char *)staging, (char *)staging + in_buf};
   cudaError_t e;
+  begin_run(c, cs);
   for (int i = 0; i < nblocks; ++i) {
     int b = i & 1;
     if (i >= 2 && (e = cudaStreamWaitEvent(xs, c->ev_done[b], 0)) != cudaSuccess) return cuda_fail(c, e, "cudaStreamWaitEvent");
@@ -333,5 +467,6 @@ extern "C" int bf_run_streaming(bf_ctx *c, const void *const *host_blocks, int n
   }
   cudaStreamWaitEvent(xs, c->ev_done[0], 0);
   if (nblocks > 1) cudaStreamWaitEvent(xs, c->ev_done[1], 0);
+  end_run(c, cs);
   return BF_OK;
 }

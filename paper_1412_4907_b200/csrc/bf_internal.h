@@ -31,12 +31,17 @@ __host__ __device__ inline int bf_tile_off(int r, int k) { return r * BF_KBLOCK 
 // row of (beam-in-tile bl, part)
 __host__ __device__ inline int bf_beam_row(int bl, int part) { return ((bl >> 4) << 5) + (part << 4) + (bl & 15); }
 
+enum { BF_MODE_POWER = 0, BF_MODE_BEAMS = 1 };
+
 struct BfParams {
   int nant, nbeam, nsamp, nint, nbin;
   int nMt, nKb;
   int nchan_run;        // channels processed by this launch
   const void *volt;     // device, first channel of this launch
   float *pow;           // device, first channel of this launch
+  void *beams;          // voltage-beam mode (bf_run_beams): fp16 (re, im) [chan][beam][nsamp], first channel of this launch
+  float beam_scale;     // voltage-beam mode: y is multiplied by this before rounding to fp16
+  int mode;             // BF_MODE_POWER (|y|^2 integrated over nint -> pow) or BF_MODE_BEAMS (y -> beams)
   const __half *wop;    // device, weight operand of the first channel of this launch
 };
 
@@ -52,6 +57,13 @@ struct bf_ctx {
   std::vector<double> h_gain;
   __half *d_wop;
   bool have_geom;
+  // tracking beams (row f3): up to two (geometry, weight operand) buffers; runs read `active`, an update
+  // writes the other one on its own stream and the next run switches over behind an event
+  int nwbuf, active, pending;      // pending: -1 none, else the buffer the next run switches to
+  char *geom_buf[2];
+  __half *wop_buf[2];
+  cudaEvent_t ev_upd, ev_use[2];
+  bool have_wevents, used[2];
   std::vector<double> h_geom;
   long long launches;
   int sm_count;     // 0 = device not probed yet
@@ -69,5 +81,7 @@ cudaError_t bf_launch_weights(const bf_ctx *c, cudaStream_t st);
 cudaError_t bf_launch_decode_weights(const bf_ctx *c, float *d_out, cudaStream_t st);
 cudaError_t bf_launch_simt(const BfParams &p, int dtype, cudaStream_t st);
 bool bf_umma_supported(const bf_ctx *c, const char **why);
+bool bf_umma_shape_supported(const bf_ctx *c, const char **why);  // ignoring nint (voltage-beam mode)
+cudaError_t bf_launch_incoherent(const bf_ctx *c, const void *volt, float *out, cudaStream_t st);
 cudaError_t bf_launch_umma(const BfParams &p, int dtype, int sm_count, cudaStream_t st);
 cudaError_t bf_launch_umma_kblock(const BfParams &p, int dtype, int sm_count, cudaStream_t st);

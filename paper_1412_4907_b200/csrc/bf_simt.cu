@@ -28,7 +28,7 @@ __device__ __forceinline__ float2 load_volt(const void *volt, size_t idx) {
   }
 }
 
-template <int DTYPE>
+template <int DTYPE, bool BEAMS>
 __global__ void __launch_bounds__(SIMT_BEAMS) bf_simt_kernel(BfParams p, int samples_per_block) {
   __shared__ float2 Ws[SIMT_NC][SIMT_BEAMS + 1];
   __shared__ float2 Xs[SIMT_TT][SIMT_NC];
@@ -84,7 +84,11 @@ __global__ void __launch_bounds__(SIMT_BEAMS) bf_simt_kernel(BfParams p, int sam
 #pragma unroll
     for (int t = 0; t < SIMT_TT; ++t) {
       int tt = t0 + t;
-      if (tt < t_end) {
+      if (BEAMS) {  // voltage-beam mode (row f4): y itself as fp16 (re, im)
+        if (tt < t_end && b < p.nbeam)
+          reinterpret_cast<__half2 *>(p.beams)[((size_t)c * p.nbeam + b) * p.nsamp + tt] =
+              __floats2half2_rn(acc[t].x * p.beam_scale, acc[t].y * p.beam_scale);
+      } else if (tt < t_end) {
         binacc = fmaf(acc[t].x, acc[t].x, binacc);
         binacc = fmaf(acc[t].y, acc[t].y, binacc);
         if ((tt + 1) % p.nint == 0) {
@@ -103,8 +107,12 @@ cudaError_t bf_launch_simt(const BfParams &p, int dtype, cudaStream_t st) {
   dim3 grid((p.nsamp + samples_per_block - 1) / samples_per_block, (p.nbeam + SIMT_BEAMS - 1) / SIMT_BEAMS,
             p.nchan_run);
   if (grid.z > 65535 || grid.y > 65535) return cudaErrorInvalidConfiguration;
-  if (dtype == BF_CI8)      bf_simt_kernel<BF_CI8><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
-  else if (dtype == BF_CI4) bf_simt_kernel<BF_CI4><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
-  else                      bf_simt_kernel<BF_CF16><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
+  if (p.mode == BF_MODE_BEAMS) {
+    if (dtype == BF_CI8)      bf_simt_kernel<BF_CI8, true><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
+    else if (dtype == BF_CI4) bf_simt_kernel<BF_CI4, true><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
+    else                      bf_simt_kernel<BF_CF16, true><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
+  } else if (dtype == BF_CI8) bf_simt_kernel<BF_CI8, false><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
+  else if (dtype == BF_CI4)   bf_simt_kernel<BF_CI4, false><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
+  else                        bf_simt_kernel<BF_CF16, false><<<grid, SIMT_BEAMS, 0, st>>>(p, samples_per_block);
   return cudaGetLastError();
 }

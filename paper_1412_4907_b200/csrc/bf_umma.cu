@@ -57,7 +57,7 @@ __device__ __forceinline__ void next_item(Item &it, int nG, int nTt) {
 // read by warps w with w % 4 == quadrant -- which all sit on SM sub-partition `quadrant`.  For <= 16
 // beams the whole epilogue therefore lands on sub-partition 0; SPREAD launches 32 warps and puts the
 // convert / MMA / TMA warps on sub-partitions 1-3 only, so that sub-partition 0 does nothing else.
-template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD, int IN>
+template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD, int IN, bool BEAMS>
 __global__ void __launch_bounds__(SPREAD ? 1024 : (EPI_WARPS + CONV_WARPS + 3) * 32, 1)
 bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, const int nTt, const int nks) {
   extern __shared__ uint8_t smem_raw[];
@@ -136,6 +136,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     const size_t mstride = (size_t)BF_TILE_BEAMS * nbin;     // output distance between M-tiles
     const bool vec_ok = (nbin % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.pow) & 15) == 0);
     const bool ragged = (p.nsamp % TILE_T) != 0;             // the last time tile of a channel is partial
+    const bool bvec_ok = BEAMS && (p.nsamp % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.beams) & 15) == 0);
     Item it = decode_item(it0, nG, nTt);
     uint32_t par0 = 0, par1 = 0;                             // parity of the next completion of t_full[0/1]
     int i = 0;
@@ -152,11 +153,19 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         if (m < gm && lane < 16 && beam < nbeam) wr |= 1u << m;
       }
       float *ptr = p.pow + ((size_t)it.c * nbeam + beam0) * nbin + (NINT_T == 0 ? 0 : it.tt * BPT + slot * BPW);
+      // voltage-beam mode (row f4): this lane's beam at the first column of this warp in tile it.tt
+      __half2 *bptr = reinterpret_cast<__half2 *>(p.beams) + ((size_t)it.c * nbeam + beam0) * p.nsamp + it.tt * TILE_T + slot * 64;
+      uint32_t bok = 0;                                      // bit m: this lane's beam of M-tile m exists
+#pragma unroll
+      for (int m = 0; m < GROUP; ++m)
+        if (m < gm && beam0 + m * BF_TILE_BEAMS < nbeam) bok |= 1u << m;
       int tt = it.tt;
-      for (int k = 0; k < run; ++k, ++i, ++tt, ptr += BPT) {
+      for (int k = 0; k < run; ++k, ++i, ++tt, ptr += BPT, bptr += TILE_T) {
         int nvalid = 1 << 30;
         float *out = ptr;
-        if (NINT_T == 0) {
+        if (BEAMS) {
+          nvalid = p.nsamp - (tt * TILE_T + slot * 64);
+        } else if (NINT_T == 0) {
           const int t_first = tt * TILE_T + slot * 64;       // first time sample of this warp's columns
           out = ptr + t_first / p.nint;
           nvalid = t_first < p.nsamp ? 1 : 0;
@@ -173,8 +182,12 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
             epilogue_skip(b_full + 16 + 8 * ACC, lane0);
             return;
           }
-          epilogue_tile<NINT_T>(t_lane + ACC * TILE_T, out + m * mstride, (wr >> m) & 1, nvalid, NINT_T != 0 && vec_ok,
-                                b_full + 16 + 8 * ACC, lane0);
+          if constexpr (BEAMS)
+            epilogue_beams_tile(t_lane + ACC * TILE_T, bptr + (size_t)m * BF_TILE_BEAMS * p.nsamp, (bok >> m) & 1, nvalid,
+                                bvec_ok, p.beam_scale, lane >= 16, b_full + 16 + 8 * ACC, lane0);
+          else
+            epilogue_tile<NINT_T>(t_lane + ACC * TILE_T, out + m * mstride, (wr >> m) & 1, nvalid, NINT_T != 0 && vec_ok,
+                                  b_full + 16 + 8 * ACC, lane0);
         };
         if constexpr (GROUP == 1) {
           if (i & 1) one(std::integral_constant<int, 1>{}, 0);
@@ -364,17 +377,17 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   if (mw == 0) tmem_dealloc(tmem_base, 512);
 }
 
-template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD, int IN>
+template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD, int IN, bool BEAMS = false>
 cudaError_t launch_k64(const BfParams &p, int sm_count, cudaStream_t st) {
   const int nG = (p.nMt + GROUP - 1) / GROUP;
   const int nTt = (p.nsamp + TILE_T - 1) / TILE_T;
   const long long total = (long long)p.nchan_run * nG * nTt;
   const int nks = (2 * p.nant + 15) / 16;
   const size_t smem = 1024 + 2 * GROUP * A_TILE_BYTES + NSTAGE * B_STAGE_BYTES + NRAW * RAW_STAGE_BYTES + 256;
-  auto kern = bf_umma_k64_kernel<NINT_T, GROUP, NSTAGE, NRAW, CONV_WARPS, SPREAD, IN>;
+  auto kern = bf_umma_k64_kernel<NINT_T, GROUP, NSTAGE, NRAW, CONV_WARPS, SPREAD, IN, BEAMS>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  if (NINT_T == 0) {
+  if (NINT_T == 0 && !BEAMS) {
     e = cudaMemsetAsync(p.pow, 0, (size_t)p.nchan_run * p.nbeam * p.nbin * sizeof(float), st);
     if (e != cudaSuccess) return e;
   }
@@ -406,14 +419,28 @@ static int umma_variant(int dtype, int nant) {
   return 0;
 }
 
-bool bf_umma_supported(const bf_ctx *c, const char **why) {
+bool bf_umma_shape_supported(const bf_ctx *c, const char **why) {
   if (!umma_variant(c->dtype, c->nant)) { *why = "needs nant % 8 == 0 (int8), % 4 == 0 (fp16), or 16 / 32 (4-bit)"; return false; }
+  return true;
+}
+
+bool bf_umma_supported(const bf_ctx *c, const char **why) {
+  if (!bf_umma_shape_supported(c, why)) return false;
   if (!nint_ok(c->nint)) { *why = "needs nint a power of two <= 64 or a multiple of 64"; return false; }
   return true;
 }
 
+// voltage-beam mode: the output (4 bytes per beam-sample) dominates the traffic; nint plays no role
+template <int IN>
+static cudaError_t launch_k64_beams(const BfParams &p, int sm_count, cudaStream_t st) {
+  if (p.nMt == 1) return launch_k64<64, 1, 2, 8, 8, false, IN, true>(p, sm_count, st);
+  if (p.nMt <= 2) return launch_k64<64, 2, 3, 4, 8, false, IN, true>(p, sm_count, st);
+  return launch_k64<64, 4, 2, 2, 8, false, IN, true>(p, sm_count, st);
+}
+
 template <int IN>
 static cudaError_t launch_k64_in(const BfParams &p, int sm_count, cudaStream_t st) {
+  if (p.mode == BF_MODE_BEAMS) return launch_k64_beams<IN>(p, sm_count, st);
   switch (p.nint) {
     case 1: return launch_k64_nint<1, IN>(p, sm_count, st);
     case 2: return launch_k64_nint<2, IN>(p, sm_count, st);

@@ -166,6 +166,57 @@ __device__ __forceinline__ void epilogue_tile(uint32_t taddr, float *out, bool w
     }
   }
 }
+// Voltage-beam epilogue ("electric-field ... beams ... output as 16-bit complex-valued
+// words"): ONE accumulator tile for ONE warp -> y[beam][t] as fp16 (re, im) pairs, scaled by
+// `scale`.  Lane l < 16 holds the re row, lane l + 16 the im row of one beam; 64 columns = 64 time samples.
+// Per 32-column chunk: pack time pairs to half2, swap halves between the two lanes of a beam (the re lane
+// keeps samples 0..15 and receives their im parts, the im lane keeps 16..31 and receives their re parts),
+// interleave with two PRMT per pair, and store 64 contiguous bytes per lane.  `out` = this lane's beam at the
+// warp's first column, `nvalid` = samples that exist from there (tail tiles), `vec_ok` = 16-byte stores allowed.
+__device__ __forceinline__ void epilogue_beams_tile(uint32_t taddr, __half2 *out, bool beam_ok, int nvalid, bool vec_ok,
+                                                    float scale, bool upper, uint32_t bar_empty, bool lane0) {
+  constexpr int CPW = TILE_T / (EPI_WARPS / 4);
+  constexpr int NCH = CPW / 32;
+#pragma unroll
+  for (int ch = 0; ch < NCH; ++ch) {
+    uint32_t v[32];
+    BF_TMEM_LD_32x32b_X32(taddr + 32 * ch, v);
+    tc_wait_ld();
+    if (ch == NCH - 1) {
+      tc_fence_before();
+      __syncwarp();
+      if (lane0) mbar_arrive(bar_empty);
+    }
+    uint32_t h[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+      const __half2 q = __floats2half2_rn(__uint_as_float(v[2 * j]) * scale, __uint_as_float(v[2 * j + 1]) * scale);
+      h[j] = *reinterpret_cast<const uint32_t *>(&q);
+    }
+    uint32_t o[16];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const uint32_t send = upper ? h[i] : h[8 + i];
+      const uint32_t mine = upper ? h[8 + i] : h[i];
+      const uint32_t recv = __shfl_xor_sync(0xffffffffu, send, 16);
+      const uint32_t re = upper ? recv : mine, im = upper ? mine : recv;
+      o[2 * i] = __byte_perm(re, im, 0x5410);      // (re, im) of the even sample
+      o[2 * i + 1] = __byte_perm(re, im, 0x7632);  // (re, im) of the odd sample
+    }
+    const int t0 = 32 * ch + (upper ? 16 : 0);     // first of this lane's 16 samples
+    if (!beam_ok) continue;
+    uint32_t *dst = reinterpret_cast<uint32_t *>(out + t0);
+    if (vec_ok && t0 + 16 <= nvalid) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        *reinterpret_cast<uint4 *>(dst + 4 * k) = make_uint4(o[4 * k], o[4 * k + 1], o[4 * k + 2], o[4 * k + 3]);
+    } else {
+#pragma unroll
+      for (int k = 0; k < 16; ++k)
+        if (t0 + k < nvalid) dst[k] = o[k];
+    }
+  }
+}
 // a lane quadrant that holds only padding rows just hands the stage back
 __device__ __forceinline__ void epilogue_skip(uint32_t bar_empty, bool lane0) {
   __syncwarp();

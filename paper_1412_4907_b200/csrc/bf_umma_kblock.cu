@@ -43,7 +43,7 @@ __device__ __forceinline__ KItem kdecode(long long idx, int nG, int nTt) {
   return it;
 }
 
-template <int NINT_T, bool IS_F16, int NA, int NB, int NR>
+template <int NINT_T, bool IS_F16, int NA, int NB, int NR, bool BEAMS>
 __global__ void __launch_bounds__(NTHREADS, 1)
 bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, const long long total_items,
                       const int nG, const int nTt) {
@@ -89,6 +89,7 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
     const uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16) + slot * 64;
     const int bl = quad * 16 + (lane & 15);
     const bool vec_ok = (p.nbin % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.pow) & 15) == 0);
+    const bool bvec_ok = BEAMS && (p.nsamp % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.beams) & 15) == 0);
     uint32_t tpar = 0;  // bit m: parity of the next completion of t_full[m] (an odd last group skips m = 1)
     for (int i = 0; i < n_items; ++i) {
       const KItem it = kdecode(it0 + i * it_step, nG, nTt);
@@ -101,6 +102,12 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
         const int beam = (it.g * KB_GROUP + m) * BF_TILE_BEAMS + bl;
         if (beam - (lane & 15) >= p.nbeam) { epilogue_skip(bar_t_empty + 8 * m, lane0); continue; }
         const bool writer = (lane < 16) && (beam < p.nbeam);
+        if constexpr (BEAMS) {  // voltage-beam mode (row f4): y itself, fp16 (re, im)
+          __half2 *yrow = reinterpret_cast<__half2 *>(p.beams) + ((size_t)it.c * p.nbeam + beam) * p.nsamp + t_first;
+          epilogue_beams_tile(t_lane + m * TILE_T, yrow, beam < p.nbeam, p.nsamp - t_first, bvec_ok, p.beam_scale,
+                              lane >= 16, bar_t_empty + 8 * m, lane0);
+          continue;
+        }
         float *row = p.pow + ((size_t)it.c * p.nbeam + beam) * p.nbin;
         if (NINT_T == 0) {
           epilogue_tile<NINT_T>(t_lane + m * TILE_T, row + t_first / p.nint, writer, t_first < p.nsamp ? 1 : 0, false,
@@ -245,7 +252,7 @@ cudaError_t make_tmap(CUtensorMap *tm, const BfParams &p, int dtype) {
   return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-template <int NINT_T, bool IS_F16>
+template <int NINT_T, bool IS_F16, bool BEAMS = false>
 cudaError_t launch_kb(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
   constexpr int NA = 3, NB = IS_F16 ? 3 : 2, NR = IS_F16 ? 0 : 3;
   CUtensorMap tm;
@@ -255,10 +262,10 @@ cudaError_t launch_kb(const BfParams &p, int dtype, int sm_count, cudaStream_t s
   const int nTt = (p.nsamp + TILE_T - 1) / TILE_T;
   const long long total = (long long)p.nchan_run * nTt * nG;
   const size_t smem = 1024 + NA * A_STAGE_BYTES + NB * B_STAGE_BYTES + NR * RAW_STAGE_BYTES + 512;
-  auto kern = bf_umma_kblock_kernel<NINT_T, IS_F16, NA, NB, NR>;
+  auto kern = bf_umma_kblock_kernel<NINT_T, IS_F16, NA, NB, NR, BEAMS>;
   e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  if (NINT_T == 0) {
+  if (NINT_T == 0 && !BEAMS) {
     e = cudaMemsetAsync(p.pow, 0, (size_t)p.nchan_run * p.nbeam * p.nbin * sizeof(float), st);
     if (e != cudaSuccess) return e;
   }
@@ -269,6 +276,7 @@ cudaError_t launch_kb(const BfParams &p, int dtype, int sm_count, cudaStream_t s
 
 template <bool IS_F16>
 cudaError_t launch_kb_nint(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
+  if (p.mode == BF_MODE_BEAMS) return launch_kb<64, IS_F16, true>(p, dtype, sm_count, st);
   switch (p.nint) {
     case 1: return launch_kb<1, IS_F16>(p, dtype, sm_count, st);
     case 2: return launch_kb<2, IS_F16>(p, dtype, sm_count, st);

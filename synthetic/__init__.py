@@ -246,6 +246,17 @@ SWEEP_BEAMS = (1, 4, 16, 64, 256, 1024)
 
 
 # ----------------------------------------------------------------------------- device-side fill
+def make_case(nant: int, nchan: int, nbeam: int, nsamp: int, nint: int, dtype: str, seed: int = 0) -> Workload:
+    """A small seeded test case of arbitrary shape: scattered near-planar array, random beam directions within
+    ~35 deg of zenith, noise plus one source at the centre of beam nbeam // 2 (the recipe of the parity tests)."""
+    rng = np.random.default_rng([seed, nant, nchan, nbeam, nsamp])
+    r = rng.uniform(-40, 40, size=(nant, 3)); r[:, 2] *= 0.05
+    f = np.linspace(380e6, 420e6, nchan) if nchan > 1 else np.array([408e6])
+    s = rng.normal(size=(nbeam, 3)); s[:, 2] = np.abs(s[:, 2]) + 1.5; s /= np.linalg.norm(s, axis=1, keepdims=True)
+    sig, amp = {"ci8": (16.0, 4.0), "cf16": (1.0, 0.5), "ci4": (2.0, 1.0)}[dtype]
+    return Workload("case", nant, nchan, nbeam, nsamp, nint, dtype, seed, r, f, s, sig, [(s[nbeam // 2].copy(), amp)])
+
+
 def fill_voltages_torch(w: Workload, device, chunk_chan: int = 16):
     """Full-size voltages generated ON `device` with torch's seeded generator (reading A11):
     same statistics as make_voltages(); bytes are what they are -- parity checks copy the very

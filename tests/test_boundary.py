@@ -96,3 +96,23 @@ def test_kernel_selection_is_static_function_of_shape(bf):
     bf.bf_set_kernel(ctx, bf.BF_KERNEL_UMMA)
     assert bf.bf_selected_kernel(ctx) == bf.BF_KERNEL_UMMA  # forced; bf_run would report BF_EUNSUPPORTED
     bf.bf_destroy(ctx)
+
+
+def test_mode_entry_points_validate_without_gpu(bf):
+    """Rows f3/f4: voltage beams, incoherent beam, double-buffered weights -- argument checks only."""
+    ctx = bf.bf_create(32, 4, 16, 256, 16)
+    one = bf.bf_workspace_bytes(ctx)
+    assert bf.bf_set_weight_buffers(ctx, 3) == bf.BF_EINVAL
+    assert bf.bf_set_weight_buffers(ctx, 2) == bf.BF_OK
+    assert bf.bf_workspace_bytes(ctx) == 2 * one          # a second (geometry, weight operand) buffer
+    assert bf.bf_set_weight_buffers(ctx, 1) == bf.BF_OK
+    r = np.zeros((32, 3)); f = np.full(4, 408e6); s = np.tile([0.0, 0.0, 1.0], (16, 1))
+    assert bf.bf_update_geometry(ctx, r, f, s) == bf.BF_EINVAL     # needs two buffers
+    assert "bf_set_weight_buffers" in bf.bf_last_error(ctx)
+    assert bf.bf_run_beams(ctx, 0x10000, 0x20000, 1.0) == bf.BF_ENOGEOM
+    assert bf.bf_run_beams(ctx, None, 0x20000, 1.0) == bf.BF_EINVAL
+    assert bf.bf_run_incoherent(ctx, None, 0x20000) == bf.BF_EINVAL
+    assert bf.bf_run_incoherent(ctx, 0x10000, None) == bf.BF_EINVAL
+    assert bf.bf_set_workspace(ctx, 0x10000, 1 << 30) == bf.BF_OK
+    assert bf.bf_set_weight_buffers(ctx, 2) == bf.BF_EINVAL        # too late: the workspace is laid out
+    bf.bf_destroy(ctx)

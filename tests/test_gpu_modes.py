@@ -1,0 +1,176 @@
+"""GPU parity of the "next" rows: voltage beams and the incoherent beam (f4) and
+double-buffered weight updates for tracking beams (f3), each through the C ABI against the oracle.
+
+Tolerances:
+* voltage beams: per (channel, beam) row  max_t |y_gpu/scale - y_ref| <= 4e-3 * rms_t |y_ref|.
+  Two error sources, both per sample: the fp16 weight operand (rms 2e-4 of |y|, worst sample of a few
+  thousand ~8e-4) and ONE rounding of each output component to fp16 (2^-11 = 4.9e-4 of that component,
+  components reach ~4 rms).  The sum stays below 3e-3 rms; 4e-3 is the bar.
+* incoherent beam: integer inputs are summed exactly and rounded once to fp32 (rel 2^-24 = 6e-8): bar 2e-7;
+  fp16 inputs are summed in fp32 (rel ~ sqrt(n) 2^-24): bar 1e-5.
+* tracking: the power bar of test_gpu_parity.py (1e-3 per row), for every block with ITS geometry.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import synthetic
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def bf():
+    import paper_1412_4907_b200 as bf
+    bf.lib()
+    return bf
+
+
+def bf_dtype(bf, w):
+    return {"ci8": bf.BF_CI8, "cf16": bf.BF_CF16, "ci4": bf.BF_CI4}[w.dtype]
+
+
+# ------------------------------------------------------------------ f4: voltage beams
+BEAM_CASES = [
+    # nant nchan nbeam nsamp dtype
+    (32, 2, 16, 512, "ci8"),
+    (32, 2, 3, 1000, "ci8"),     # ragged time tail, padding rows in the quadrant
+    (32, 1, 65, 260, "ci8"),     # second M tile, tail tile of 4 samples
+    (32, 1, 130, 256, "ci8"),    # three M tiles (beam groups of 4)
+    (32, 2, 8, 250, "ci8"),      # nsamp % 4 != 0: scalar stores
+    (16, 2, 9, 300, "ci8"),
+    (64, 2, 33, 512, "ci8"),     # K-blocked kernel, int8
+    (64, 2, 16, 256, "cf16"),    # K-blocked kernel, fp16
+    (5, 2, 3, 77, "ci8"),        # generic kernel only
+    (32, 2, 16, 256, "ci4"),
+]
+
+
+@pytest.mark.parametrize("nant,nchan,nbeam,nsamp,dtype", BEAM_CASES)
+@pytest.mark.parametrize("kernel", ["simt", "auto"])
+def test_voltage_beams_match_oracle(bf, nant, nchan, nbeam, nsamp, dtype, kernel):
+    import torch
+    w = synthetic.make_case(nant, nchan, nbeam, nsamp, 1, dtype)
+    v = w.make_voltages()
+    ref = oracle.beams(w.ant_xyz, w.freqs, w.beam_dir, v)  # [C][B][T] complex128
+    scale = 0.25 if dtype != "cf16" else 2.0
+    B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, 1, dtype=bf_dtype(bf, w),
+                      kernel=bf.BF_KERNEL_SIMT if kernel == "simt" else bf.BF_KERNEL_AUTO)
+    B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
+    y = torch.full((w.nchan, w.nbeam, w.nsamp, 2), float("nan"), dtype=torch.float16, device="cuda")
+    B.run_beams(torch.from_numpy(v).cuda(), y, scale=scale)
+    torch.cuda.synchronize()
+    out = y.cpu().numpy().astype(np.float64)
+    B.close()
+    assert np.isfinite(out).all()
+    yg = (out[..., 0] + 1j * out[..., 1]) / scale
+    err = np.abs(yg - ref).max(axis=-1)
+    rms = np.sqrt((np.abs(ref) ** 2).mean(axis=-1))
+    worst = (err / rms).max()
+    assert worst <= 4e-3, f"worst row error {worst:.3e}"
+
+
+def test_voltage_beams_square_to_the_powers(bf):
+    """|y|^2 summed over nint (from the fp16 beams) agrees with bf_run's fused powers on the same input."""
+    import torch
+    w = synthetic.make_workload("tiny").sub(nchan=4)
+    v = torch.from_numpy(w.make_voltages()).cuda()
+    B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint)
+    B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
+    P = B.run(v).cpu().numpy().astype(np.float64)
+    y = B.run_beams(v, scale=0.5).cpu().numpy().astype(np.float64) / 0.5
+    B.close()
+    P2 = (y ** 2).sum(-1).reshape(w.nchan, w.nbeam, -1, w.nint).sum(-1)
+    assert (np.abs(P2 - P).max(axis=-1) / P.mean(axis=-1)).max() < 2e-3
+
+
+# ------------------------------------------------------------------ f4: incoherent beam
+INC_CASES = [
+    # nant nchan nsamp nint dtype
+    (32, 3, 1024, 16, "ci8"),
+    (32, 2, 4096, 64, "ci8"),
+    (8, 2, 128, 1, "ci8"),        # one sample per bin, 16-byte bins
+    (5, 2, 77, 7, "ci8"),         # unaligned bins
+    (256, 2, 512, 64, "ci8"),     # 32 KiB bins: one block per bin
+    (32, 2, 256, 16, "ci4"),
+    (3, 2, 50, 5, "ci4"),
+    (16, 2, 256, 32, "cf16"),
+    (256, 1, 256, 128, "cf16"),
+]
+
+
+@pytest.mark.parametrize("nant,nchan,nsamp,nint,dtype", INC_CASES)
+def test_incoherent_beam_matches_oracle(bf, nant, nchan, nsamp, nint, dtype):
+    import torch
+    w = synthetic.make_case(nant, nchan, 1, nsamp, nint, dtype)
+    v = w.make_voltages()
+    ref = oracle.incoherent(v, nint)
+    B = bf.Beamformer(nant, nchan, 1, nsamp, nint, dtype=bf_dtype(bf, w))
+    P = torch.full((nchan, nsamp // nint), float("nan"), dtype=torch.float32, device="cuda")
+    B.run_incoherent(torch.from_numpy(v).cuda(), P)   # no geometry needed
+    torch.cuda.synchronize()
+    out = P.cpu().numpy().astype(np.float64)
+    B.close()
+    tol = 1e-5 if dtype == "cf16" else 2e-7
+    assert np.isfinite(out).all()
+    assert (np.abs(out - ref) / ref).max() <= tol
+
+
+def test_incoherent_full_size_sampled(bf):
+    """medium-sized buffer in the launch configuration bench.py --mode incoherent times; sampled bins vs the oracle."""
+    import torch
+    w = synthetic.make_workload("medium").sub(nchan=64)
+    v = synthetic.fill_voltages_torch(w, torch.device("cuda"))
+    B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint)
+    P = B.run_incoherent(v).cpu().numpy().astype(np.float64)
+    B.close()
+    for c in (0, 31, 63):
+        ref = oracle.incoherent(v[c:c + 1].cpu().numpy(), w.nint)[0]
+        assert (np.abs(P[c] - ref) / ref).max() <= 2e-7
+
+
+# ------------------------------------------------------------------ f3: tracking beams (double-buffered weights)
+def test_tracking_updates_switch_weights_between_runs(bf):
+    import torch
+    w = synthetic.make_workload("tiny").sub(nchan=8)
+    v = w.make_voltages()
+    vd = torch.from_numpy(v).cuda()
+    # three pointings: the beam fan drifts by a fraction of a beam width per block
+    dirs = []
+    for k in range(3):
+        th = np.deg2rad(np.linspace(-30, 30, w.nbeam) + 0.7 * k)
+        dirs.append(np.stack([np.sin(th), np.zeros_like(th), np.cos(th)], axis=1))
+    refs = [oracle.beamform(w.ant_xyz, w.freqs, d, v, w.nint) for d in dirs]
+    B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint, weight_buffers=2)
+    run_s, upd_s = torch.cuda.Stream(), torch.cuda.Stream()
+    B.set_geometry(w.ant_xyz, w.freqs, dirs[0], stream=run_s)
+    outs = []
+    # no host synchronisation anywhere in the loop: ordering is the library's job
+    for rep in range(4):
+        for k in range(3):
+            P = B.run(vd, stream=run_s)
+            outs.append((k, P))
+            B.update_geometry(w.ant_xyz, w.freqs, dirs[(k + 1) % 3], update_stream=upd_s)
+    torch.cuda.synchronize()
+    for k, P in outs:
+        out = P.cpu().numpy().astype(np.float64)
+        worst = (np.abs(out - refs[k]).max(axis=-1) / refs[k].mean(axis=-1)).max()
+        assert worst <= 1e-3, (k, worst)
+    # the pointings really differ (the test would pass trivially otherwise)
+    assert (np.abs(refs[1] - refs[0]).max(axis=-1) / refs[0].mean(axis=-1)).max() > 0.05
+    # weights reported after an update are the new ones
+    B.update_geometry(w.ant_xyz, w.freqs, dirs[2], update_stream=upd_s)
+    Wg = B.weights()
+    Wo = oracle.weights(w.ant_xyz, w.freqs, dirs[2])
+    assert np.abs(Wg - Wo).max() < 2.0 ** -10
+    B.close()
+
+
+def test_update_geometry_needs_two_buffers(bf):
+    w = synthetic.make_workload("tiny").sub(nchan=2)
+    B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint)
+    B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
+    with pytest.raises(bf.BfError) as e:
+        B.update_geometry(w.ant_xyz, w.freqs, w.beam_dir)
+    assert e.value.code == bf.BF_EINVAL
+    B.close()
