@@ -195,6 +195,9 @@ def main():
     ap.add_argument("--config", default="medium")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "simt", "umma"])
+    ap.add_argument("--mode", default="power", choices=["power", "beams", "incoherent"],
+                    help="power = the headline path (bf_run); beams / incoherent = SURVEY 8(f) row f4 side modes")
+    ap.add_argument("--nbeam", type=int, default=0, help="override the workload's beam count (beams mode: default 8)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--chan-per-chunk", type=int, default=0, help="e2e: channels per H2D chunk (0 = nchan/8)")
@@ -223,6 +226,12 @@ def main():
     W = max(3, args.warmup)
     K = max(1, args.steps)
     w = workload_for(args.config)
+    if args.mode == "beams" or args.nbeam:
+        # the S-engine ships "8 beams from the generated 128-beam grid ... as 16-bit complex-valued words"
+        w = w.sub(nbeam=args.nbeam or 8)
+    if args.mode != "power":
+        args.no_e2e = True
+        args.no_cpu_baseline = True
     w.seed = rank_seed(w.seed, rank)
     peaks = load_peaks()
     kern = {"auto": bf.BF_KERNEL_AUTO, "simt": bf.BF_KERNEL_SIMT, "umma": bf.BF_KERNEL_UMMA}[args.kernel]
@@ -233,6 +242,13 @@ def main():
     v = synthetic.fill_voltages_torch(w, dev)
     P = B.empty_powers()
     stream = torch.cuda.current_stream(dev)
+    run_step = lambda: B.run(v, P, stream)
+    if args.mode == "beams":
+        Y = torch.empty((w.nchan, w.nbeam, w.nsamp, 2), dtype=torch.float16, device=dev)
+        run_step = lambda: B.run_beams(v, Y, 0.25, stream)
+    elif args.mode == "incoherent":
+        Pi = torch.empty((w.nchan, w.nbin), dtype=torch.float32, device=dev)
+        run_step = lambda: B.run_incoherent(v, Pi, stream)
 
     def barrier():
         if dist:
@@ -241,7 +257,7 @@ def main():
 
     # ---------------------------------------------------------------- device-resident timing
     for _ in range(W):
-        B.run(v, P, stream)
+        run_step()
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
@@ -251,14 +267,14 @@ def main():
     barrier()
     ev[0].record(stream)
     for k in range(K):
-        B.run(v, P, stream)
+        run_step()
         ev[k + 1].record(stream)
     barrier()
     launches = B.launches - l0
     clocks = sampler.stop() if rank == 0 else None
     total_ms = ev[0].elapsed_time(ev[K])
     per_launch_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(K)]
-    flop_step = 8.0 * w.cmac
+    flop_step = 8.0 * w.cmac if args.mode != "incoherent" else 4.0 * w.nchan * w.nsamp * w.nant  # |x|^2 + add
     total_ms_max, flop_all = aggregate(total_ms, flop_step * K, td if dist else None, dev)
     value = flop_all / (total_ms_max * 1e-3) / 1e12
     ms_per_step = total_ms_max / K
@@ -267,11 +283,15 @@ def main():
     # roofline of the dominant (only) kernel: a dense contraction -> tensor bound; HBM-bound when
     # the algorithmic bytes at measured bandwidth take longer than the flops at measured tensor peak
     abytes = algorithmic_bytes(w)
+    if args.mode == "beams":
+        abytes = w.in_bytes + w.nchan * w.nbeam * w.nant * 4 + w.nchan * w.nbeam * w.nsamp * 4  # fp16 complex out
+    elif args.mode == "incoherent":
+        abytes = w.in_bytes + w.nchan * w.nbin * 4
     t_hbm = abytes / (peaks["hbm_gbs"] * 1e9)
     t_tensor = flop_step / (peaks["tensor_tflops"] * 1e12)
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
+    if os.path.exists(tpath) and args.mode == "power":
         try:
             traffic = json.load(open(tpath)).get(w.name)
         except Exception:
@@ -347,11 +367,11 @@ def main():
 
     if rank == 0:
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "metric": METRIC if args.mode == "power" else METRIC + " [side mode: %s]" % args.mode, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f16xf16->f32" if B.selected_kernel == bf.BF_KERNEL_UMMA else "f32",
+            "dtype": "i8->i32 (dp4a)" if args.mode == "incoherent" else ("f16xf16->f32" if B.selected_kernel == bf.BF_KERNEL_UMMA else "f32"),
             "data": "synthetic",
-            "config": {"workload": w.name, "nant": w.nant, "nchan": w.nchan, "nbeam": w.nbeam, "nsamp": w.nsamp,
+            "config": {"workload": w.name if args.mode == "power" else w.name + ":" + args.mode, "nant": w.nant, "nchan": w.nchan, "nbeam": w.nbeam, "nsamp": w.nsamp,
                        "nint": w.nint, "input": w.dtype, "l2": "input buffer (%.0f MB) >> L2 (126 MB), no flush needed" % (w.in_bytes / 1e6),
                        "kernel": {1: "simt", 2: "umma"}[B.selected_kernel], "parallelism": f"replicas x{world}"},
             "ant_samples_per_s": world * w.nchan * w.nsamp * w.nant * K / (total_ms_max * 1e-3),
