@@ -57,7 +57,10 @@ enum bf_dtype {
 enum bf_kernel {
   BF_KERNEL_AUTO = 0, /* pick the fastest kernel that supports the shape */
   BF_KERNEL_SIMT = 1, /* generic fp32 CUDA-core kernel (any shape; Algorithm 1's structure) */
-  BF_KERNEL_UMMA = 2  /* tcgen05/TMEM tensor-core kernel with the fused |.|^2 + integrate epilogue */
+  BF_KERNEL_UMMA = 2, /* tcgen05/TMEM tensor-core kernels with the fused |.|^2 + integrate epilogue (the library
+                         picks the variant) */
+  BF_KERNEL_UMMA_F16 = 3, /* only the fp16-operand variants (int8 input converted in-kernel) */
+  BF_KERNEL_UMMA_I8 = 4   /* only the int8-operand variant (kind::i8, two-limb weights; few beams, nant <= 32) */
 };
 
 /*
@@ -78,8 +81,11 @@ int bf_set_dtype(bf_ctx *ctx, int dtype);
  * if the forced kernel cannot run the context's shape. */
 int bf_set_kernel(bf_ctx *ctx, int kernel);
 
-/* Which kernel bf_run will launch for this context (enum bf_kernel value, never AUTO). */
+/* Which kernel family bf_run will launch for this context: BF_KERNEL_SIMT or BF_KERNEL_UMMA. */
 int bf_selected_kernel(const bf_ctx *ctx);
+
+/* Name of the kernel bf_run will launch: "simt", "umma-f16-resident", "umma-f16-kblock", "umma-i8". */
+const char *bf_kernel_name(const bf_ctx *ctx);
 
 /* Number of kernels this context has launched so far (all streams), for accounting. */
 long long bf_launch_count(const bf_ctx *ctx);

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libbf.so")
 
 BF_OK, BF_EINVAL, BF_ENOGEOM, BF_ECUDA, BF_EUNSUPPORTED, BF_ENOMEM = 0, -1, -2, -3, -4, -5
 BF_CI8, BF_CF16, BF_CI4 = 0, 1, 2
-BF_KERNEL_AUTO, BF_KERNEL_SIMT, BF_KERNEL_UMMA = 0, 1, 2
+BF_KERNEL_AUTO, BF_KERNEL_SIMT, BF_KERNEL_UMMA, BF_KERNEL_UMMA_F16, BF_KERNEL_UMMA_I8 = 0, 1, 2, 3, 4
 
 # every symbol include/bf.h declares: name -> (restype, argtypes)
 _vp, _i, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
@@ -29,6 +29,7 @@ SYMBOLS = {
     "bf_set_dtype": (_i, [_vp, _i]),
     "bf_set_kernel": (_i, [_vp, _i]),
     "bf_selected_kernel": (_i, [_vp]),
+    "bf_kernel_name": (ctypes.c_char_p, [_vp]),
     "bf_launch_count": (ctypes.c_longlong, [_vp]),
     "bf_workspace_bytes": (_sz, [_vp]),
     "bf_set_workspace": (_i, [_vp, _vp, _sz]),
@@ -109,6 +110,10 @@ def bf_set_kernel(ctx, kernel):
 
 def bf_selected_kernel(ctx):
     return lib().bf_selected_kernel(ctx)
+
+
+def bf_kernel_name(ctx):
+    return lib().bf_kernel_name(ctx).decode()
 
 
 def bf_launch_count(ctx):
@@ -316,6 +321,10 @@ class Beamformer:
     @property
     def selected_kernel(self):
         return bf_selected_kernel(self.ctx)
+
+    @property
+    def kernel_name(self):
+        return bf_kernel_name(self.ctx)
 
     @property
     def launches(self):

@@ -33,9 +33,16 @@ size_t bf_in_bytes_per_chan(const bf_ctx *c) {
 size_t bf_wop_bytes_per_chan(const bf_ctx *c) {
   return (size_t)c->nMt * c->nKb * BF_TILE_ROWS * BF_KBLOCK * sizeof(__half);
 }
-static size_t geom_bytes(const bf_ctx *c) {
+static size_t geom_bytes(const bf_ctx *c) {  // positions, frequencies, directions, gains, int8-operand scales
   return align_up(sizeof(double) * (3 * (size_t)c->nant + c->nchan + 3 * (size_t)c->nbeam +
-                                    2 * (size_t)c->nchan * c->nant), BF_ALIGN);
+                                    2 * (size_t)c->nchan * c->nant + c->nchan), BF_ALIGN);
+}
+// the int8 two-limb operand exists whenever the shape could take bf_umma_i8.cu (any nint)
+static bool i8_shape(const bf_ctx *c) {
+  return c->dtype == BF_CI8 && c->nant % 8 == 0 && c->nant <= 32 && c->nbeam <= BF_I8_MAX_BEAMS;
+}
+static size_t wop8_bytes(const bf_ctx *c) {
+  return i8_shape(c) ? align_up((size_t)c->nchan * bf_i8_ncol(c->nbeam) * 64, BF_ALIGN) : 0;
 }
 
 extern "C" const char *bf_version(void) { return "paper_1412_4907_b200 0.1 (sm_100a)"; }
@@ -61,6 +68,7 @@ extern "C" bf_ctx *bf_create(int nant, int nchan, int nbeam, int nsamp, int nint
   c->have_events = false;
   c->nwbuf = 1; c->active = 0; c->pending = -1;
   c->geom_buf[0] = c->geom_buf[1] = nullptr; c->wop_buf[0] = c->wop_buf[1] = nullptr;
+  c->wop8_buf[0] = c->wop8_buf[1] = nullptr; c->d_wop8 = nullptr; c->d_i8scale = nullptr;
   c->have_wevents = false; c->used[0] = c->used[1] = false;
   c->err[0] = 0;
   return c;
@@ -85,17 +93,51 @@ extern "C" int bf_set_dtype(bf_ctx *c, int dtype) {
 
 extern "C" int bf_set_kernel(bf_ctx *c, int kernel) {
   if (!c) return BF_EINVAL;
-  if (kernel != BF_KERNEL_AUTO && kernel != BF_KERNEL_SIMT && kernel != BF_KERNEL_UMMA)
+  if (kernel != BF_KERNEL_AUTO && kernel != BF_KERNEL_SIMT && kernel != BF_KERNEL_UMMA &&
+      kernel != BF_KERNEL_UMMA_F16 && kernel != BF_KERNEL_UMMA_I8)
     return fail(c, BF_EINVAL, "unknown kernel %d", kernel);
   c->kernel_forced = kernel;
   return BF_OK;
 }
 
+// the int8 kernel takes over below this many beams (measured crossover against the fp16 kernel)
+#define BF_I8_AUTO_BEAMS 16
+
+// which kernel bf_run launches: BF_KERNEL_SIMT, BF_KERNEL_UMMA_F16 or BF_KERNEL_UMMA_I8; 0 + *why if the
+// forced kernel cannot run the shape
+static int pick_kernel(const bf_ctx *c, int mode, const char **why) {
+  int k = c->kernel_forced;
+  *why = "";
+  if (k == BF_KERNEL_SIMT) return BF_KERNEL_SIMT;
+  const bool i8_ok = mode == BF_MODE_POWER && i8_shape(c) && bf_umma_i8_supported(c);
+  if (k == BF_KERNEL_UMMA_I8) {
+    if (!i8_ok) *why = "int8 kernel needs complex int8 input, nant % 8 == 0 and <= 32, <= 32 beams, nint 2^k <= 32 or % 32 == 0";
+    return i8_ok ? BF_KERNEL_UMMA_I8 : 0;
+  }
+  if (k != BF_KERNEL_UMMA_F16 && i8_ok && c->nbeam <= BF_I8_AUTO_BEAMS) return BF_KERNEL_UMMA_I8;
+  const bool f16_ok = mode == BF_MODE_BEAMS ? bf_umma_shape_supported(c, why) : bf_umma_supported(c, why);
+  if (f16_ok) return BF_KERNEL_UMMA_F16;
+  if (i8_ok && k != BF_KERNEL_UMMA_F16) return BF_KERNEL_UMMA_I8;   // e.g. nint = 96: only the int8 kernel integrates it
+  return k == BF_KERNEL_AUTO ? BF_KERNEL_SIMT : 0;
+}
+
 extern "C" int bf_selected_kernel(const bf_ctx *c) {
   if (!c) return BF_EINVAL;
-  if (c->kernel_forced != BF_KERNEL_AUTO) return c->kernel_forced;
   const char *why;
-  return bf_umma_supported(c, &why) ? BF_KERNEL_UMMA : BF_KERNEL_SIMT;
+  const int k = pick_kernel(c, BF_MODE_POWER, &why);
+  if (k == 0) return c->kernel_forced == BF_KERNEL_UMMA_I8 || c->kernel_forced == BF_KERNEL_UMMA_F16 ? BF_KERNEL_UMMA : c->kernel_forced;
+  return k == BF_KERNEL_SIMT ? BF_KERNEL_SIMT : BF_KERNEL_UMMA;
+}
+
+extern "C" const char *bf_kernel_name(const bf_ctx *c) {
+  if (!c) return "";
+  const char *why;
+  switch (pick_kernel(c, BF_MODE_POWER, &why)) {
+    case BF_KERNEL_SIMT: return "simt";
+    case BF_KERNEL_UMMA_I8: return "umma-i8";
+    case BF_KERNEL_UMMA_F16: return 2 * c->nant <= 64 && c->dtype != BF_CF16 ? "umma-f16-resident" : "umma-f16-kblock";
+    default: return "unsupported";
+  }
 }
 
 extern "C" long long bf_launch_count(const bf_ctx *c) { return c ? c->launches : 0; }
@@ -104,7 +146,7 @@ static size_t wop_bytes(const bf_ctx *c) { return align_up((size_t)c->nchan * bf
 
 extern "C" size_t bf_workspace_bytes(const bf_ctx *c) {
   if (!c) return 0;
-  return (size_t)c->nwbuf * (geom_bytes(c) + wop_bytes(c));
+  return (size_t)c->nwbuf * (geom_bytes(c) + wop_bytes(c) + wop8_bytes(c));
 }
 
 extern "C" int bf_set_weight_buffers(bf_ctx *c, int n) {
@@ -122,7 +164,9 @@ static void select_buffer(bf_ctx *c, int i) {
   c->d_freq = c->d_ant + 3 * (size_t)c->nant;
   c->d_dir = c->d_freq + c->nchan;
   c->d_gain = c->d_dir + 3 * (size_t)c->nbeam;
+  c->d_i8scale = c->d_gain + 2 * (size_t)c->nchan * c->nant;
   c->d_wop = c->wop_buf[i];
+  c->d_wop8 = c->wop8_buf[i];
 }
 
 // no fallback: the device must be Blackwell (compute capability 10.x)
@@ -156,11 +200,30 @@ extern "C" int bf_set_workspace(bf_ctx *c, void *dev_ptr, size_t bytes) {
   for (int i = 0; i < c->nwbuf; ++i) {
     c->geom_buf[i] = p + (size_t)i * geom_bytes(c);
     c->wop_buf[i] = (__half *)(p + (size_t)c->nwbuf * geom_bytes(c) + (size_t)i * wop_bytes(c));
+    c->wop8_buf[i] = wop8_bytes(c) ? (signed char *)(p + (size_t)c->nwbuf * (geom_bytes(c) + wop_bytes(c)) + (size_t)i * wop8_bytes(c))
+                                   : nullptr;
   }
   c->active = 0; c->pending = -1; c->used[0] = c->used[1] = false;
   select_buffer(c, 0);
   c->have_geom = false;
   return BF_OK;
+}
+
+// per-channel scale of the int8 two-limb operand: (largest |gain| of the channel) / 16256
+static cudaError_t upload_i8scale(bf_ctx *c, cudaStream_t st) {
+  if (!c->d_wop8) return cudaSuccess;
+  c->h_i8scale.assign(c->nchan, 1.0 / BF_I8_QSCALE);
+  if (c->have_gains)
+    for (int ch = 0; ch < c->nchan; ++ch) {
+      double g2 = 0.0;
+      for (int n = 0; n < c->nant; ++n) {
+        const double *g = c->h_gain.data() + 2 * ((size_t)ch * c->nant + n);
+        const double a = g[0] * g[0] + g[1] * g[1];
+        if (a > g2) g2 = a;
+      }
+      c->h_i8scale[ch] = (g2 > 0.0 ? sqrt(g2) : 1.0) / BF_I8_QSCALE;
+    }
+  return cudaMemcpyAsync(c->d_i8scale, c->h_i8scale.data(), c->nchan * sizeof(double), cudaMemcpyHostToDevice, st);
 }
 
 static int check_geometry(bf_ctx *c, const double *ant, const double *freq, const double *dir) {
@@ -189,9 +252,10 @@ static int upload_and_generate(bf_ctx *c, const double *ant, const double *freq,
     e = cudaMemcpyAsync(c->d_gain, c->h_gain.data(), c->h_gain.size() * sizeof(double), cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(c, e, "gain H2D copy");
   }
+  if ((e = upload_i8scale(c, st)) != cudaSuccess) return cuda_fail(c, e, "int8 scale H2D copy");
   e = bf_launch_weights(c, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "weight generator launch");
-  c->launches += 1;
+  c->launches += c->d_wop8 ? 2 : 1;
   return BF_OK;
 }
 
@@ -270,9 +334,10 @@ extern "C" int bf_set_antenna_gains(bf_ctx *c, const double *gains, int per_chan
     select_buffer(c, c->active);
   }
   if (c->have_gains) e = cudaMemcpyAsync(c->d_gain, c->h_gain.data(), c->h_gain.size() * sizeof(double), cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = upload_i8scale(c, st);
   if (e == cudaSuccess) e = bf_launch_weights(c, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "weight regeneration");
-  c->launches += 1;
+  c->launches += c->d_wop8 ? 2 : 1;
   return BF_OK;
 }
 
@@ -312,13 +377,15 @@ static int launch_range(bf_ctx *c, const void *volt, void *out, int chan0, int n
   p.beam_scale = scale;
   p.mode = mode;
   p.wop = c->d_wop + (size_t)chan0 * (bf_wop_bytes_per_chan(c) / sizeof(__half));
-  int k = c->kernel_forced;
+  p.wop8 = c->d_wop8 ? c->d_wop8 + (size_t)chan0 * bf_i8_ncol(c->nbeam) * 64 : nullptr;
+  p.i8scale = c->d_i8scale + chan0;
   const char *why = "";
-  bool umma_ok = mode == BF_MODE_BEAMS ? bf_umma_shape_supported(c, &why) : bf_umma_supported(c, &why);
-  if (k == BF_KERNEL_AUTO) k = umma_ok ? BF_KERNEL_UMMA : BF_KERNEL_SIMT;
-  if (k == BF_KERNEL_UMMA && !umma_ok) return fail(c, BF_EUNSUPPORTED, "tensor-core kernel cannot run this shape: %s", why);
-  cudaError_t e = (k == BF_KERNEL_UMMA) ? bf_launch_umma(p, c->dtype, c->sm_count, st) : bf_launch_simt(p, c->dtype, st);
-  if (e != cudaSuccess) return cuda_fail(c, e, k == BF_KERNEL_UMMA ? "tensor-core kernel launch" : "SIMT kernel launch");
+  const int k = pick_kernel(c, mode, &why);
+  if (k == 0) return fail(c, BF_EUNSUPPORTED, "tensor-core kernel cannot run this shape: %s", why);
+  cudaError_t e = k == BF_KERNEL_UMMA_I8    ? bf_launch_umma_i8(p, c->sm_count, st)
+                  : k == BF_KERNEL_UMMA_F16 ? bf_launch_umma(p, c->dtype, c->sm_count, st)
+                                            : bf_launch_simt(p, c->dtype, st);
+  if (e != cudaSuccess) return cuda_fail(c, e, k == BF_KERNEL_SIMT ? "SIMT kernel launch" : "tensor-core kernel launch");
   c->launches += 1;
   return BF_OK;
 }

@@ -43,7 +43,21 @@ struct BfParams {
   float beam_scale;     // voltage-beam mode: y is multiplied by this before rounding to fp16
   int mode;             // BF_MODE_POWER (|y|^2 integrated over nint -> pow) or BF_MODE_BEAMS (y -> beams)
   const __half *wop;    // device, weight operand of the first channel of this launch
+  const signed char *wop8;  // int8 two-limb weight operand of the first channel (bf_umma_i8.cu), or NULL
+  const double *i8scale;    // per channel: y = (128 hi + lo) * i8scale[c]
+  int dbg;
 };
+
+// ---- int8 two-limb weight operand (bf_umma_i8.cu; few beams, small arrays) ---------------------
+// Each real coefficient a (the (re, -im) / (im, re) expansion above, gains folded in) is quantised to 15 bits,
+// q = rint(a / scale_c), scale_c = gmax_c / 16256 (gmax_c = largest |gain| of the channel, 1 without gains), and
+// split into two int8 limbs q = 128 hi + lo, hi = floor((q + 64) / 128) in [-127, 127], lo in [-64, 63].
+// Rows (= accumulator columns): 32 per chunk of 8 beams, row 32 ch + 4 i + j holds beam 8 ch + i,
+// j = 0 re-hi, 1 im-hi, 2 re-lo, 3 im-lo.  Memory: int8 [chan][ncol rows][64 bytes], each row's 16-byte chunk k
+// stored at chunk k ^ ((row >> 1) & 3): the 64-byte-swizzled shared-memory image tcgen05.mma reads.
+#define BF_I8_MAX_BEAMS 32
+#define BF_I8_QSCALE 16256.0
+__host__ __device__ inline int bf_i8_ncol(int nbeam) { return nbeam <= 8 ? 32 : nbeam <= 16 ? 64 : 128; }
 
 struct bf_ctx {
   int nant, nchan, nbeam, nsamp, nint, nbin;
@@ -54,14 +68,17 @@ struct bf_ctx {
   double *d_ant, *d_freq, *d_dir;
   double *d_gain;          // [nchan][nant][2] complex gains (always per channel on the device)
   bool have_gains;         // false = all ones (d_gain not read)
-  std::vector<double> h_gain;
+  std::vector<double> h_gain, h_i8scale;
   __half *d_wop;
+  signed char *d_wop8;     // int8 two-limb operand (NULL when the shape never takes the int8 kernel)
+  double *d_i8scale;       // [nchan]
   bool have_geom;
   // tracking beams (row f3): up to two (geometry, weight operand) buffers; runs read `active`, an update
   // writes the other one on its own stream and the next run switches over behind an event
   int nwbuf, active, pending;      // pending: -1 none, else the buffer the next run switches to
   char *geom_buf[2];
   __half *wop_buf[2];
+  signed char *wop8_buf[2];
   cudaEvent_t ev_upd, ev_use[2];
   bool have_wevents, used[2];
   std::vector<double> h_geom;
@@ -82,6 +99,8 @@ cudaError_t bf_launch_decode_weights(const bf_ctx *c, float *d_out, cudaStream_t
 cudaError_t bf_launch_simt(const BfParams &p, int dtype, cudaStream_t st);
 bool bf_umma_supported(const bf_ctx *c, const char **why);
 bool bf_umma_shape_supported(const bf_ctx *c, const char **why);  // ignoring nint (voltage-beam mode)
+bool bf_umma_i8_supported(const bf_ctx *c);
+cudaError_t bf_launch_umma_i8(const BfParams &p, int sm_count, cudaStream_t st);
 cudaError_t bf_launch_incoherent(const bf_ctx *c, const void *volt, float *out, cudaStream_t st);
 cudaError_t bf_launch_umma(const BfParams &p, int dtype, int sm_count, cudaStream_t st);
 cudaError_t bf_launch_umma_kblock(const BfParams &p, int dtype, int sm_count, cudaStream_t st);

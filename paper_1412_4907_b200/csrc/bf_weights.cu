@@ -10,6 +10,23 @@
 
 #define BF_C0 299792458.0
 
+// W'[c][b][n] = g[c][n] e^{-i 2 pi f_c/c0 (r_n . s_b)} in fp64
+__device__ __forceinline__ void steering_weight(const double *__restrict__ ant, const double *__restrict__ freq,
+                                                const double *__restrict__ dir, const double *__restrict__ gain,
+                                                int nant, int c, int b, int n, double &wre, double &wim) {
+  double dot = ant[3 * n] * dir[3 * b] + ant[3 * n + 1] * dir[3 * b + 1] + ant[3 * n + 2] * dir[3 * b + 2];
+  double turns = freq[c] * dot / BF_C0;
+  turns -= rint(turns);  // |turns| <= 1/2: exact subtraction, no accuracy lost to the big phase
+  double s, co;
+  sincospi(2.0 * turns, &s, &co);
+  wre = co; wim = -s;  // e^{-i phi}
+  if (gain) {  // W' = g W: antenna mask / gain calibration folded into the coefficients
+    const double gre = gain[2 * ((size_t)c * nant + n)], gim = gain[2 * ((size_t)c * nant + n) + 1];
+    const double tre = gre * wre - gim * wim, tim = gre * wim + gim * wre;
+    wre = tre; wim = tim;
+  }
+}
+
 __global__ void bf_weights_kernel(const double *__restrict__ ant, const double *__restrict__ freq,
                                   const double *__restrict__ dir, const double *__restrict__ gain,
                                   __half *__restrict__ wop, int nant,
@@ -29,23 +46,42 @@ __global__ void bf_weights_kernel(const double *__restrict__ ant, const double *
   int part = bf_row_part(r);
   float a0 = 0.f, a1 = 0.f;
   if (b < nbeam && n < nant) {
-    double dot = ant[3 * n] * dir[3 * b] + ant[3 * n + 1] * dir[3 * b + 1] + ant[3 * n + 2] * dir[3 * b + 2];
-    double turns = freq[c] * dot / BF_C0;
-    turns -= rint(turns);  // |turns| <= 1/2: exact subtraction, no accuracy lost to the big phase
-    double s, co;
-    sincospi(2.0 * turns, &s, &co);
-    double wre = co, wim = -s;  // e^{-i phi}
-    if (gain) {  // W' = g W: antenna mask / gain calibration folded into the coefficients
-      const double gre = gain[2 * ((size_t)c * nant + n)], gim = gain[2 * ((size_t)c * nant + n) + 1];
-      const double tre = gre * wre - gim * wim, tim = gre * wim + gim * wre;
-      wre = tre; wim = tim;
-    }
+    double wre, wim;
+    steering_weight(ant, freq, dir, gain, nant, c, b, n, wre, wim);
     if (part == 0) { a0 = (float)wre; a1 = (float)(-wim); }
     else           { a0 = (float)wim; a1 = (float)wre; }
   }
   int kb = (2 * n) / BF_KBLOCK, kk = (2 * n) % BF_KBLOCK;
   size_t o = (((size_t)c * nMt + mt) * nKb + kb) * (BF_TILE_ROWS * BF_KBLOCK) + bf_tile_off(r, kk);
   *reinterpret_cast<__half2 *>(wop + o) = __floats2half2_rn(a0, a1);
+}
+
+// the same weights as two int8 limbs in the bf_umma_i8.cu operand layout (bf_internal.h); one thread per
+// (chan, row, antenna slot 0..31)
+__global__ void bf_weights_i8_kernel(const double *__restrict__ ant, const double *__restrict__ freq,
+                                     const double *__restrict__ dir, const double *__restrict__ gain,
+                                     const double *__restrict__ scale, signed char *__restrict__ wop8, int nant,
+                                     int nchan, int nbeam, int ncol) {
+  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  long long total = (long long)nchan * ncol * 32;
+  if (idx >= total) return;
+  const int n = (int)(idx & 31);
+  const int row = (int)((idx >> 5) % ncol);
+  const int c = (int)((idx >> 5) / ncol);
+  const int b = 8 * (row >> 5) + ((row & 31) >> 2), j = row & 3;   // j: 0 re-hi, 1 im-hi, 2 re-lo, 3 im-lo
+  int l0 = 0, l1 = 0;
+  if (b < nbeam && n < nant) {
+    double wre, wim;
+    steering_weight(ant, freq, dir, gain, nant, c, b, n, wre, wim);
+    const double a0 = (j & 1) ? wim : wre, a1 = (j & 1) ? wre : -wim;   // coefficients of x_re, x_im
+    const int q0 = (int)rint(a0 / scale[c]), q1 = (int)rint(a1 / scale[c]);
+    const int h0 = (q0 + 64) >> 7, h1 = (q1 + 64) >> 7;                 // floor((q + 64) / 128)
+    l0 = (j & 2) ? q0 - 128 * h0 : h0;
+    l1 = (j & 2) ? q1 - 128 * h1 : h1;
+  }
+  const int k = 2 * n;                                                  // byte position inside the 64-byte row
+  const size_t o = ((size_t)c * ncol + row) * 64 + ((((k >> 4) ^ ((row >> 1) & 3)) << 4) | (k & 15));
+  *reinterpret_cast<char2 *>(wop8 + o) = make_char2((signed char)l0, (signed char)l1);
 }
 
 cudaError_t bf_launch_weights(const bf_ctx *c, cudaStream_t st) {
@@ -55,6 +91,14 @@ cudaError_t bf_launch_weights(const bf_ctx *c, cudaStream_t st) {
   bf_weights_kernel<<<(unsigned)blocks, threads, 0, st>>>(c->d_ant, c->d_freq, c->d_dir,
                                                           c->have_gains ? c->d_gain : nullptr, c->d_wop, c->nant,
                                                           c->nchan, c->nbeam, c->nMt, c->nKb);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess || !c->d_wop8) return e;
+  const int ncol = bf_i8_ncol(c->nbeam);
+  total = (long long)c->nchan * ncol * 32;
+  blocks = (total + threads - 1) / threads;
+  bf_weights_i8_kernel<<<(unsigned)blocks, threads, 0, st>>>(c->d_ant, c->d_freq, c->d_dir,
+                                                             c->have_gains ? c->d_gain : nullptr, c->d_i8scale,
+                                                             c->d_wop8, c->nant, c->nchan, c->nbeam, ncol);
   return cudaGetLastError();
 }
 
@@ -77,10 +121,33 @@ __global__ void bf_decode_weights_kernel(const __half *__restrict__ wop, float *
   out[2 * idx + 1] = wim;
 }
 
+// int8 two-limb operand -> logical fp32 [chan][beam][ant][2]
+__global__ void bf_decode_weights_i8_kernel(const signed char *__restrict__ wop8, const double *__restrict__ scale,
+                                            float *__restrict__ out, int nant, int nchan, int nbeam, int ncol) {
+  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  long long total = (long long)nchan * nbeam * nant;
+  if (idx >= total) return;
+  int n = (int)(idx % nant);
+  long long t = idx / nant;
+  int b = (int)(t % nbeam);
+  int c = (int)(t / nbeam);
+  const int row0 = 32 * (b >> 3) + 4 * (b & 7), k = 2 * n;
+  auto at = [&](int row) { return (int)wop8[((size_t)c * ncol + row) * 64 + ((((k >> 4) ^ ((row >> 1) & 3)) << 4) | (k & 15))]; };
+  // coefficient of x_re in the re row is W_re, in the im row W_im
+  out[2 * idx] = (float)((128 * at(row0) + at(row0 + 2)) * scale[c]);
+  out[2 * idx + 1] = (float)((128 * at(row0 + 1) + at(row0 + 3)) * scale[c]);
+}
+
 cudaError_t bf_launch_decode_weights(const bf_ctx *c, float *d_out, cudaStream_t st) {
   long long total = (long long)c->nchan * c->nbeam * c->nant;
   int threads = 256;
   long long blocks = (total + threads - 1) / threads;
+  if (c->d_wop8 && c->kernel_forced != BF_KERNEL_SIMT && c->kernel_forced != BF_KERNEL_UMMA_F16) {
+    // the int8 kernel is the one that runs: report ITS operand
+    bf_decode_weights_i8_kernel<<<(unsigned)blocks, threads, 0, st>>>(c->d_wop8, c->d_i8scale, d_out, c->nant, c->nchan,
+                                                                      c->nbeam, bf_i8_ncol(c->nbeam));
+    return cudaGetLastError();
+  }
   bf_decode_weights_kernel<<<(unsigned)blocks, threads, 0, st>>>(c->d_wop, d_out, c->nant, c->nchan, c->nbeam,
                                                                  c->nMt, c->nKb);
   return cudaGetLastError();

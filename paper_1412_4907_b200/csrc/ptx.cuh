@@ -133,6 +133,31 @@ __host__ __device__ constexpr uint32_t make_idesc_f16(uint32_t M, uint32_t N) {
   return (1u << 4) | (0u << 7) | (0u << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
 }
 
+// D[tmem] (+)= A[smem] * B[smem], int8 inputs, int32 accumulate (K = 32 per instruction)
+BF_DEVI void mma_i8_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// K-major operand with rows of 64 bytes, 64-byte swizzle (16-byte chunk index ^= (row >> 1) & 3; the
+// pattern repeats every 8 rows = 512 bytes = the stride byte offset); layout type 4 = SWIZZLE_64B
+BF_DEVI uint64_t make_sdesc_k_sw64(uint32_t saddr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr >> 4) & 0x3FFF);
+  d |= (uint64_t)1 << 16;
+  d |= (uint64_t)(512 >> 4) << 32;
+  d |= (uint64_t)1 << 46;
+  d |= (uint64_t)4 << 61;
+  return d;
+}
+// Instruction descriptor for kind::i8: [4,6) D format 2 = s32 | [7,10) A format 1 = signed 8 bit | [10,13) B
+// format 1 = signed 8 bit | bit 15 / 16: A / B major 0 = K | [17,23) N >> 3 | [24,29) M >> 4
+__host__ __device__ constexpr uint32_t make_idesc_i8(uint32_t M, uint32_t N) {
+  return (2u << 4) | (1u << 7) | (1u << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
+}
+
 // 32 lanes x 32 consecutive 32-bit columns: thread l of the warp gets lane (base lane + l)
 #define BF_TMEM_LD_32x32b_X32(taddr, r)                                                           \
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "                                           \

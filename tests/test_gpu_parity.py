@@ -63,7 +63,7 @@ def run_gpu(bf, w, v_host, kernel):
 
 
 def kernels(bf):
-    return [bf.BF_KERNEL_SIMT, bf.BF_KERNEL_AUTO]
+    return [bf.BF_KERNEL_SIMT, bf.BF_KERNEL_AUTO, bf.BF_KERNEL_UMMA_F16]
 
 
 # ------------------------------------------------------------------ a1: weights
@@ -122,7 +122,7 @@ SMALL = [
 ]
 
 
-@pytest.mark.parametrize("kernel", ["simt", "auto"])
+@pytest.mark.parametrize("kernel", ["simt", "auto", "f16"])
 @pytest.mark.parametrize("shape", SMALL, ids=lambda s: "N%d-C%d-B%d-T%d-I%d-%s" % s)
 def test_small_shapes(bf, shape, kernel):
     N, C, B, T, I, dtype = shape
@@ -134,8 +134,71 @@ def test_small_shapes(bf, shape, kernel):
     w = synthetic.Workload("small", N, C, B, T, I, dtype, 0, r, f, s, sig, [(s[B // 2].copy(), amp)])
     v = w.make_voltages()
     ref = oracle.beamform(r, f, s, v, I)
-    out, used = run_gpu(bf, w, v, bf.BF_KERNEL_SIMT if kernel == "simt" else bf.BF_KERNEL_AUTO)
+    k = {"simt": bf.BF_KERNEL_SIMT, "auto": bf.BF_KERNEL_AUTO, "f16": bf.BF_KERNEL_UMMA_F16}[kernel]
+    if kernel == "f16":
+        B_ = bf.Beamformer(N, C, B, T, I, dtype=bf_dtype(bf, w), kernel=k)
+        name = B_.kernel_name
+        B_.close()
+        if name == "unsupported":
+            pytest.skip("no fp16 tensor-core variant for this shape")
+    out, used = run_gpu(bf, w, v, k)
     check_rows(out, ref, tol_for(I))
+
+
+# ------------------------------------------------------------------ the int8-operand kernel (few beams), forced
+I8_SHAPES = [
+    # nant nchan nbeam nsamp nint
+    (32, 3, 1, 256, 16),
+    (32, 2, 4, 1000, 8),       # ragged time tail: the TMA zero-fills past nsamp
+    (32, 2, 8, 384, 1),        # nint = 1: every lane stores its own sample
+    (32, 2, 9, 512, 2),        # second 8-beam chunk (64 accumulator columns)
+    (32, 2, 16, 512, 4),
+    (32, 2, 16, 4096, 16),     # sweep's shape: several tiles per CTA, both epilogue sets
+    (32, 2, 13, 768, 32),      # one bin per warp
+    (32, 2, 16, 1536, 64),     # nint = 64: two tiles per super-tile, running sums in registers
+    (32, 1, 7, 960, 96),       # nint = 96 = 3 x 32: only this kernel integrates it on tensor cores
+    (32, 1, 16, 2048, 1024),   # long bins
+    (32, 1, 32, 512, 16),      # 32 beams: 128 accumulator columns
+    (32, 2, 17, 300, 4),       # ragged, third chunk mostly padding
+    (8, 2, 4, 128, 16),        # rows of 16 bytes: one K step, zero-filled to 32
+    (16, 2, 9, 300, 4),
+    (24, 2, 5, 256, 8),        # rows of 48 bytes
+]
+
+
+@pytest.mark.parametrize("shape", I8_SHAPES, ids=lambda s: "N%d-C%d-B%d-T%d-I%d" % s)
+def test_i8_kernel_shapes(bf, shape):
+    N, C, B, T, I = shape
+    w = synthetic.make_case(N, C, B, T, I, "ci8", seed=3)
+    v = w.make_voltages()
+    ref = oracle.beamform(w.ant_xyz, w.freqs, w.beam_dir, v, I)
+    out, _ = run_gpu(bf, w, v, bf.BF_KERNEL_UMMA_I8)
+    # 15-bit weights: far inside the 1e-3 bar even at nint = 1 (measured ~1e-4 there)
+    worst = check_rows(out, ref, TOL)
+    print(f"i8 {shape} worst={worst:.2e}")
+
+
+def test_i8_kernel_is_the_auto_choice_for_few_beams_and_f16_can_be_forced(bf):
+    w = synthetic.make_workload("sweep", nbeam=16).sub(nchan=4, nsamp=2048)
+    v = w.make_voltages()
+    ref = oracle.beamform(w.ant_xyz, w.freqs, w.beam_dir, v, w.nint)
+    B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint)
+    assert B.kernel_name == "umma-i8"
+    B.close()
+    for k, name in ((bf.BF_KERNEL_UMMA_I8, "umma-i8"), (bf.BF_KERNEL_UMMA_F16, "umma-f16-resident")):
+        B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint, kernel=k)
+        assert B.kernel_name == name
+        B.close()
+        out, _ = run_gpu(bf, w, v, k)
+        check_rows(out, ref)
+    # shapes it does not take are refused when forced
+    import torch
+    B = bf.Beamformer(64, 2, 4, 256, 16, kernel=bf.BF_KERNEL_UMMA_I8)
+    B.set_geometry(synthetic.grid(8, 8, 3.0, 3.0), [1e8, 2e8], synthetic.zenith_fan(4))
+    with pytest.raises(bf.BfError) as e:
+        B.run(torch.zeros((2, 256, 64, 2), dtype=torch.int8, device="cuda"))
+    assert e.value.code == bf.BF_EUNSUPPORTED
+    B.close()
 
 
 def test_int8_extremes(bf):
@@ -197,7 +260,7 @@ def test_full_size_sampled_channels(bf, name, nbeam, nsample):
 
 
 # ------------------------------------------------------------------ f2: antenna mask / complex gains in the weights
-@pytest.mark.parametrize("kernel", ["simt", "auto"])
+@pytest.mark.parametrize("kernel", ["simt", "auto", "f16"])
 @pytest.mark.parametrize("mode", ["mask", "per_antenna", "per_channel"])
 def test_antenna_gains(bf, mode, kernel):
     """W' = g W (PAPER.md:180 sub-arraying mask, PAPER.md:50 gain calibration).  The oracle knows nothing about
@@ -219,7 +282,7 @@ def test_antenna_gains(bf, mode, kernel):
     x = (v[..., 0].astype(np.float64) + 1j * v[..., 1]) * gfull[:, None, :]
     ref = oracle.beamform(w.ant_xyz, w.freqs, w.beam_dir, np.ascontiguousarray(x), w.nint)
     B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint,
-                      kernel=bf.BF_KERNEL_SIMT if kernel == "simt" else bf.BF_KERNEL_AUTO)
+                      kernel={"simt": bf.BF_KERNEL_SIMT, "auto": bf.BF_KERNEL_AUTO, "f16": bf.BF_KERNEL_UMMA_F16}[kernel])
     B.set_antenna_gains(g, per_channel=(mode == "per_channel"))   # before the geometry: applied by set_geometry
     B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
     vd = torch.from_numpy(v).cuda()
