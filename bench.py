@@ -194,7 +194,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="medium")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--kernel", default="auto", choices=["auto", "simt", "umma"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "simt", "umma", "f16", "i8"])
     ap.add_argument("--mode", default="power", choices=["power", "beams", "incoherent"],
                     help="power = the headline path (bf_run); beams / incoherent = SURVEY 8(f) row f4 side modes")
     ap.add_argument("--nbeam", type=int, default=0, help="override the workload's beam count (beams mode: default 8)")
@@ -234,7 +234,8 @@ def main():
         args.no_cpu_baseline = True
     w.seed = rank_seed(w.seed, rank)
     peaks = load_peaks()
-    kern = {"auto": bf.BF_KERNEL_AUTO, "simt": bf.BF_KERNEL_SIMT, "umma": bf.BF_KERNEL_UMMA}[args.kernel]
+    kern = {"auto": bf.BF_KERNEL_AUTO, "simt": bf.BF_KERNEL_SIMT, "umma": bf.BF_KERNEL_UMMA,
+            "f16": bf.BF_KERNEL_UMMA_F16, "i8": bf.BF_KERNEL_UMMA_I8}[args.kernel]
     dt = {"ci8": bf.BF_CI8, "cf16": bf.BF_CF16, "ci4": bf.BF_CI4}[w.dtype]
 
     B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint, dtype=dt, kernel=kern, device=dev)
@@ -369,11 +370,11 @@ def main():
         line = {
             "metric": METRIC if args.mode == "power" else METRIC + " [side mode: %s]" % args.mode, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "i8->i32 (dp4a)" if args.mode == "incoherent" else ("f16xf16->f32" if B.selected_kernel == bf.BF_KERNEL_UMMA else "f32"),
+            "dtype": "i8->i32 (dp4a)" if args.mode == "incoherent" else {"umma-i8": "i8xi8->i32", "simt": "f32"}.get(B.kernel_name, "f16xf16->f32"),
             "data": "synthetic",
             "config": {"workload": w.name if args.mode == "power" else w.name + ":" + args.mode, "nant": w.nant, "nchan": w.nchan, "nbeam": w.nbeam, "nsamp": w.nsamp,
                        "nint": w.nint, "input": w.dtype, "l2": "input buffer (%.0f MB) >> L2 (126 MB), no flush needed" % (w.in_bytes / 1e6),
-                       "kernel": {1: "simt", 2: "umma"}[B.selected_kernel], "parallelism": f"replicas x{world}"},
+                       "kernel": B.kernel_name, "parallelism": f"replicas x{world}"},
             "ant_samples_per_s": world * w.nchan * w.nsamp * w.nant * K / (total_ms_max * 1e-3),
             "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
             "context": {"paper_k20_tflops": 1.3, "note": "paper's number is a Tesla K20 with 4-bit input (PAPER.md:15): context, not a baseline for this config"},

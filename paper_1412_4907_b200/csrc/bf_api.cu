@@ -101,7 +101,7 @@ extern "C" int bf_set_kernel(bf_ctx *c, int kernel) {
 }
 
 // the int8 kernel takes over below this many beams (measured crossover against the fp16 kernel)
-#define BF_I8_AUTO_BEAMS 16
+#define BF_I8_AUTO_BEAMS 32
 
 // which kernel bf_run launches: BF_KERNEL_SIMT, BF_KERNEL_UMMA_F16 or BF_KERNEL_UMMA_I8; 0 + *why if the
 // forced kernel cannot run the shape

@@ -45,7 +45,6 @@ struct BfParams {
   const __half *wop;    // device, weight operand of the first channel of this launch
   const signed char *wop8;  // int8 two-limb weight operand of the first channel (bf_umma_i8.cu), or NULL
   const double *i8scale;    // per channel: y = (128 hi + lo) * i8scale[c]
-  int dbg;
 };
 
 // ---- int8 two-limb weight operand (bf_umma_i8.cu; few beams, small arrays) ---------------------

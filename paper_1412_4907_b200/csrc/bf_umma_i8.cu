@@ -24,9 +24,10 @@
 //
 // Warp roles (one persistent CTA per SM over a contiguous range of (channel, super-tile)): warps 0-7 epilogue
 // (two sets of four; set s takes the super-tiles of its parity, warp quadrant q = TMEM lanes 32q..), warp 8
-// MMA issue + TMEM allocation, warp 9 one thread issuing TMA.  ~190 KiB of input in flight per SM.
+// MMA issue + TMEM allocation, warp 9 (WIDE: 9 and 10) one thread each issuing TMA.  ~190 KiB of input in
+// flight per SM.  All role loops keep 32-bit wrap counters: a 64-bit division per tile in the single producer
+// thread was measurably on the critical path.
 #include <cuda.h>
-#include <stdlib.h>
 
 #include "bf_internal.h"
 #include "ptx.cuh"
@@ -125,7 +126,7 @@ bf_umma_i8_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
     const bool writer = (lane & ((LBIN >> HALVINGS) - 1)) == 0;   // one lane per (bin, beam) after the plain butterfly steps
     const int nbeam = p.nbeam, nbin = p.nbin;
     int c = c0, sp = sp0;
-    long long ti = 0;                                             // tile counter of this CTA (all roles count alike)
+    int ti = 0;                                                   // tile counter of this CTA (all roles count alike)
     for (int s = 0; s < n_super; ++s) {
       if ((s & 1) == set) {
         float acc[NCH][8];
@@ -134,8 +135,8 @@ bf_umma_i8_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
 #pragma unroll
           for (int i = 0; i < 8; ++i) acc[ch][i] = 0.f;
         for (int g = 0; g < G; ++g, ++ti) {
-          const int a = (int)(ti % NACC);
-          mbar_wait(bar_t_full + 8 * a, (uint32_t)((ti / NACC) & 1));
+          const int a = ti & (NACC - 1);
+          mbar_wait(bar_t_full + 8 * a, (uint32_t)((ti >> ilog2(NACC)) & 1));
           tc_fence_after();
 #pragma unroll
           for (int ch = 0; ch < NCH; ++ch) {
@@ -147,7 +148,6 @@ bf_umma_i8_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
               __syncwarp();
               if (lane0) mbar_arrive(bar_t_empty + 8 * a);
             }
-            if (p.dbg & 1) continue;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
               const int re = ((int)v[4 * i] << 7) + (int)v[4 * i + 2];       // 128 hi + lo, exact
@@ -163,7 +163,7 @@ bf_umma_i8_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
         const int bin = (32 / LBIN) * (4 * sp + quad) + lane / LBIN;
 #pragma unroll
         for (int ch = 0; ch < NCH; ++ch) {
-          if (!(p.dbg & 2)) LaneReduce<8, LBIN / 2>::run(acc[ch], lane);
+          LaneReduce<8, LBIN / 2>::run(acc[ch], lane);
           if (writer && bin < nbin) {
 #pragma unroll
             for (int j = 0; j < NFINAL; ++j) {
@@ -181,7 +181,8 @@ bf_umma_i8_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
     // =========================================================================== MMA issue
     constexpr uint32_t idesc = make_idesc_i8(L_TILE_T, NCOL);
     int c = c0, sp = sp0, prev_c = -1, wi = 0, wb = 0;
-    long long ti = 0;
+    int ti = 0, st = 0;
+    uint32_t st_par = 0;
     for (int s = 0; s < n_super; ++s) {
       if (c != prev_c) {
         if (wi > 0 && elect_one()) tc_commit(bar_w_empty + 8 * wb);   // my MMAs so far have left the old buffer
@@ -192,20 +193,21 @@ bf_umma_i8_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
       }
       const uint64_t bdesc = make_sdesc_k_sw64(sW + wb * W_BYTES);
       for (int g = 0; g < G; ++g, ++ti) {
-        const int st = (int)(ti % NST), a = (int)(ti % NACC);
-        mbar_wait(bar_a_full + 8 * st, (uint32_t)((ti / NST) & 1));
-        mbar_wait(bar_t_empty + 8 * a, (uint32_t)(((ti / NACC) & 1) ^ 1));
+        const int a = ti & (NACC - 1);
+        mbar_wait(bar_a_full + 8 * st, st_par);
+        mbar_wait(bar_t_empty + 8 * a, (uint32_t)(((ti >> ilog2(NACC)) & 1) ^ 1));
         tc_fence_after();
         if (elect_one()) {
           const uint64_t adesc = make_sdesc_k_sw64(sA + st * L_STAGE_BYTES);
           const uint32_t d = tmem_base + a * NCOL;
 #pragma unroll
           for (int k = 0; k < 2; ++k)   // 32 bytes along K inside the 64-byte swizzle atom
-            if (k < nks && !(p.dbg & 4)) mma_i8_ss(d, adesc + 2 * k, bdesc + 2 * k, idesc, k > 0);
+            if (k < nks) mma_i8_ss(d, adesc + 2 * k, bdesc + 2 * k, idesc, k > 0);
           tc_commit(bar_t_full + 8 * a);
           tc_commit(bar_a_empty + 8 * st);
         }
         __syncwarp();
+        if (++st == NST) { st = 0; st_par ^= 1; }
       }
       if (++sp == n_super_chan) { sp = 0; ++c; }
     }
@@ -214,7 +216,8 @@ bf_umma_i8_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
     tma_prefetch_desc(&tmap);
     tma_prefetch_desc(&tmap32);
     int c = c0, sp = sp0, prev_c = -1, wi = 0;
-    long long ti = 0;
+    int st = 0;
+    uint32_t st_par = 1;
     for (int s = 0; s < n_super; ++s) {
       if (c != prev_c) {
         prev_c = c;
@@ -224,11 +227,10 @@ bf_umma_i8_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
         bulk_g2s(sW + wb * W_BYTES, reinterpret_cast<const char *>(p.wop8) + (size_t)c * W_BYTES, W_BYTES, bar_w_full + 8 * wb);
         ++wi;
       }
-      for (int g = 0; g < G; ++g, ++ti) {
-        const int st = (int)(ti % NST);
-        mbar_wait(bar_a_empty + 8 * st, (uint32_t)(((ti / NST) & 1) ^ 1));
+      for (int g = 0; g < G; ++g) {
+        mbar_wait(bar_a_empty + 8 * st, st_par);
         mbar_arrive_expect_tx(bar_a_full + 8 * st, L_STAGE_BYTES);
-        if (G == 1 && !(p.dbg & 8)) {  // the four quadrants are contiguous: one box of 128 samples
+        if (G == 1) {  // the four quadrants are contiguous: one box of 128 samples
           tma_load_3d(sA + st * L_STAGE_BYTES, &tmap, 0, L_TILE_T * sp, c, bar_a_full + 8 * st);
         } else {
 #pragma unroll
@@ -236,6 +238,7 @@ bf_umma_i8_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
             tma_load_3d(sA + st * L_STAGE_BYTES + q * L_BOX_BYTES, &tmap32, 0, 32 * G * (4 * sp + q) + 32 * g, c,
                         bar_a_full + 8 * st);
         }
+        if (++st == NST) { st = 0; st_par ^= 1; }
       }
       if (++sp == n_super_chan) { sp = 0; ++c; }
     }
@@ -257,7 +260,7 @@ bf_umma_i8_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
 constexpr int W_STAGE_BYTES = 128 * 128;
 
 template <int NCOL, int LBIN, int NST>
-__global__ void __launch_bounds__(L_THREADS, 1)
+__global__ void __launch_bounds__(L_THREADS + 32, 1)
 bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap32,
                    const long long total_super, const int n_super_chan, const int G) {
   extern __shared__ uint8_t smem_raw[];
@@ -309,7 +312,7 @@ bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
     const bool writer = (lane & ((LB >> HALVINGS) - 1)) == 0;
     const int nbeam = p.nbeam, nbin = p.nbin;
     int c = c0, sp = sp0;
-    long long ti = 0;
+    int ti = 0;                                                   // tile counter of this CTA (all roles count alike)
     for (int s = 0; s < n_super; ++s) {
       if ((s & 1) == set) {
         float acc[NCH][8], acc1[LBIN == 0 ? NCH : 1][8];   // acc1: the odd sample's own bin when nint = 1
@@ -318,8 +321,8 @@ bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
 #pragma unroll
           for (int i = 0; i < 8; ++i) acc[ch][i] = 0.f;
         for (int g = 0; g < G; ++g, ++ti) {
-          const int a = (int)(ti % NACC);
-          mbar_wait(bar_t_full + 8 * a, (uint32_t)((ti / NACC) & 1));
+          const int a = ti & (NACC - 1);
+          mbar_wait(bar_t_full + 8 * a, (uint32_t)((ti >> ilog2(NACC)) & 1));
           tc_fence_after();
 #pragma unroll
           for (int ch = 0; ch < NCH; ++ch) {
@@ -384,7 +387,8 @@ bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
     // =========================================================================== MMA issue
     constexpr uint32_t idesc = make_idesc_i8(128, NCOL);
     int c = c0, sp = sp0, prev_c = -1, wi = 0, wb = 0;
-    long long ti = 0;
+    int ti = 0, st = 0;
+    uint32_t st_par = 0;
     for (int s = 0; s < n_super; ++s) {
       if (c != prev_c) {
         if (wi > 0 && elect_one()) tc_commit(bar_w_empty + 8 * wb);
@@ -395,9 +399,9 @@ bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
       }
       const uint64_t bdesc = make_sdesc_k_sw64(sW + wb * W_BYTES);
       for (int g = 0; g < G; ++g, ++ti) {
-        const int st = (int)(ti % NST), a = (int)(ti % NACC);
-        mbar_wait(bar_a_full + 8 * st, (uint32_t)((ti / NST) & 1));
-        mbar_wait(bar_t_empty + 8 * a, (uint32_t)(((ti / NACC) & 1) ^ 1));
+        const int a = ti & (NACC - 1);
+        mbar_wait(bar_a_full + 8 * st, st_par);
+        mbar_wait(bar_t_empty + 8 * a, (uint32_t)(((ti >> ilog2(NACC)) & 1) ^ 1));
         tc_fence_after();
         if (elect_one()) {
           const uint64_t adesc = make_sdesc_k_sw128(sA + st * W_STAGE_BYTES);
@@ -410,27 +414,36 @@ bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
           tc_commit(bar_a_empty + 8 * st);
         }
         __syncwarp();
+        if (++st == NST) { st = 0; st_par ^= 1; }
       }
       if (++sp == n_super_chan) { sp = 0; ++c; }
     }
-  } else if (warp == L_TMA_WARP && lane == 0) {
-    // =========================================================================== TMA producer (one thread)
+  } else if ((warp == L_TMA_WARP || warp == L_TMA_WARP + 1) && lane == 0) {
+    // =========================================================================== TMA producers (two threads)
+    // producer j issues the tiles of parity j (measured: the TMA unit overlaps two boxes, 0.097 -> 0.092 ms on
+    // the sweep); producer 0 also brings in the coefficients
+    const int pj = warp - L_TMA_WARP;
+    constexpr int npj = 2;
+    static_assert(NST % npj == 0, "stages are dealt to the producers by parity");
     tma_prefetch_desc(&tmap);
     tma_prefetch_desc(&tmap32);
     int c = c0, sp = sp0, prev_c = -1, wi = 0;
-    long long ti = 0;
+    int ti = 0, st = pj;                 // producer j: tiles j, j + npj, .. -> stages j, j + npj, .. (NST even)
+    uint32_t st_par = 1;                 // parity of a_empty[st] to wait for (passes on the fresh barrier)
     for (int s = 0; s < n_super; ++s) {
       if (c != prev_c) {
         prev_c = c;
-        const int wb = wi & 1;
-        mbar_wait(bar_w_empty + 8 * wb, (uint32_t)(((wi >> 1) & 1) ^ 1));
-        mbar_arrive_expect_tx(bar_w_full + 8 * wb, W_BYTES);
-        bulk_g2s(sW + wb * W_BYTES, reinterpret_cast<const char *>(p.wop8) + (size_t)c * W_BYTES, W_BYTES, bar_w_full + 8 * wb);
+        if (pj == 0) {
+          const int wb = wi & 1;
+          mbar_wait(bar_w_empty + 8 * wb, (uint32_t)(((wi >> 1) & 1) ^ 1));
+          mbar_arrive_expect_tx(bar_w_full + 8 * wb, W_BYTES);
+          bulk_g2s(sW + wb * W_BYTES, reinterpret_cast<const char *>(p.wop8) + (size_t)c * W_BYTES, W_BYTES, bar_w_full + 8 * wb);
+        }
         ++wi;
       }
       for (int g = 0; g < G; ++g, ++ti) {
-        const int st = (int)(ti % NST);
-        mbar_wait(bar_a_empty + 8 * st, (uint32_t)(((ti / NST) & 1) ^ 1));
+        if (npj == 2 && (ti & 1) != pj) continue;
+        mbar_wait(bar_a_empty + 8 * st, st_par);
         mbar_arrive_expect_tx(bar_a_full + 8 * st, W_STAGE_BYTES);
         if (G == 1) {   // rows (sample pairs) 128 sp .. 128 sp + 127: one box
           tma_load_3d(sA + st * W_STAGE_BYTES, &tmap, 0, 128 * sp, c, bar_a_full + 8 * st);
@@ -439,6 +452,7 @@ bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
           for (int q = 0; q < 4; ++q)
             tma_load_3d(sA + st * W_STAGE_BYTES + q * 4096, &tmap32, 0, 32 * G * (4 * sp + q) + 32 * g, c, bar_a_full + 8 * st);
         }
+        if ((st += npj) >= NST) { st -= NST; st_par ^= 1; }
       }
       if (++sp == n_super_chan) { sp = 0; ++c; }
     }
@@ -509,7 +523,7 @@ cudaError_t launch_i8w(const BfParams &p, int sm_count, cudaStream_t st) {
   e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   const int grid = (int)(total < sm_count ? total : sm_count);
-  kern<<<grid, L_THREADS, smem, st>>>(p, tm, tm32, total, n_super_chan, G);
+  kern<<<grid, L_THREADS + 32, smem, st>>>(p, tm, tm32, total, n_super_chan, G);
   return cudaGetLastError();
 }
 
@@ -568,12 +582,9 @@ bool bf_umma_i8_supported(const bf_ctx *c) {
   return (I <= 32 && (I & (I - 1)) == 0) || I % 32 == 0;
 }
 
-cudaError_t bf_launch_umma_i8(const BfParams &p_, int sm_count, cudaStream_t st) {
-  BfParams p = p_;
-  { const char *e = getenv("BF_DBG"); p.dbg = e ? atoi(e) : 0; }
+cudaError_t bf_launch_umma_i8(const BfParams &p, int sm_count, cudaStream_t st) {
   // 32 antennas, an even number of samples and nint 2^k <= 64 or a multiple of 64: rows of two samples
-  const bool wide = p.nant == 32 && p.nsamp % 2 == 0 && ((p.nint <= 64 && (p.nint & (p.nint - 1)) == 0) || p.nint % 64 == 0) &&
-                    !(p.dbg & 16);
+  const bool wide = p.nant == 32 && p.nsamp % 2 == 0 && ((p.nint <= 64 && (p.nint & (p.nint - 1)) == 0) || p.nint % 64 == 0);
   if (wide) {
     if (p.nbeam <= 8) return launch_i8w_nint<32>(p, sm_count, st);
     if (p.nbeam <= 16) return launch_i8w_nint<64>(p, sm_count, st);
