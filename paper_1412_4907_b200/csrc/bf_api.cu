@@ -109,7 +109,7 @@ static int pick_kernel(const bf_ctx *c, int mode, const char **why) {
   int k = c->kernel_forced;
   *why = "";
   if (k == BF_KERNEL_SIMT) return BF_KERNEL_SIMT;
-  const bool i8_ok = mode == BF_MODE_POWER && i8_shape(c) && bf_umma_i8_supported(c);
+  const bool i8_ok = i8_shape(c) && bf_umma_i8_supported(c, mode);
   if (k == BF_KERNEL_UMMA_I8) {
     if (!i8_ok) *why = "int8 kernel needs complex int8 input, nant % 8 == 0 and <= 32, <= 32 beams, nint 2^k <= 32 or % 32 == 0";
     return i8_ok ? BF_KERNEL_UMMA_I8 : 0;

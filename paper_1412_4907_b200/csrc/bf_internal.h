@@ -98,7 +98,7 @@ cudaError_t bf_launch_decode_weights(const bf_ctx *c, float *d_out, cudaStream_t
 cudaError_t bf_launch_simt(const BfParams &p, int dtype, cudaStream_t st);
 bool bf_umma_supported(const bf_ctx *c, const char **why);
 bool bf_umma_shape_supported(const bf_ctx *c, const char **why);  // ignoring nint (voltage-beam mode)
-bool bf_umma_i8_supported(const bf_ctx *c);
+bool bf_umma_i8_supported(const bf_ctx *c, int mode);
 cudaError_t bf_launch_umma_i8(const BfParams &p, int sm_count, cudaStream_t st);
 cudaError_t bf_launch_incoherent(const bf_ctx *c, const void *volt, float *out, cudaStream_t st);
 cudaError_t bf_launch_umma(const BfParams &p, int dtype, int sm_count, cudaStream_t st);

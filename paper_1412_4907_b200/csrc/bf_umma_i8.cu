@@ -259,7 +259,8 @@ bf_umma_i8_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
 // LBIN: lanes per bin (nint / 2 for 2 <= nint <= 64, 32 for nint = 64 G); 0 = nint 1 (two bins per lane).
 constexpr int W_STAGE_BYTES = 128 * 128;
 
-template <int NCOL, int LBIN, int NST>
+// BEAMS: voltage-beam mode (row f4): y itself as fp16 (re, im), no detection, nint ignored.
+template <int NCOL, int LBIN, int NST, bool BEAMS>
 __global__ void __launch_bounds__(L_THREADS + 32, 1)
 bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap32,
                    const long long total_super, const int n_super_chan, const int G) {
@@ -314,7 +315,40 @@ bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
     int c = c0, sp = sp0;
     int ti = 0;                                                   // tile counter of this CTA (all roles count alike)
     for (int s = 0; s < n_super; ++s) {
-      if ((s & 1) == set) {
+      if (BEAMS && (s & 1) == set) {
+        // ---- voltage beams: lane r holds samples 2r and 2r+1 of every beam; 8 bytes per beam and lane
+        const int a = ti & (NACC - 1);
+        mbar_wait(bar_t_full + 8 * a, (uint32_t)((ti >> ilog2(NACC)) & 1));
+        tc_fence_after();
+        const float sc = (float)p.i8scale[c] * p.beam_scale;
+        const int t = 2 * (32 * (4 * sp + quad) + lane);
+        __half2 *yrow = reinterpret_cast<__half2 *>(p.beams) + (size_t)c * nbeam * p.nsamp + t;
+#pragma unroll
+        for (int ch = 0; ch < NCH; ++ch) {
+          uint32_t v[32], u[32];
+          BF_TMEM_LD_32x32b_X32(t_lane + a * 2 * NCOL + 32 * ch, v);
+          BF_TMEM_LD_32x32b_X32(t_lane + a * 2 * NCOL + NCOL + 32 * ch, u);
+          tc_wait_ld();
+          if (ch == NCH - 1) {
+            tc_fence_before();
+            __syncwarp();
+            if (lane0) mbar_arrive(bar_t_empty + 8 * a);
+          }
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int re = ((int)v[4 * i] << 7) + (int)v[4 * i + 2];
+            const int im = ((int)v[4 * i + 1] << 7) + (int)v[4 * i + 3];
+            const int ro = ((int)u[4 * i] << 7) + (int)u[4 * i + 2];
+            const int io = ((int)u[4 * i + 1] << 7) + (int)u[4 * i + 3];
+            const __half2 ye = __floats2half2_rn((float)re * sc, (float)im * sc);
+            const __half2 yo = __floats2half2_rn((float)ro * sc, (float)io * sc);
+            if (8 * ch + i < nbeam && t < p.nsamp)
+              *reinterpret_cast<uint2 *>(yrow + (size_t)(8 * ch + i) * p.nsamp) =
+                  make_uint2(*reinterpret_cast<const uint32_t *>(&ye), *reinterpret_cast<const uint32_t *>(&yo));
+          }
+        }
+        ++ti;
+      } else if ((s & 1) == set) {
         float acc[NCH][8], acc1[LBIN == 0 ? NCH : 1][8];   // acc1: the odd sample's own bin when nint = 1
 #pragma unroll
         for (int ch = 0; ch < NCH; ++ch)
@@ -508,18 +542,18 @@ cudaError_t make_tmap_wide(CUtensorMap *tm, const BfParams &p, int box_rows) {
   return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-template <int NCOL, int LBIN>
+template <int NCOL, int LBIN, bool BEAMS = false>
 cudaError_t launch_i8w(const BfParams &p, int sm_count, cudaStream_t st) {
   constexpr int NST = 12;
   CUtensorMap tm, tm32;
   cudaError_t e = make_tmap_wide(&tm, p, 128);
   if (e == cudaSuccess) e = make_tmap_wide(&tm32, p, 32);
   if (e != cudaSuccess) return e;
-  const int G = p.nint <= 64 ? 1 : p.nint / 64;
+  const int G = BEAMS || p.nint <= 64 ? 1 : p.nint / 64;
   const int n_super_chan = (p.nsamp + 256 * G - 1) / (256 * G);
   const long long total = (long long)p.nchan_run * n_super_chan;
   const size_t smem = 1024 + 2 * NCOL * L_ROW_BYTES + NST * W_STAGE_BYTES + 1024;
-  auto kern = bf_umma_i8w_kernel<NCOL, LBIN, NST>;
+  auto kern = bf_umma_i8w_kernel<NCOL, LBIN, NST, BEAMS>;
   e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   const int grid = (int)(total < sm_count ? total : sm_count);
@@ -576,13 +610,19 @@ cudaError_t launch_i8_nint(const BfParams &p, int sm_count, cudaStream_t st) {
 
 // which shapes the int8 kernel takes: complex int8, nant a multiple of 8 up to 32 (rows of <= 64 bytes that
 // TMA can address), up to BF_I8_MAX_BEAMS beams, nint a power of two <= 32 or a multiple of 32
-bool bf_umma_i8_supported(const bf_ctx *c) {
+bool bf_umma_i8_supported(const bf_ctx *c, int mode) {
   if (c->dtype != BF_CI8 || c->nant % 8 != 0 || c->nant > 32 || c->nbeam > BF_I8_MAX_BEAMS) return false;
+  if (mode == BF_MODE_BEAMS) return c->nant == 32 && c->nsamp % 2 == 0;   // the WIDE variant only
   const int I = c->nint;
   return (I <= 32 && (I & (I - 1)) == 0) || I % 32 == 0;
 }
 
 cudaError_t bf_launch_umma_i8(const BfParams &p, int sm_count, cudaStream_t st) {
+  if (p.mode == BF_MODE_BEAMS) {
+    if (p.nbeam <= 8) return launch_i8w<32, 0, true>(p, sm_count, st);
+    if (p.nbeam <= 16) return launch_i8w<64, 0, true>(p, sm_count, st);
+    return launch_i8w<128, 0, true>(p, sm_count, st);
+  }
   // 32 antennas, an even number of samples and nint 2^k <= 64 or a multiple of 64: rows of two samples
   const bool wide = p.nant == 32 && p.nsamp % 2 == 0 && ((p.nint <= 64 && (p.nint & (p.nint - 1)) == 0) || p.nint % 64 == 0);
   if (wide) {

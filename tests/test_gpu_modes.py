@@ -43,19 +43,23 @@ BEAM_CASES = [
     (64, 2, 16, 256, "cf16"),    # K-blocked kernel, fp16
     (5, 2, 3, 77, "ci8"),        # generic kernel only
     (32, 2, 16, 256, "ci4"),
+    (32, 3, 1, 2050, "ci8"),     # int8 kernel: one beam, several tiles, ragged tail of one sample pair
+    (32, 2, 32, 768, "ci8"),     # int8 kernel: 128 accumulator columns
 ]
 
 
 @pytest.mark.parametrize("nant,nchan,nbeam,nsamp,dtype", BEAM_CASES)
-@pytest.mark.parametrize("kernel", ["simt", "auto"])
+@pytest.mark.parametrize("kernel", ["simt", "auto", "f16"])
 def test_voltage_beams_match_oracle(bf, nant, nchan, nbeam, nsamp, dtype, kernel):
     import torch
     w = synthetic.make_case(nant, nchan, nbeam, nsamp, 1, dtype)
     v = w.make_voltages()
     ref = oracle.beams(w.ant_xyz, w.freqs, w.beam_dir, v)  # [C][B][T] complex128
     scale = 0.25 if dtype != "cf16" else 2.0
-    B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, 1, dtype=bf_dtype(bf, w),
-                      kernel=bf.BF_KERNEL_SIMT if kernel == "simt" else bf.BF_KERNEL_AUTO)
+    k = {"simt": bf.BF_KERNEL_SIMT, "auto": bf.BF_KERNEL_AUTO, "f16": bf.BF_KERNEL_UMMA_F16}[kernel]
+    if kernel == "f16" and (nant % 8 != 0 or (dtype == "ci4" and nant % 16 != 0)):
+        pytest.skip("no fp16 tensor-core variant for this shape")
+    B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, 1, dtype=bf_dtype(bf, w), kernel=k)
     B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
     y = torch.full((w.nchan, w.nbeam, w.nsamp, 2), float("nan"), dtype=torch.float16, device="cuda")
     B.run_beams(torch.from_numpy(v).cuda(), y, scale=scale)
