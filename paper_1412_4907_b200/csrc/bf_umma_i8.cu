@@ -513,6 +513,27 @@ PFN_encodeTiled get_encode() {
   return fn;
 }
 
+// The tensor maps depend only on (pointer, nant, nsamp, nchan, view): a streaming caller alternates between a few
+// buffers, so the last few encodings are kept (host-side cost only; launch-bound shapes like `tiny` notice).
+struct TmapKey { const void *ptr; int nant, nsamp, nchan, wide, rows; };
+struct TmapSlot { TmapKey k; CUtensorMap tm; bool used; };
+thread_local TmapSlot g_tmaps[8];
+thread_local int g_tmap_next = 0;
+
+template <typename F>
+cudaError_t cached_tmap(CUtensorMap *tm, const BfParams &p, int wide, int rows, F make) {
+  const TmapKey k = {p.volt, p.nant, p.nsamp, p.nchan_run, wide, rows};
+  for (TmapSlot &s : g_tmaps)
+    if (s.used && s.k.ptr == k.ptr && s.k.nant == k.nant && s.k.nsamp == k.nsamp && s.k.nchan == k.nchan &&
+        s.k.wide == k.wide && s.k.rows == k.rows) { *tm = s.tm; return cudaSuccess; }
+  cudaError_t e = make(tm, p, rows);
+  if (e != cudaSuccess) return e;
+  TmapSlot &s = g_tmaps[g_tmap_next];
+  g_tmap_next = (g_tmap_next + 1) % 8;
+  s.k = k; s.tm = *tm; s.used = true;
+  return cudaSuccess;
+}
+
 // 3-D view of the int8 voltages as bytes: {2 nant, nsamp, nchan}; box {64, 32, 1}, 64-byte swizzle; bytes past
 // 2 nant and samples past nsamp are zero-filled
 cudaError_t make_tmap(CUtensorMap *tm, const BfParams &p, int box_rows) {
@@ -546,16 +567,22 @@ template <int NCOL, int LBIN, bool BEAMS = false>
 cudaError_t launch_i8w(const BfParams &p, int sm_count, cudaStream_t st) {
   constexpr int NST = 12;
   CUtensorMap tm, tm32;
-  cudaError_t e = make_tmap_wide(&tm, p, 128);
-  if (e == cudaSuccess) e = make_tmap_wide(&tm32, p, 32);
+  cudaError_t e = cached_tmap(&tm, p, 1, 128, make_tmap_wide);
+  if (e == cudaSuccess) e = cached_tmap(&tm32, p, 1, 32, make_tmap_wide);
   if (e != cudaSuccess) return e;
   const int G = BEAMS || p.nint <= 64 ? 1 : p.nint / 64;
   const int n_super_chan = (p.nsamp + 256 * G - 1) / (256 * G);
   const long long total = (long long)p.nchan_run * n_super_chan;
   const size_t smem = 1024 + 2 * NCOL * L_ROW_BYTES + NST * W_STAGE_BYTES + 1024;
   auto kern = bf_umma_i8w_kernel<NCOL, LBIN, NST, BEAMS>;
-  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
+  static thread_local int attr_dev = -1;   // once per instantiation and device
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (attr_dev != dev) {
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_dev = dev;
+  }
   const int grid = (int)(total < sm_count ? total : sm_count);
   kern<<<grid, L_THREADS + 32, smem, st>>>(p, tm, tm32, total, n_super_chan, G);
   return cudaGetLastError();
@@ -578,8 +605,8 @@ template <int NCOL, int LBIN>
 cudaError_t launch_i8(const BfParams &p, int sm_count, cudaStream_t st) {
   constexpr int NST = 24;
   CUtensorMap tm, tm32;
-  cudaError_t e = make_tmap(&tm, p, L_TILE_T);
-  if (e == cudaSuccess) e = make_tmap(&tm32, p, L_BOX_ROWS);
+  cudaError_t e = cached_tmap(&tm, p, 0, L_TILE_T, make_tmap);
+  if (e == cudaSuccess) e = cached_tmap(&tm32, p, 0, L_BOX_ROWS, make_tmap);
   if (e != cudaSuccess) return e;
   const int G = p.nint <= 32 ? 1 : p.nint / 32;
   const int n_super_chan = (p.nsamp + L_TILE_T * G - 1) / (L_TILE_T * G);
