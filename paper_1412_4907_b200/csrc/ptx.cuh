@@ -82,7 +82,7 @@ BF_DEVI void mbar_wait(uint32_t bar, uint32_t parity) {
   for (;;) {
 #pragma unroll 1
     for (int k = 0; k < 4096; ++k)
-      if (mbar_try_wait_hint(bar, parity, 20000u)) return;
+      if (mbar_try_wait(bar, parity)) return;
     if (clock64() - t0 > 4000000000LL) asm volatile("trap;");
   }
 }

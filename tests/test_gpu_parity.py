@@ -163,6 +163,13 @@ I8_SHAPES = [
     (8, 2, 4, 128, 16),        # rows of 16 bytes: one K step, zero-filled to 32
     (16, 2, 9, 300, 4),
     (24, 2, 5, 256, 8),        # rows of 48 bytes
+    (32, 1, 1, 2, 1),          # degenerate: one row of two samples
+    (32, 1, 1, 2, 2),
+    (32, 3, 2, 64, 64),        # one bin per channel, a quarter of a tile
+    (32, 1, 3, 130, 1),        # 65 rows: a full warp quadrant plus one row
+    (32, 1, 4, 131, 1),        # odd nsamp: narrow variant
+    (8, 1, 1, 1, 1),           # one sample
+    (32, 2, 8, 66048, 32),     # 258 tiles per channel: super-tile ranges that straddle channels
 ]
 
 
