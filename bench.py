@@ -198,6 +198,8 @@ def main():
     ap.add_argument("--mode", default="power", choices=["power", "beams", "incoherent"],
                     help="power = the headline path (bf_run); beams / incoherent = SURVEY 8(f) row f4 side modes")
     ap.add_argument("--nbeam", type=int, default=0, help="override the workload's beam count (beams mode: default 8)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = one full replica per rank (default); strong = ONE workload, channels sharded over the ranks")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--chan-per-chunk", type=int, default=0, help="e2e: channels per H2D chunk (0 = nchan/8)")
@@ -232,7 +234,12 @@ def main():
     if args.mode != "power":
         args.no_e2e = True
         args.no_cpu_baseline = True
-    w.seed = rank_seed(w.seed, rank)
+    if args.scaling == "strong" and world > 1:
+        from paper_1412_4907_b200 import shard
+        c0, c1 = shard.channel_range(w.nchan, world, rank)   # channels are independent: no exchange
+        w = w.sub(chan_idx=list(range(c0, c1)))
+    else:
+        w.seed = rank_seed(w.seed, rank)
     peaks = load_peaks()
     kern = {"auto": bf.BF_KERNEL_AUTO, "simt": bf.BF_KERNEL_SIMT, "umma": bf.BF_KERNEL_UMMA,
             "f16": bf.BF_KERNEL_UMMA_F16, "i8": bf.BF_KERNEL_UMMA_I8}[args.kernel]
@@ -369,12 +376,12 @@ def main():
     if rank == 0:
         line = {
             "metric": METRIC if args.mode == "power" else METRIC + " [side mode: %s]" % args.mode, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None,
             "dtype": "i8->i32 (dp4a)" if args.mode == "incoherent" else {"umma-i8": "i8xi8->i32", "simt": "f32"}.get(B.kernel_name, "f16xf16->f32"),
             "data": "synthetic",
             "config": {"workload": w.name if args.mode == "power" else w.name + ":" + args.mode, "nant": w.nant, "nchan": w.nchan, "nbeam": w.nbeam, "nsamp": w.nsamp,
                        "nint": w.nint, "input": w.dtype, "l2": "input buffer (%.0f MB) >> L2 (126 MB), no flush needed" % (w.in_bytes / 1e6),
-                       "kernel": B.kernel_name, "parallelism": f"replicas x{world}"},
+                       "kernel": B.kernel_name, "parallelism": (f"channel shards x{world}" if args.scaling == "strong" and world > 1 else f"replicas x{world}")},
             "ant_samples_per_s": world * w.nchan * w.nsamp * w.nant * K / (total_ms_max * 1e-3),
             "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
             "context": {"paper_k20_tflops": 1.3, "note": "paper's number is a Tesla K20 with 4-bit input (PAPER.md:15): context, not a baseline for this config"},

@@ -39,7 +39,16 @@ def _worker(rank, world, port, out):
     units = float(w.cmac) * 8
     dist.barrier()
     t_max, u_sum = bench.aggregate(local_ms, units, dist, torch.device("cpu"))
-    out[rank] = (t_max, u_sum, float(P.sum()), int(v.astype(np.int64).sum()))
+    # channel sharding of ONE workload (strong scaling): rank r holds channels [c0, c1) and the gather
+    # rebuilds the cube every rank would have computed alone
+    from paper_1412_4907_b200 import shard
+    wf = synthetic.make_workload("tiny").sub(nchan=5, nsamp=64)      # 5 channels over 2 ranks: 3 + 2
+    c0, c1 = shard.channel_range(wf.nchan, world, rank)
+    ws = wf.sub(chan_idx=list(range(c0, c1)))
+    Ps = oracle.beamform(ws.ant_xyz, ws.freqs, ws.beam_dir, wf.make_voltages()[c0:c1], ws.nint)
+    full = shard.gather_powers(torch.from_numpy(Ps), wf.nchan, dist).numpy()
+    ref = oracle.beamform(wf.ant_xyz, wf.freqs, wf.beam_dir, wf.make_voltages(), wf.nint)
+    out[rank] = (t_max, u_sum, float(P.sum()), int(v.astype(np.int64).sum()), (c0, c1), bool(np.array_equal(full, ref)))
     dist.destroy_process_group()
 
 
@@ -49,10 +58,26 @@ def test_two_ranks_aggregate_and_shard():
     out = mgr.dict()
     mp.spawn(_worker, args=(world, _free_port(), out), nprocs=world, join=True)
     assert set(out.keys()) == {0, 1}
-    (t0, u0, p0, s0), (t1, u1, p1, s1) = out[0], out[1]
+    (t0, u0, p0, s0, r0, ok0), (t1, u1, p1, s1, r1, ok1) = out[0], out[1]
+    assert r0 == (0, 3) and r1 == (3, 5) and ok0 and ok1   # channel shards tile the cube, gather is exact
     assert t0 == t1 == 15.0                       # max over ranks
     assert u0 == u1 and u0 == 2 * 8 * 2 * 16 * 32 * 64  # sum over ranks of 8*C*B*N*T
     assert s0 != s1 and p0 != p1                  # the replicas really beamformed different buffers
+
+
+def test_channel_range_properties():
+    from paper_1412_4907_b200 import shard
+    for nchan in (0, 1, 5, 64, 1023):
+        for world in (1, 2, 3, 8):
+            r = [shard.channel_range(nchan, world, k) for k in range(world)]
+            assert r[0][0] == 0 and r[-1][1] == nchan
+            assert all(r[k][1] == r[k + 1][0] for k in range(world - 1))
+            sizes = [b - a for a, b in r]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        shard.channel_range(4, 2, 2)
+    t = torch.arange(24.0).reshape(2, 3, 4)
+    assert shard.gather_powers(t, 2) is t
 
 
 def test_single_process_aggregate_is_identity():
