@@ -227,6 +227,9 @@ def main():
 
     W = max(3, args.warmup)
     K = max(1, args.steps)
+    if args.config.startswith("sweep") and args.nbeam:
+        # the sweep's beam rule (A3) for any beam count, named sweep-B<n>
+        args.config, args.nbeam = f"sweep-{args.nbeam}", 0
     w = workload_for(args.config)
     if args.mode == "beams" or args.nbeam:
         # the S-engine ships "8 beams from the generated 128-beam grid ... as 16-bit complex-valued words"
