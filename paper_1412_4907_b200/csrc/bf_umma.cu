@@ -92,9 +92,12 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     else is_tma = true;                                                // 31
   }
 
+  // full rows (nant = 32): the convert warps work as two groups of four on alternate tiles (see the convert role)
+  const bool split = p.nant == 32;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < NSTAGE; ++s) { mbar_init(bar_b_full + 8 * s, CONV_WARPS); mbar_init(bar_b_empty + 8 * s, 2); }
-    for (int s = 0; s < NRAW; ++s) { mbar_init(bar_r_full + 8 * s, 1); mbar_init(bar_r_empty + 8 * s, CONV_WARPS); }
+    const int nconv = split ? CONV_WARPS / 2 : CONV_WARPS;   // warps that convert one tile
+    for (int s = 0; s < NSTAGE; ++s) { mbar_init(bar_b_full + 8 * s, nconv); mbar_init(bar_b_empty + 8 * s, 2); }
+    for (int s = 0; s < NRAW; ++s) { mbar_init(bar_r_full + 8 * s, 1); mbar_init(bar_r_empty + 8 * s, nconv); }
     for (int s = 0; s < 2; ++s) {
       mbar_init(bar_a_full + 8 * s, 1); mbar_init(bar_a_empty + 8 * s, 2);
       mbar_init(bar_t_full + 8 * s, 1);          mbar_init(bar_t_empty + 8 * s, EPI_WARPS);
@@ -227,23 +230,32 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     }
     int rs = 0, st = 0;              // raw slot / operand stage of the current item
     uint32_t rpar = 0, bpar = 1;     // parities to wait for on r_full[rs] / b_empty[st]
-    if (npieces == PIECES * CONV_THREADS) {
-      // ---- full rows (nant = 32): every thread owns PIECES pieces, piece k sits KSTEP bytes after
-      // piece 0 in the operand stage and 16 * CONV_THREADS bytes after it in the raw slot, so all
-      // shared-memory accesses are [register + immediate]
-      constexpr int FULL_NPR = IN == BF_CI4 ? 2 : 4;
-      constexpr uint32_t KSTEP = (CONV_THREADS / FULL_NPR / 8) * 1024;
-      uint32_t raw = sR + 16 * ctid, dst = sB + p_dst[0];
-      for (int i = 0; i < n_items; ++i) {
-        mbar_wait(bar_r_full + 8 * rs, rpar);
-        uint4 x[PIECES];
+    if (split) {
+      // ---- full rows (nant = 32), two groups of four warps on alternate tiles.  A tile's conversion is a chain of
+      // dependent latencies (barrier, LDS, barrier, STS, proxy fence, arrive) that one warp walks once per tile; with
+      // all eight warps on the same tile that chain, not the ring depth, set the rate.  Two tiles are now in
+      // conversion at any time.  Thread gtid of a group owns pieces gtid + 128 k: row (gtid + 128 k) / NPR, so piece
+      // k sits KSTEP bytes after piece 0 in the operand stage and 16 * GT bytes after it in the raw slot: all
+      // shared-memory accesses are [register + immediate].
+      constexpr int NPR = IN == BF_CI4 ? 2 : 4;                          // 16-byte pieces per time sample
+      constexpr int GT = CONV_THREADS / 2, GP = TILE_T * NPR / GT;       // threads per group, pieces per thread
+      constexpr uint32_t KSTEP = (GT / NPR / 8) * 1024;
+      const int grp = cw >> 2, gtid = ctid & (GT - 1);
+      const int t0 = gtid / NPR, q0 = gtid % NPR;
+      const uint32_t raw0 = sR + 16 * gtid;
+      const uint32_t dst0 = sB + (uint32_t)((t0 >> 3) * 1024 + (t0 & 7) * 128 + (((CPP * q0) ^ (t0 & 7)) << 4));
+      for (int i = grp; i < n_items; i += 2) {
+        const int rs = i % NRAW, st = i % NSTAGE;
+        const uint32_t raw = raw0 + rs * RAW_STAGE_BYTES, dst = dst0 + st * B_STAGE_BYTES;
+        mbar_wait(bar_r_full + 8 * rs, (uint32_t)((i / NRAW) & 1));
+        uint4 x[GP];
 #pragma unroll
-        for (int k = 0; k < PIECES; ++k) x[k] = ld_shared_v4(raw + k * (16 * CONV_THREADS));
-        mbar_wait(bar_b_empty + 8 * st, bpar);
+        for (int k = 0; k < GP; ++k) x[k] = ld_shared_v4(raw + k * (16 * GT));
+        mbar_wait(bar_b_empty + 8 * st, (uint32_t)(((i / NSTAGE) & 1) ^ 1));
         if (IN == BF_CI4) {
           const uint32_t d1 = dst ^ 16u, d2 = dst ^ 32u, d3 = dst ^ 48u;
 #pragma unroll
-          for (int k = 0; k < PIECES; ++k) {
+          for (int k = 0; k < GP; ++k) {
             uint32_t h[4];
             cvt_i4x8_f16x8(x[k].x, h); st_shared_v4(dst + k * KSTEP, h[0], h[1], h[2], h[3]);
             cvt_i4x8_f16x8(x[k].y, h); st_shared_v4(d1 + k * KSTEP, h[0], h[1], h[2], h[3]);
@@ -253,7 +265,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         } else {
           const uint32_t d1 = dst ^ 16u;
 #pragma unroll
-          for (int k = 0; k < PIECES; ++k) {
+          for (int k = 0; k < GP; ++k) {
             uint32_t h[8];
             cvt_i8x4_f16x4(x[k].x, h[0], h[1]);
             cvt_i8x4_f16x4(x[k].y, h[2], h[3]);
@@ -269,9 +281,6 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
           mbar_arrive(bar_r_empty + 8 * rs);  // raw bytes are converted: slot may be refilled
           mbar_arrive(bar_b_full + 8 * st);
         }
-        raw += RAW_STAGE_BYTES; dst += B_STAGE_BYTES;
-        if (++rs == NRAW) { rs = 0; rpar ^= 1; raw -= NRAW * RAW_STAGE_BYTES; }
-        if (++st == NSTAGE) { st = 0; bpar ^= 1; dst -= NSTAGE * B_STAGE_BYTES; }
       }
     } else {
       // ---- short rows (nant < 32): generic piece table
