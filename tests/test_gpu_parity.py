@@ -119,6 +119,8 @@ SMALL = [
     (32, 1, 130, 512, 64, "ci4"),
     (16, 2, 5, 256, 1, "ci4"),       # K' = 32: half a K-block
     (24, 2, 7, 128, 16, "ci4"),      # rows of 24 bytes: generic kernel only
+    (32, 40, 64, 5000, 8, "ci8"),    # 800 items: 5-6 per CTA, both convert groups busy, ragged tail (5000 = 19*256 + 136)
+    (32, 30, 100, 3000, 4, "ci4"),   # same for the 4-bit unpack, two M-tiles per item
 ]
 
 
