@@ -6,8 +6,16 @@
 One "step" is one pass of the whole hot path (ingest -> contraction -> |.|^2 -> integrate) over one
 synthetic `medium` buffer (BASELINE.json configs[1]: 32 antennas, 1024 channels, 128 beams, 32768
 samples, complex int8, nint 64).  Prints ONE JSON line (rank 0).  Metric: beamforming TFLOP/s at
-8 flop per complex MAC.  N > 1 runs one replica per GPU on its own buffer (channels
-are independent, so the path shards with no exchange; "weak" scaling) and reports the aggregate.
+8 flop per complex MAC.
+
+The default run (N = 1, --config medium) also times every other BASELINE.json configuration (tiny, the six
+beam-count sweep points, large-N, streaming) with the same procedure and reports them under "configs", and
+compares the GPU powers of ALL channels of the headline buffer with the oracle ("max_err").
+
+--gpus N > 1 without a torchrun environment starts N ranks itself (torch.distributed.run, one per GPU);
+each rank beamforms its own replica (channels are independent, so the path shards with no exchange; "weak"
+scaling), or with --scaling strong a contiguous range of ONE workload's channels; NCCL is used only for the
+barrier and the two timing all-reduces.
 
 --impl reference times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
 """
@@ -15,10 +23,13 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
+import socket
 import statistics
 import subprocess
 import sys
+import threading
 import time
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
@@ -26,6 +37,8 @@ sys.path.insert(0, ROOT)
 
 METRIC = "beamforming TFLOP/s (8 flop/complex MAC)"
 UNIT = "TFLOP/s"
+L2_BYTES = 126e6
+ALL_CONFIGS = ["tiny", "sweep-1", "sweep-4", "sweep-16", "sweep-64", "sweep-256", "sweep-1024", "large-N", "streaming"]
 
 
 def load_peaks():
@@ -71,58 +84,143 @@ def aggregate(total_ms_local: float, units_local: float, dist_mod=None, device=N
     return float(t.item()), float(u.item())
 
 
-class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+# ------------------------------------------------------------------------------------------ multi-rank launcher
+def free_port() -> int:
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    return port
 
-    def __init__(self, index=0):
-        self.proc = None
-        self.index = index
+
+def launcher_command(ngpus: int, argv, port=None):
+    """The torchrun command `bench.py --gpus N` re-executes itself under when no rank environment is set."""
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={ngpus}",
+            "--master-addr", "127.0.0.1", "--master-port", str(port or free_port()), os.path.abspath(__file__)] + list(argv)
+
+
+def maybe_spawn(args, argv):
+    """--gpus N > 1 and no WORLD_SIZE: start the N ranks here and pass their output through."""
+    if args.gpus <= 1 or "WORLD_SIZE" in os.environ:
+        return None
+    return subprocess.call(launcher_command(args.gpus, argv))
+
+
+def launcher_selftest(args) -> int:
+    """CPU check of the multi-rank plumbing (tests/test_multirank_cpu.py): every rank joins a gloo group,
+    'processes' (rank + 1) units in (rank + 1) ms, and rank 0 prints the aggregate -- the code path of the real
+    bench (environment, barrier, MAX / SUM all-reduces, one JSON line) without a GPU."""
+    import torch.distributed as td
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        td.init_process_group("gloo")
+        td.barrier()
+    ms, units = aggregate(float(rank + 1), float(rank + 1), td if world > 1 else None, "cpu")
+    if rank == 0:
+        print(json.dumps({"selftest": "launcher", "n_gpus": world, "requested_gpus": args.gpus, "max_ms": ms, "units": units,
+                          "value": units / ms}))
+    if world > 1:
+        td.destroy_process_group()
+    return 0
+
+
+# ------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """SM clock, power and throttle reasons sampled DURING the timed region: NVML in a thread of this
+    process (one sample every ~1 ms), nvidia-smi as the fallback."""
+    REASONS = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
+
+    def __init__(self, index=0, period_s=0.001):
+        self.index, self.period = index, period_s
+        self.samples, self.reasons, self.power = [], set(), []
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thread = None
+        self._smi = None
+        self.source = None
+
+    def _loop(self, nv, h):
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for nm, bit in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(self.period)
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-i", str(self.index), "-lms", "20"], stdout=subprocess.PIPE,
-                                         stderr=subprocess.DEVNULL, text=True)
+            import pynvml as nv
+            nv.nvmlInit()
+            idx = self.index
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            if vis:
+                try:
+                    idx = int(vis.split(",")[self.index])
+                except Exception:
+                    pass
+            h = nv.nvmlDeviceGetHandleByIndex(idx)
+            self.max_mhz = float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            self._thread = threading.Thread(target=self._loop, args=(nv, h), daemon=True)
+            self._thread.start()
+            self.source = "nvml"
+            return
         except Exception:
-            self.proc = None
+            self._thread = None
+        try:
+            q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+                 "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+            self._smi = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i", str(self.index),
+                                          "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.source = "nvidia-smi"
+        except Exception:
+            self._smi = None
 
     def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        if self.proc is None:
-            return out
-        time.sleep(0.05)
-        self.proc.terminate()
-        try:
-            text, _ = self.proc.communicate(timeout=5)
-        except Exception:
-            self.proc.kill()
-            text = ""
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ln in text.splitlines():
-            f = [x.strip() for x in ln.split(",")]
-            if len(f) < 7:
-                continue
+        out = {"sm_mhz": None, "sm_min_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0, "power_w_max": None,
+               "source": self.source}
+        if self._thread is not None:
+            self._stop.set()
+            self._thread.join(timeout=2)
+        elif self._smi is not None:
+            time.sleep(0.05)
+            self._smi.terminate()
             try:
-                sm.append(float(f[0])); mx.append(float(f[1]))
-            except ValueError:
-                continue
-            for nm, val in zip(names, f[3:7]):
-                if val.lower().startswith("active"):
-                    reasons.add(nm)
-        if sm:
-            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), samples=len(sm))
-        out["reasons"] = sorted(reasons)
+                text, _ = self._smi.communicate(timeout=5)
+            except Exception:
+                self._smi.kill()
+                text = ""
+            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+            for ln in text.splitlines():
+                f = [x.strip() for x in ln.split(",")]
+                if len(f) < 7:
+                    continue
+                try:
+                    self.samples.append(float(f[0]))
+                    self.max_mhz = float(f[1])
+                    self.power.append(float(f[2]))
+                except ValueError:
+                    continue
+                for nm, val in zip(names, f[3:7]):
+                    if val.lower().startswith("active"):
+                        self.reasons.add(nm)
+            out["sm_max_mhz"] = self.max_mhz
+        if self.samples:
+            out.update(sm_mhz=statistics.median(self.samples), sm_min_mhz=min(self.samples), samples=len(self.samples))
+        if self.power:
+            out["power_w_max"] = max(self.power)
+        out["reasons"] = sorted(self.reasons)
         return out
 
 
+# ------------------------------------------------------------------------------------------ oracle legs
 def time_oracle_sample(w, v_host_fn, target_s=15.0, max_chan=1 << 30):
     """The oracle as it stands on the host cores, on whole channels of the workload; returns
-    (TFLOP/s, cores, description).  v_host_fn(chan_list) -> numpy voltages of those channels."""
-    import numpy as np
+    (TFLOP/s, cores, description, seconds, channels, powers of those channels).  v_host_fn(chan_list) -> numpy voltages."""
     import oracle
     cores = oracle.num_threads()
     # calibrate on `cores` channels (one per thread), then size the sample for ~target_s
@@ -131,7 +229,7 @@ def time_oracle_sample(w, v_host_fn, target_s=15.0, max_chan=1 << 30):
     ws = w.sub(chan_idx=chans)
     v = v_host_fn(chans)
     t0 = time.perf_counter()
-    oracle.beamform(ws.ant_xyz, ws.freqs, ws.beam_dir, v, ws.nint)
+    ref = oracle.beamform(ws.ant_xyz, ws.freqs, ws.beam_dir, v, ws.nint)
     dt0 = time.perf_counter() - t0
     per_chan = dt0 / n0
     n = int(max(n0, min(max_chan, w.nchan, target_s / max(per_chan, 1e-9))))
@@ -142,12 +240,20 @@ def time_oracle_sample(w, v_host_fn, target_s=15.0, max_chan=1 << 30):
         ws = w.sub(chan_idx=chans)
         v = v_host_fn(chans)
         t0 = time.perf_counter()
-        oracle.beamform(ws.ant_xyz, ws.freqs, ws.beam_dir, v, ws.nint)
+        ref = oracle.beamform(ws.ant_xyz, ws.freqs, ws.beam_dir, v, ws.nint)
         dt = time.perf_counter() - t0
     else:
         n, dt = n0, dt0
     flop = 8.0 * n * w.nbeam * w.nant * w.nsamp
-    return flop / dt / 1e12, cores, f"{n} of {w.nchan} channels x all {w.nbeam} beams x all {w.nsamp} samples, {dt:.2f} s", dt, n
+    return flop / dt / 1e12, cores, f"{n} of {w.nchan} channels x all {w.nbeam} beams x all {w.nsamp} samples, {dt:.2f} s", dt, n, ref
+
+
+def row_error(P_gpu, P_ref):
+    """north_star's bar: worst over (chan, beam) rows of max_j |P_gpu - P_ref| / mean_j P_ref."""
+    import numpy as np
+    P_gpu = np.asarray(P_gpu, dtype=np.float64)
+    err = np.abs(P_gpu - P_ref).max(axis=-1)
+    return float((err / np.maximum(P_ref.mean(axis=-1), 1e-300)).max())
 
 
 def run_reference(args):
@@ -155,7 +261,6 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    import numpy as np
     import oracle
     w = workload_for(args.config)
     cores = oracle.num_threads()
@@ -187,6 +292,118 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------ one configuration on the device
+class Timed:
+    """One workload resident on the device, timed with CUDA events on the launching stream."""
+
+    def __init__(self, bf, synthetic, torch, w, dev, kernel, mode="power"):
+        self.bf, self.torch, self.w, self.dev, self.mode = bf, torch, w, dev, mode
+        dt = {"ci8": bf.BF_CI8, "cf16": bf.BF_CF16, "ci4": bf.BF_CI4}[w.dtype]
+        self.B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint, dtype=dt, kernel=kernel, device=dev)
+        self.B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
+        v = synthetic.fill_voltages_torch(w, dev)
+        # inputs smaller than twice the L2 are rotated through enough copies that no launch finds its input cached
+        self.ncopy = 1 if w.in_bytes >= 2 * L2_BYTES else int(math.ceil(2 * L2_BYTES / w.in_bytes)) + 1
+        self.v = [v] + [v.clone() for _ in range(self.ncopy - 1)]
+        self.l2 = ("input buffer (%.0f MB) > 2 x L2 (126 MB): no flush needed" % (w.in_bytes / 1e6) if self.ncopy == 1 else
+                   "input (%.1f MB) fits L2: %d copies rotated (%.0f MB > 2 x L2) so every launch reads HBM" %
+                   (w.in_bytes / 1e6, self.ncopy, self.ncopy * w.in_bytes / 1e6))
+        self.P = self.B.empty_powers()
+        self.stream = torch.cuda.current_stream(dev)
+        self.probe = torch.zeros(4, dtype=torch.int64, device=dev)
+        self.B.set_clock_probe(self.probe)
+        self.k = 0
+        if mode == "beams":
+            self.Y = torch.empty((w.nchan, w.nbeam, w.nsamp, 2), dtype=torch.float16, device=dev)
+        elif mode == "incoherent":
+            self.Pi = torch.empty((w.nchan, w.nbin), dtype=torch.float32, device=dev)
+
+    def step(self):
+        v = self.v[self.k % self.ncopy]
+        self.k += 1
+        if self.mode == "beams":
+            self.B.run_beams(v, self.Y, 0.25, self.stream)
+        elif self.mode == "incoherent":
+            self.B.run_incoherent(v, self.Pi, self.stream)
+        else:
+            self.B.run(v, self.P, self.stream)
+
+    def flop_step(self):
+        w = self.w
+        return 8.0 * w.cmac if self.mode != "incoherent" else 4.0 * w.nchan * w.nsamp * w.nant  # |x|^2 + add
+
+    def abytes(self):
+        w = self.w
+        if self.mode == "beams":
+            return w.in_bytes + w.nchan * w.nbeam * w.nant * 4 + w.nchan * w.nbeam * w.nsamp * 4  # fp16 complex out
+        if self.mode == "incoherent":
+            return w.in_bytes + w.nchan * w.nbin * 4
+        return algorithmic_bytes(w)
+
+    def measure(self, K, W, barrier, sample_clocks=True, rank=0):
+        torch = self.torch
+        for _ in range(W):
+            self.step()
+        barrier()
+        sampler = ClockSampler(self.dev.index or 0)
+        if sample_clocks and rank == 0:
+            sampler.start()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
+        l0 = self.B.launches
+        barrier()
+        ev[0].record(self.stream)
+        for k in range(K):
+            self.step()
+            ev[k + 1].record(self.stream)
+        barrier()
+        launches = self.B.launches - l0
+        clocks = sampler.stop() if (sample_clocks and rank == 0) else None
+        total_ms = ev[0].elapsed_time(ev[K])
+        per = [ev[k].elapsed_time(ev[k + 1]) for k in range(K)]
+        pr = [int(x) for x in self.probe.cpu().tolist()]
+        if clocks is not None and pr[3] > pr[1]:
+            # the SM clock the LAST timed launch really ran at, from the kernel's own counters (bf_set_clock_probe)
+            clocks["kernel_sm_mhz"] = (pr[2] - pr[0]) / (pr[3] - pr[1]) * 1e3
+            clocks["kernel_cta0_ms"] = (pr[3] - pr[1]) * 1e-6
+        return total_ms, per, launches, clocks
+
+    def roofline(self, kernel_ms, total_ms, clocks, peaks, traffic):
+        """Roofline of the dominant (only) kernel: a dense contraction -> tensor bound; HBM-bound when the
+        algorithmic bytes at measured bandwidth take longer than the flops at the measured tensor peak."""
+        flop, ab = self.flop_step(), self.abytes()
+        t_hbm = ab / (peaks["hbm_gbs"] * 1e9)
+        # which measured GEMM figure is the tensor roofline: the BURST one for a kernel timed alone in a short region with no
+        # power cap seen, the SUSTAINED one once the region is long or the cap was active (both fractions are printed)
+        capped = bool(clocks) and "sw_power_cap" in (clocks.get("reasons") or [])
+        sustained = capped or total_ms >= 1000.0
+        tpeak = peaks["tensor_tflops"] if sustained else peaks["tensor_tflops_burst"]
+        tkind = ("sustained (power cap seen or timed region >= 1 s)" if sustained
+                 else f"burst (timed region {total_ms:.0f} ms, no power cap seen)")
+        t_tensor = flop / (peaks["tensor_tflops_burst"] * 1e12)
+        if t_tensor >= t_hbm:
+            ach = flop / (kernel_ms * 1e-3) / 1e12
+            return {"bound": "tensor", "achieved": ach, "peak": tpeak, "unit": "TFLOP/s", "frac": ach / tpeak, "traffic": traffic,
+                    "peak_kind": peaks["source"] + " bf16/fp16 dense GEMM, " + tkind,
+                    "frac_of_burst": ach / peaks["tensor_tflops_burst"], "frac_of_sustained": ach / peaks["tensor_tflops"],
+                    "kernel_ms": kernel_ms, "algorithmic_flop": flop, "algorithmic_bytes": ab}
+        ach = ab / (kernel_ms * 1e-3) / 1e9
+        return {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
+                "traffic": traffic, "peak_kind": peaks["source"] + " copy bandwidth", "kernel_ms": kernel_ms,
+                "algorithmic_flop": flop, "algorithmic_bytes": ab}
+
+    def close(self):
+        self.B.close()
+        self.v = None
+
+
+def load_traffic(name):
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(tpath)).get(name)
+    except Exception:
+        return None
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -202,12 +419,19 @@ def main():
                     help="N > 1: weak = one full replica per rank (default); strong = ONE workload, channels sharded over the ranks")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the table of the other BASELINE.json configurations")
     ap.add_argument("--chan-per-chunk", type=int, default=0, help="e2e: channels per H2D chunk (0 = nchan/8)")
+    ap.add_argument("--selftest-launcher", action="store_true", help="CPU check of the --gpus N launcher (no GPU work)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    rc = maybe_spawn(args, sys.argv[1:])
+    if rc is not None:
+        return rc
+    if args.selftest_launcher:
+        return launcher_selftest(args)
 
-    import numpy as np
+    import numpy as np  # noqa: F401
     import torch
     import synthetic
     import paper_1412_4907_b200 as bf
@@ -219,8 +443,11 @@ def main():
     dist = world > 1
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    if local >= torch.cuda.device_count():
+        raise SystemExit(f"rank {rank}: local rank {local} has no GPU ({torch.cuda.device_count()} visible)")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+    td = None
     if dist:
         import torch.distributed as td
         td.init_process_group("nccl", device_id=dev)
@@ -246,86 +473,24 @@ def main():
     peaks = load_peaks()
     kern = {"auto": bf.BF_KERNEL_AUTO, "simt": bf.BF_KERNEL_SIMT, "umma": bf.BF_KERNEL_UMMA,
             "f16": bf.BF_KERNEL_UMMA_F16, "i8": bf.BF_KERNEL_UMMA_I8}[args.kernel]
-    dt = {"ci8": bf.BF_CI8, "cf16": bf.BF_CF16, "ci4": bf.BF_CI4}[w.dtype]
-
-    B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint, dtype=dt, kernel=kern, device=dev)
-    B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
-    v = synthetic.fill_voltages_torch(w, dev)
-    P = B.empty_powers()
-    stream = torch.cuda.current_stream(dev)
-    run_step = lambda: B.run(v, P, stream)
-    if args.mode == "beams":
-        Y = torch.empty((w.nchan, w.nbeam, w.nsamp, 2), dtype=torch.float16, device=dev)
-        run_step = lambda: B.run_beams(v, Y, 0.25, stream)
-    elif args.mode == "incoherent":
-        Pi = torch.empty((w.nchan, w.nbin), dtype=torch.float32, device=dev)
-        run_step = lambda: B.run_incoherent(v, Pi, stream)
 
     def barrier():
         if dist:
             td.barrier()
         torch.cuda.synchronize(dev)
 
-    # ---------------------------------------------------------------- device-resident timing
-    for _ in range(W):
-        run_step()
-    barrier()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
-    l0 = B.launches
-    barrier()
-    ev[0].record(stream)
-    for k in range(K):
-        run_step()
-        ev[k + 1].record(stream)
-    barrier()
-    launches = B.launches - l0
-    clocks = sampler.stop() if rank == 0 else None
-    total_ms = ev[0].elapsed_time(ev[K])
-    per_launch_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(K)]
-    flop_step = 8.0 * w.cmac if args.mode != "incoherent" else 4.0 * w.nchan * w.nsamp * w.nant  # |x|^2 + add
-    total_ms_max, flop_all = aggregate(total_ms, flop_step * K, td if dist else None, dev)
+    # ---------------------------------------------------------------- device-resident timing (headline)
+    T = Timed(bf, synthetic, torch, w, dev, kern, args.mode)
+    B = T.B
+    total_ms, per_launch_ms, launches, clocks = T.measure(K, W, barrier, rank=rank)
+    flop_step = T.flop_step()
+    total_ms_max, flop_all = aggregate(total_ms, flop_step * K, td, dev)
     value = flop_all / (total_ms_max * 1e-3) / 1e12
     ms_per_step = total_ms_max / K
     avg_kernel_ms = statistics.mean(per_launch_ms)
-
-    # roofline of the dominant (only) kernel: a dense contraction -> tensor bound; HBM-bound when
-    # the algorithmic bytes at measured bandwidth take longer than the flops at measured tensor peak
-    abytes = algorithmic_bytes(w)
-    if args.mode == "beams":
-        abytes = w.in_bytes + w.nchan * w.nbeam * w.nant * 4 + w.nchan * w.nbeam * w.nsamp * 4  # fp16 complex out
-    elif args.mode == "incoherent":
-        abytes = w.in_bytes + w.nchan * w.nbin * 4
-    t_hbm = abytes / (peaks["hbm_gbs"] * 1e9)
-    # which measured GEMM figure is the tensor roofline: the BURST one for a kernel timed alone in a short region at
-    # full clocks, the SUSTAINED one once the timed region is long or the power cap was seen during it (the
-    # cuBLAS loop behind the sustained figure runs power-capped at ~1.3 GHz; this kernel settles at ~1.4 GHz)
-    capped = bool(clocks) and "sw_power_cap" in (clocks.get("reasons") or [])
-    sustained = capped or total_ms >= 1000.0
-    tpeak = peaks["tensor_tflops"] if sustained else peaks["tensor_tflops_burst"]
-    tkind = ("sustained (power cap seen or timed region >= 1 s)" if sustained
-             else f"burst (timed region {total_ms:.0f} ms at full clocks, no power cap seen)")
-    t_tensor = flop_step / (tpeak * 1e12)
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath) and args.mode == "power":
-        try:
-            traffic = json.load(open(tpath)).get(w.name)
-        except Exception:
-            traffic = None
-    if t_tensor >= t_hbm:
-        ach = flop_step / (avg_kernel_ms * 1e-3) / 1e12
-        roof = {"bound": "tensor", "achieved": ach, "peak": tpeak, "unit": "TFLOP/s",
-                "frac": ach / tpeak, "traffic": traffic, "peak_kind": peaks["source"] + " bf16/fp16 dense GEMM, " + tkind,
-                "frac_of_burst": ach / peaks["tensor_tflops_burst"], "frac_of_sustained": ach / peaks["tensor_tflops"],
-                "kernel_ms": avg_kernel_ms}
-    else:
-        ach = abytes / (avg_kernel_ms * 1e-3) / 1e9
-        roof = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": ach / peaks["hbm_gbs"], "traffic": traffic, "peak_kind": peaks["source"] + " copy bandwidth",
-                "kernel_ms": avg_kernel_ms}
+    roof = T.roofline(avg_kernel_ms, total_ms, clocks, peaks, load_traffic(w.name) if args.mode == "power" else None)
+    kernel_name, l2_note = B.kernel_name, T.l2
+    v, P = T.v[0], T.P
 
     # ---------------------------------------------------------------- end to end through the C ABI with HOST buffers
     e2e = None
@@ -335,6 +500,8 @@ def main():
         hp = torch.empty(P.shape, dtype=torch.float32, pin_memory=True)
         cpc = args.chan_per_chunk or max(1, w.nchan // 8)
         cs, xs = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+        P_dev = P.clone()   # the device-resident result, kept for the whole-buffer parity figure below
+        T.v = None
         del v
         torch.cuda.empty_cache()
         Ke = min(K, 10)
@@ -367,7 +534,7 @@ def main():
         barrier()
         Ke *= steps_per_call
         e2e_ms = e0.elapsed_time(e1)
-        e2e_ms, e2e_flop = aggregate(e2e_ms, flop_step * Ke, td if dist else None, dev)
+        e2e_ms, e2e_flop = aggregate(e2e_ms, flop_step * Ke, td, dev)
         e2e = {"value": e2e_flop / (e2e_ms * 1e-3) / 1e12, "unit": UNIT,
                "h2d_bytes_per_step": int(w.in_bytes), "d2h_bytes_per_step": d2h, "steps": Ke,
                "ms_per_step": e2e_ms / Ke, "h2d_gbs": w.in_bytes / (e2e_ms / Ke * 1e-3) / 1e9,
@@ -376,30 +543,64 @@ def main():
         sample_src = hv
     else:
         sample_src = v
+        P_dev = P
 
     # ---------------------------------------------------------------- oracle on the host cores (rank 0, N=1)
-    cpu = None
+    cpu, max_err = None, None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         def v_host(chans):
             return sample_src[chans].cpu().numpy() if sample_src.is_cuda else sample_src[chans].numpy()
-        val, cores, desc, _, _ = time_oracle_sample(w, v_host)
+        val, cores, desc, _, nref, ref = time_oracle_sample(w, v_host)
         cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        # whole-buffer parity of the very launch configuration that was timed: every channel the oracle computed
+        # (outside the timed region) against the device-resident powers
+        max_err = {"value": row_error(P_dev[:nref].cpu().numpy(), ref), "bar": 1e-3, "channels": nref, "of": w.nchan,
+                   "definition": "max over (chan, beam) rows of max_j |P_gpu - P_ref| / mean_j P_ref"}
+        del ref
+    T.close()
+    v = None
+    del T, P, P_dev, sample_src, v
+    torch.cuda.empty_cache()
+
+    # ---------------------------------------------------------------- the other BASELINE.json configurations
+    configs = None
+    if rank == 0 and world == 1 and args.config == "medium" and args.mode == "power" and not args.no_configs and not args.nbeam:
+        configs = {"medium": {"ms": avg_kernel_ms, "bound": roof["bound"], "frac": roof["frac"],
+                              "frac_of_burst": roof.get("frac_of_burst"), "frac_of_sustained": roof.get("frac_of_sustained"),
+                              "achieved": roof["achieved"], "unit": roof["unit"], "traffic": roof["traffic"], "kernel": kernel_name,
+                              "tflops": flop_step / (avg_kernel_ms * 1e-3) / 1e12, "steps": K, "clocks": clocks, "l2": l2_note}}
+        for name in ALL_CONFIGS:
+            wc = workload_for(name)
+            Tc = Timed(bf, synthetic, torch, wc, dev, bf.BF_KERNEL_AUTO)
+            Kc = 200 if name == "tiny" else 30
+            tot, per, _, clk = Tc.measure(Kc, 5, barrier)
+            ms = statistics.mean(per)
+            r = Tc.roofline(ms, tot, clk, peaks, load_traffic(wc.name))
+            configs[wc.name] = {
+                "ms": ms, "bound": r["bound"], "frac": r["frac"], "frac_of_burst": r.get("frac_of_burst"),
+                "frac_of_sustained": r.get("frac_of_sustained"), "achieved": r["achieved"], "unit": r["unit"],
+                "traffic": r["traffic"], "kernel": Tc.B.kernel_name, "tflops": Tc.flop_step() / (ms * 1e-3) / 1e12,
+                "steps": Kc, "clocks": clk, "l2": Tc.l2}
+            Tc.close()
+            del Tc
+            torch.cuda.empty_cache()
 
     if rank == 0:
         line = {
-            "metric": METRIC if args.mode == "power" else METRIC + " [side mode: %s]" % args.mode, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "metric": METRIC if args.mode == "power" else METRIC + " [side mode: %s]" % args.mode, "value": value, "unit": UNIT,
+            "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None,
-            "dtype": "i8->i32 (dp4a)" if args.mode == "incoherent" else {"umma-i8": "i8xi8->i32", "simt": "f32"}.get(B.kernel_name, "f16xf16->f32"),
+            "dtype": "i8->i32 (dp4a)" if args.mode == "incoherent" else {"umma-i8": "i8xi8->i32", "simt": "f32"}.get(kernel_name, "f16xf16->f32"),
             "data": "synthetic",
-            "config": {"workload": w.name if args.mode == "power" else w.name + ":" + args.mode, "nant": w.nant, "nchan": w.nchan, "nbeam": w.nbeam, "nsamp": w.nsamp,
-                       "nint": w.nint, "input": w.dtype, "l2": "input buffer (%.0f MB) >> L2 (126 MB), no flush needed" % (w.in_bytes / 1e6),
-                       "kernel": B.kernel_name, "parallelism": (f"channel shards x{world}" if args.scaling == "strong" and world > 1 else f"replicas x{world}")},
+            "config": {"workload": w.name if args.mode == "power" else w.name + ":" + args.mode, "nant": w.nant, "nchan": w.nchan,
+                       "nbeam": w.nbeam, "nsamp": w.nsamp, "nint": w.nint, "input": w.dtype, "l2": l2_note, "kernel": kernel_name,
+                       "parallelism": (f"channel shards x{world}" if args.scaling == "strong" and world > 1 else f"replicas x{world}")},
             "ant_samples_per_s": world * w.nchan * w.nsamp * w.nant * K / (total_ms_max * 1e-3),
-            "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "roofline": roof, "cpu_baseline": cpu, "max_err": max_err, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "configs": configs,
             "context": {"paper_k20_tflops": 1.3, "note": "paper's number is a Tesla K20 with 4-bit input (PAPER.md:15): context, not a baseline for this config"},
         }
         print(json.dumps(line))
-    B.close()
     if dist:
         td.destroy_process_group()
     return 0

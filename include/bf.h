@@ -199,6 +199,16 @@ int bf_run_host(bf_ctx *ctx, const void *host_voltages, float *host_powers, void
 int bf_run_streaming(bf_ctx *ctx, const void *const *host_blocks, int nblocks, float *powers,
                      void *staging, size_t staging_bytes, void *compute_stream, void *copy_stream);
 
+/*
+ * Measurement hook: when `dev_u64x4` is a non-NULL DEVICE pointer to four 64-bit words,
+ * CTA 0 of every hot-path kernel the context launches afterwards writes
+ *   { clock64 at start, globaltimer (ns) at start, clock64 at end, globaltimer (ns) at end }
+ * so the caller can compute the SM clock the kernel really ran at, (c1 - c0) / (t1 - t0) GHz -- nvidia-smi's
+ * sampled clock is too coarse for a millisecond kernel.  NULL switches it off (the default).  Two scalar
+ * stores per launch; no effect on the result.
+ */
+int bf_set_clock_probe(bf_ctx *ctx, void *dev_u64x4);
+
 /* Message for the last error on this context ("" if none).  Valid until the next call on ctx. */
 const char *bf_last_error(const bf_ctx *ctx);
 

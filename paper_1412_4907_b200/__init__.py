@@ -44,6 +44,7 @@ SYMBOLS = {
     "bf_staging_bytes": (_sz, [_vp, _i]),
     "bf_run_host": (_i, [_vp, _vp, _vp, _vp, _sz, _i, _vp, _vp]),
     "bf_run_streaming": (_i, [_vp, ctypes.POINTER(_vp), _i, _vp, _vp, _sz, _vp, _vp]),
+    "bf_set_clock_probe": (_i, [_vp, _vp]),
     "bf_last_error": (ctypes.c_char_p, [_vp]),
     "bf_version": (ctypes.c_char_p, []),
 }
@@ -199,6 +200,10 @@ def bf_run_streaming(ctx, host_blocks, powers, staging, staging_bytes, compute_s
                                   _stream(compute_stream), _stream(copy_stream))
 
 
+def bf_set_clock_probe(ctx, dev_u64x4):
+    return lib().bf_set_clock_probe(ctx, _ptr(dev_u64x4))
+
+
 def bf_last_error(ctx):
     s = lib().bf_last_error(ctx)
     return s.decode() if s else ""
@@ -317,6 +322,10 @@ class Beamformer:
         nbytes = 2 * ((in_bytes + 1023) // 1024 * 1024)
         st = self._get_staging(nbytes)
         self._check(bf_run_streaming(self.ctx, host_blocks, powers, st, nbytes, compute_stream, copy_stream))
+
+    def set_clock_probe(self, dev_u64x4):
+        """dev_u64x4: torch int64 tensor of 4 elements on the device (or None): see bf_set_clock_probe."""
+        self._check(bf_set_clock_probe(self.ctx, dev_u64x4))
 
     @property
     def selected_kernel(self):

@@ -27,6 +27,16 @@ static int cuda_fail(bf_ctx *c, cudaError_t e, const char *what) {
   return fail(c, BF_ECUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 
+// every stream-ordering guarantee of the library (tracking beams, host / streaming overlap) rests on these two
+static int wait_event(bf_ctx *c, cudaStream_t st, cudaEvent_t ev) {
+  cudaError_t e = cudaStreamWaitEvent(st, ev, 0);
+  return e == cudaSuccess ? BF_OK : cuda_fail(c, e, "cudaStreamWaitEvent");
+}
+static int record_event(bf_ctx *c, cudaEvent_t ev, cudaStream_t st) {
+  cudaError_t e = cudaEventRecord(ev, st);
+  return e == cudaSuccess ? BF_OK : cuda_fail(c, e, "cudaEventRecord");
+}
+
 size_t bf_in_bytes_per_chan(const bf_ctx *c) {
   return (size_t)c->nsamp * c->nant * (c->dtype == BF_CI8 ? 2 : c->dtype == BF_CI4 ? 1 : 4);
 }
@@ -70,6 +80,7 @@ extern "C" bf_ctx *bf_create(int nant, int nchan, int nbeam, int nsamp, int nint
   c->geom_buf[0] = c->geom_buf[1] = nullptr; c->wop_buf[0] = c->wop_buf[1] = nullptr;
   c->wop8_buf[0] = c->wop8_buf[1] = nullptr; c->d_wop8 = nullptr; c->d_i8scale = nullptr;
   c->have_wevents = false; c->used[0] = c->used[1] = false;
+  c->d_probe = nullptr;
   c->err[0] = 0;
   return c;
 }
@@ -77,7 +88,10 @@ extern "C" bf_ctx *bf_create(int nant, int nchan, int nbeam, int nsamp, int nint
 extern "C" void bf_destroy(bf_ctx *c) {
   if (!c) return;
   if (c->have_events)
-    for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_copied[i]); cudaEventDestroy(c->ev_done[i]); }
+  {
+    for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_copied[i]); cudaEventDestroy(c->ev_done[i]); cudaEventDestroy(c->ev_kdone[i]); }
+    cudaStreamDestroy(c->d2h_stream);
+  }
   if (c->have_wevents) { cudaEventDestroy(c->ev_upd); cudaEventDestroy(c->ev_use[0]); cudaEventDestroy(c->ev_use[1]); }
   delete c;
 }
@@ -87,7 +101,16 @@ extern "C" const char *bf_last_error(const bf_ctx *c) { return c ? c->err : "nul
 extern "C" int bf_set_dtype(bf_ctx *c, int dtype) {
   if (!c) return BF_EINVAL;
   if (dtype != BF_CI8 && dtype != BF_CF16 && dtype != BF_CI4) return fail(c, BF_EINVAL, "unknown dtype %d", dtype);
+  // the workspace layout (which weight operands exist) depends on the element type
+  if (c->ws && dtype != c->dtype) return fail(c, BF_EINVAL, "bf_set_dtype must be called before bf_set_workspace");
   c->dtype = dtype;
+  return BF_OK;
+}
+
+extern "C" int bf_set_clock_probe(bf_ctx *c, void *dev_u64x4) {
+  if (!c) return BF_EINVAL;
+  if (((uintptr_t)dev_u64x4) % 8) return fail(c, BF_EINVAL, "clock probe must be 8-byte aligned");
+  c->d_probe = (unsigned long long *)dev_u64x4;
   return BF_OK;
 }
 
@@ -109,7 +132,7 @@ static int pick_kernel(const bf_ctx *c, int mode, const char **why) {
   int k = c->kernel_forced;
   *why = "";
   if (k == BF_KERNEL_SIMT) return BF_KERNEL_SIMT;
-  const bool i8_ok = i8_shape(c) && bf_umma_i8_supported(c, mode);
+  const bool i8_ok = i8_shape(c) && bf_umma_i8_supported(c, mode) && (c->d_wop8 != nullptr || c->ws == nullptr);
   if (k == BF_KERNEL_UMMA_I8) {
     if (!i8_ok) *why = "int8 kernel needs complex int8 input, nant % 8 == 0 and <= 32, <= 32 beams, nint 2^k <= 32 or % 32 == 0";
     return i8_ok ? BF_KERNEL_UMMA_I8 : 0;
@@ -266,8 +289,8 @@ extern "C" int bf_set_geometry(bf_ctx *c, const double *ant, const double *freq,
   if (!c->ws) return fail(c, BF_ENOGEOM, "bf_set_workspace must be called before bf_set_geometry");
   if ((rc = probe_device(c)) != BF_OK) return rc;
   if (c->pending >= 0) {  // an update in flight is superseded: this call defines the weights of the next run
+    if ((rc = wait_event(c, (cudaStream_t)stream, c->ev_upd)) != BF_OK) return rc;
     c->active = c->pending; c->pending = -1;
-    cudaStreamWaitEvent((cudaStream_t)stream, c->ev_upd, 0);
   }
   select_buffer(c, c->active);
   if ((rc = upload_and_generate(c, ant, freq, dir, (cudaStream_t)stream)) != BF_OK) return rc;
@@ -297,12 +320,12 @@ extern "C" int bf_update_geometry(bf_ctx *c, const double *ant, const double *fr
   cudaStream_t us = (cudaStream_t)update_stream;
   const int target = 1 - c->active;  // a second update before any run overwrites the same (unused) buffer
   // runs that read `target` before the last switch may still be executing on the run stream
-  if (c->used[target]) cudaStreamWaitEvent(us, c->ev_use[target], 0);
+  if (c->used[target] && (rc = wait_event(c, us, c->ev_use[target])) != BF_OK) return rc;
   select_buffer(c, target);
   rc = upload_and_generate(c, ant, freq, dir, us);
   select_buffer(c, c->active);
   if (rc != BF_OK) return rc;
-  cudaEventRecord(c->ev_upd, us);
+  if ((rc = record_event(c, c->ev_upd, us)) != BF_OK) return rc;
   c->pending = target;
   return BF_OK;
 }
@@ -329,8 +352,9 @@ extern "C" int bf_set_antenna_gains(bf_ctx *c, const double *gains, int per_chan
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e = cudaSuccess;
   if (c->pending >= 0) {  // regenerate the weights the next run will use
+    int rc = wait_event(c, st, c->ev_upd);
+    if (rc != BF_OK) return rc;
     c->active = c->pending; c->pending = -1;
-    cudaStreamWaitEvent(st, c->ev_upd, 0);
     select_buffer(c, c->active);
   }
   if (c->have_gains) e = cudaMemcpyAsync(c->d_gain, c->h_gain.data(), c->h_gain.size() * sizeof(double), cudaMemcpyHostToDevice, st);
@@ -347,7 +371,8 @@ extern "C" int bf_get_weights(bf_ctx *c, float *host_out, void *stream) {
   if (!c->have_geom) return fail(c, BF_ENOGEOM, "no geometry set");
   cudaStream_t st = (cudaStream_t)stream;
   if (c->pending >= 0) {  // report the weights the next run will use
-    cudaStreamWaitEvent(st, c->ev_upd, 0);
+    int rc = wait_event(c, st, c->ev_upd);
+    if (rc != BF_OK) return rc;
     c->active = c->pending; c->pending = -1;
     select_buffer(c, c->active);
   }
@@ -379,6 +404,7 @@ static int launch_range(bf_ctx *c, const void *volt, void *out, int chan0, int n
   p.wop = c->d_wop + (size_t)chan0 * (bf_wop_bytes_per_chan(c) / sizeof(__half));
   p.wop8 = c->d_wop8 ? c->d_wop8 + (size_t)chan0 * bf_i8_ncol(c->nbeam) * 64 : nullptr;
   p.i8scale = c->d_i8scale + chan0;
+  p.probe = c->d_probe;
   const char *why = "";
   const int k = pick_kernel(c, mode, &why);
   if (k == 0) return fail(c, BF_EUNSUPPORTED, "tensor-core kernel cannot run this shape: %s", why);
@@ -398,30 +424,40 @@ static int check_run(bf_ctx *c, const void *volt, const void *pow) {
 }
 
 // tracking beams (row f3): switch to freshly generated weights once their generator has finished
-static void begin_run(bf_ctx *c, cudaStream_t st) {
+static int begin_run(bf_ctx *c, cudaStream_t st) {
   if (c->pending >= 0) {
-    cudaStreamWaitEvent(st, c->ev_upd, 0);
+    int rc = wait_event(c, st, c->ev_upd);
+    if (rc != BF_OK) return rc;
     c->active = c->pending;
     c->pending = -1;
     select_buffer(c, c->active);
   }
+  return BF_OK;
 }
 // ... and remember when the last reader of the active buffer is done, for the next update of it
-static void end_run(bf_ctx *c, cudaStream_t st) {
-  if (c->nwbuf == 2 && ensure_wevents(c) == BF_OK) {
-    cudaEventRecord(c->ev_use[c->active], st);
-    c->used[c->active] = true;
-  }
+static int end_run(bf_ctx *c, cudaStream_t st) {
+  if (c->nwbuf != 2) return BF_OK;
+  int rc = ensure_wevents(c);
+  if (rc == BF_OK) rc = record_event(c, c->ev_use[c->active], st);
+  if (rc == BF_OK) c->used[c->active] = true;
+  return rc;
+}
+// a failed launch must still leave the buffer bookkeeping consistent; the first error wins
+static int finish_run(bf_ctx *c, cudaStream_t st, int rc) {
+  char msg[sizeof(c->err)];
+  memcpy(msg, c->err, sizeof(msg));
+  const int rc2 = end_run(c, st);
+  if (rc != BF_OK) { memcpy(c->err, msg, sizeof(msg)); return rc; }
+  return rc2;
 }
 
 extern "C" int bf_run(bf_ctx *c, const void *voltages, float *powers, void *stream) {
   int rc = check_run(c, voltages, powers);
   if (rc != BF_OK) return rc;
   if (((uintptr_t)voltages) % 16) return fail(c, BF_EINVAL, "voltages must be 16-byte aligned");
-  begin_run(c, (cudaStream_t)stream);
+  if ((rc = begin_run(c, (cudaStream_t)stream)) != BF_OK) return rc;
   rc = launch_range(c, voltages, powers, 0, c->nchan, (cudaStream_t)stream);
-  end_run(c, (cudaStream_t)stream);
-  return rc;
+  return finish_run(c, (cudaStream_t)stream, rc);
 }
 
 extern "C" int bf_run_beams(bf_ctx *c, const void *voltages, void *beams, float scale, void *stream) {
@@ -430,10 +466,9 @@ extern "C" int bf_run_beams(bf_ctx *c, const void *voltages, void *beams, float 
   if (((uintptr_t)voltages) % 16) return fail(c, BF_EINVAL, "voltages must be 16-byte aligned");
   if (((uintptr_t)beams) % 4) return fail(c, BF_EINVAL, "beams must be 4-byte aligned");
   if (!isfinite(scale) || scale == 0.f) return fail(c, BF_EINVAL, "scale must be finite and non-zero");
-  begin_run(c, (cudaStream_t)stream);
+  if ((rc = begin_run(c, (cudaStream_t)stream)) != BF_OK) return rc;
   rc = launch_range(c, voltages, beams, 0, c->nchan, (cudaStream_t)stream, BF_MODE_BEAMS, scale);
-  end_run(c, (cudaStream_t)stream);
-  return rc;
+  return finish_run(c, (cudaStream_t)stream, rc);
 }
 
 extern "C" int bf_run_incoherent(bf_ctx *c, const void *voltages, float *powers, void *stream) {
@@ -452,8 +487,12 @@ static int ensure_events(bf_ctx *c) {
   for (int i = 0; i < 2; ++i) {
     cudaError_t e = cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_kdone[i], cudaEventDisableTiming);
     if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventCreate");
   }
+  // the read-back queue of bf_run_host (the one stream the library owns)
+  cudaError_t e = cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking);
+  if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamCreate");
   c->have_events = true;
   return BF_OK;
 }
@@ -475,7 +514,7 @@ extern "C" int bf_run_host(bf_ctx *c, const void *host_volt, float *host_pow, vo
   if (!staging || ((uintptr_t)staging) % BF_ALIGN) return fail(c, BF_EINVAL, "staging must be a %d-byte aligned device pointer", BF_ALIGN);
   if (staging_bytes < bf_staging_bytes(c, chan_per_chunk)) return fail(c, BF_ENOMEM, "staging too small");
   if ((rc = ensure_events(c)) != BF_OK) return rc;
-  cudaStream_t cs = (cudaStream_t)compute_stream, xs = (cudaStream_t)copy_stream;
+  cudaStream_t cs = (cudaStream_t)compute_stream, xs = (cudaStream_t)copy_stream, ds = c->d2h_stream;
   const size_t in_chan = bf_in_bytes_per_chan(c), out_chan = (size_t)c->nbeam * c->nbin * sizeof(float);
   const size_t in_buf = align_up((size_t)chan_per_chunk * in_chan, BF_ALIGN);
   const size_t out_buf = align_up((size_t)chan_per_chunk * out_chan, BF_ALIGN);
@@ -483,26 +522,33 @@ extern "C" int bf_run_host(bf_ctx *c, const void *host_volt, float *host_pow, vo
   char *out[2] = {(char *)staging + 2 * in_buf, (char *)staging + 2 * in_buf + out_buf};
   cudaError_t e;
   int k = 0;
-  begin_run(c, cs);
-  for (int c0 = 0; c0 < c->nchan; c0 += chan_per_chunk, ++k) {
-    int n = c->nchan - c0 < chan_per_chunk ? c->nchan - c0 : chan_per_chunk;
-    int b = k & 1;
-    // staging half b is free once the kernel + D2H that used it two chunks ago are done
-    if (k >= 2 && (e = cudaStreamWaitEvent(xs, c->ev_done[b], 0)) != cudaSuccess) return cuda_fail(c, e, "cudaStreamWaitEvent");
+  if ((rc = begin_run(c, cs)) != BF_OK) return rc;
+  // Three queues: H2D on the copy stream, kernels on the compute stream, D2H on the library's own stream, so
+  // that kernel k+1 never waits for the read-back of chunk k (the step takes "the duration of the
+  // slowest stage").  Input half b is free once kernel k-2 has run (ev_kdone), output half b once its D2H is done.
+  for (int c0 = 0; c0 < c->nchan && rc == BF_OK; c0 += chan_per_chunk, ++k) {
+    const int n = c->nchan - c0 < chan_per_chunk ? c->nchan - c0 : chan_per_chunk;
+    const int b = k & 1;
+    if (k >= 2 && (rc = wait_event(c, xs, c->ev_kdone[b])) != BF_OK) break;
     e = cudaMemcpyAsync(in[b], (const char *)host_volt + (size_t)c0 * in_chan, (size_t)n * in_chan, cudaMemcpyHostToDevice, xs);
-    if (e != cudaSuccess) return cuda_fail(c, e, "voltage H2D copy");
-    cudaEventRecord(c->ev_copied[b], xs);
-    cudaStreamWaitEvent(cs, c->ev_copied[b], 0);
-    if ((rc = launch_range(c, in[b], (float *)out[b], c0, n, cs)) != BF_OK) return rc;
-    e = cudaMemcpyAsync((char *)host_pow + (size_t)c0 * out_chan, out[b], (size_t)n * out_chan, cudaMemcpyDeviceToHost, cs);
-    if (e != cudaSuccess) return cuda_fail(c, e, "power D2H copy");
-    cudaEventRecord(c->ev_done[b], cs);
+    if (e != cudaSuccess) { rc = cuda_fail(c, e, "voltage H2D copy"); break; }
+    if ((rc = record_event(c, c->ev_copied[b], xs)) != BF_OK) break;
+    if ((rc = wait_event(c, cs, c->ev_copied[b])) != BF_OK) break;
+    if (k >= 2 && (rc = wait_event(c, cs, c->ev_done[b])) != BF_OK) break;   // out[b] has been read back
+    if ((rc = launch_range(c, in[b], (float *)out[b], c0, n, cs)) != BF_OK) break;
+    if ((rc = record_event(c, c->ev_kdone[b], cs)) != BF_OK) break;
+    if ((rc = wait_event(c, ds, c->ev_kdone[b])) != BF_OK) break;
+    e = cudaMemcpyAsync((char *)host_pow + (size_t)c0 * out_chan, out[b], (size_t)n * out_chan, cudaMemcpyDeviceToHost, ds);
+    if (e != cudaSuccess) { rc = cuda_fail(c, e, "power D2H copy"); break; }
+    rc = record_event(c, c->ev_done[b], ds);
   }
-  // the next call on this context must not overwrite staging that is still in flight
-  cudaStreamWaitEvent(xs, c->ev_done[0], 0);
-  if (k > 1) cudaStreamWaitEvent(xs, c->ev_done[1], 0);
-  end_run(c, cs);
-  return BF_OK;
+  // whoever synchronises the two caller streams has the powers on the host, and the next call on this context
+  // cannot overwrite staging that is still in flight
+  for (int b = 0; b < (k > 1 ? 2 : 1) && rc == BF_OK && k > 0; ++b) {
+    if ((rc = wait_event(c, cs, c->ev_done[b])) != BF_OK) break;
+    rc = wait_event(c, xs, c->ev_done[b]);
+  }
+  return finish_run(c, cs, rc);
 }
 
 extern "C" int bf_run_streaming(bf_ctx *c, const void *const *host_blocks, int nblocks, float *powers, void *staging,
@@ -521,19 +567,18 @@ extern "C" int bf_run_streaming(bf_ctx *c, const void *const *host_blocks, int n
   const size_t out_elems = (size_t)c->nchan * c->nbeam * c->nbin;
   char *in[2] = {(char *)staging, (char *)staging + in_buf};
   cudaError_t e;
-  begin_run(c, cs);
-  for (int i = 0; i < nblocks; ++i) {
-    int b = i & 1;
-    if (i >= 2 && (e = cudaStreamWaitEvent(xs, c->ev_done[b], 0)) != cudaSuccess) return cuda_fail(c, e, "cudaStreamWaitEvent");
+  if ((rc = begin_run(c, cs)) != BF_OK) return rc;
+  int i = 0;
+  for (; i < nblocks && rc == BF_OK; ++i) {
+    const int b = i & 1;
+    if (i >= 2 && (rc = wait_event(c, xs, c->ev_kdone[b])) != BF_OK) break;
     e = cudaMemcpyAsync(in[b], host_blocks[i], in_bytes, cudaMemcpyHostToDevice, xs);
-    if (e != cudaSuccess) return cuda_fail(c, e, "block H2D copy");
-    cudaEventRecord(c->ev_copied[b], xs);
-    cudaStreamWaitEvent(cs, c->ev_copied[b], 0);
-    if ((rc = launch_range(c, in[b], powers + (size_t)i * out_elems, 0, c->nchan, cs)) != BF_OK) return rc;
-    cudaEventRecord(c->ev_done[b], cs);
+    if (e != cudaSuccess) { rc = cuda_fail(c, e, "block H2D copy"); break; }
+    if ((rc = record_event(c, c->ev_copied[b], xs)) != BF_OK) break;
+    if ((rc = wait_event(c, cs, c->ev_copied[b])) != BF_OK) break;
+    if ((rc = launch_range(c, in[b], powers + (size_t)i * out_elems, 0, c->nchan, cs)) != BF_OK) break;
+    rc = record_event(c, c->ev_kdone[b], cs);
   }
-  cudaStreamWaitEvent(xs, c->ev_done[0], 0);
-  if (nblocks > 1) cudaStreamWaitEvent(xs, c->ev_done[1], 0);
-  end_run(c, cs);
-  return BF_OK;
+  for (int b = 0; b < (i > 1 ? 2 : 1) && rc == BF_OK && i > 0; ++b) rc = wait_event(c, xs, c->ev_kdone[b]);
+  return finish_run(c, cs, rc);
 }

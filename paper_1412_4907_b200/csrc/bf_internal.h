@@ -45,6 +45,7 @@ struct BfParams {
   const __half *wop;    // device, weight operand of the first channel of this launch
   const signed char *wop8;  // int8 two-limb weight operand of the first channel (bf_umma_i8.cu), or NULL
   const double *i8scale;    // per channel: y = (128 hi + lo) * i8scale[c]
+  unsigned long long *probe;  // bf_set_clock_probe: 4 words written by CTA 0, or NULL
 };
 
 // ---- int8 two-limb weight operand (bf_umma_i8.cu; few beams, small arrays) ---------------------
@@ -84,8 +85,10 @@ struct bf_ctx {
   long long launches;
   int sm_count;     // 0 = device not probed yet
   int device_ok;    // -1 unknown, 0 no, 1 yes
-  cudaEvent_t ev_copied[2], ev_done[2];
+  cudaEvent_t ev_copied[2], ev_done[2], ev_kdone[2];   // H2D landed / D2H landed / kernel finished, per staging half
+  cudaStream_t d2h_stream;                             // bf_run_host's read-back queue (created with the events)
   bool have_events;
+  unsigned long long *d_probe;   // bf_set_clock_probe
   char err[512];
 };
 

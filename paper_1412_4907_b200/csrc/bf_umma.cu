@@ -33,6 +33,23 @@ using namespace bfk;
 
 constexpr int MAX_INPUT_PIECES = TILE_T * 4;  // 16-byte input pieces per tile at nant = 32
 
+// BF_K64_UPFRONT: the epilogue warps request all their TMEM columns of a tile at once (64 registers of data) and
+// hand the accumulator stage back after one wait.  The registers come from the other roles: 28 warps are launched
+// at 72 registers, the four epilogue warpgroups grow to 96, the convert / MMA / TMA warpgroups shrink to 40
+// (setmaxnreg; 16*32*96 + 12*32*40 = 28*32*72).
+#ifndef BF_K64_UPFRONT
+#define BF_K64_UPFRONT 1
+#endif
+#ifndef BF_K64_EPI_REGS
+#define BF_K64_EPI_REGS 96
+#endif
+#ifndef BF_K64_OTHER_REGS
+#define BF_K64_OTHER_REGS 40
+#endif
+template <bool SPREAD> constexpr bool upfront_v = BF_K64_UPFRONT && !SPREAD;
+template <bool SPREAD, int CONV_WARPS> constexpr int k64_threads_v =
+    SPREAD ? 1024 : (upfront_v<SPREAD> ? (EPI_WARPS + CONV_WARPS + 4) * 32 : (EPI_WARPS + CONV_WARPS + 3) * 32);
+
 struct Item { int c, g, tt; };
 
 __device__ __forceinline__ Item decode_item(long long idx, int nG, int nTt) {
@@ -58,7 +75,7 @@ __device__ __forceinline__ void next_item(Item &it, int nG, int nTt) {
 // beams the whole epilogue therefore lands on sub-partition 0; SPREAD launches 32 warps and puts the
 // convert / MMA / TMA warps on sub-partitions 1-3 only, so that sub-partition 0 does nothing else.
 template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD, int IN, bool BEAMS>
-__global__ void __launch_bounds__(SPREAD ? 1024 : (EPI_WARPS + CONV_WARPS + 3) * 32, 1)
+__global__ void __launch_bounds__(k64_threads_v<SPREAD, CONV_WARPS>, 1)
 bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, const int nTt, const int nks) {
   extern __shared__ uint8_t smem_raw[];
   constexpr int CONV_THREADS = CONV_WARPS * 32;
@@ -111,6 +128,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(s_tmem));
   tmem_base = __shfl_sync(0xffffffffu, tmem_base, 0);
+  probe_mark(p.probe, 0);
 
   // this CTA's contiguous item range
   const long long it0 = total_items * blockIdx.x / gridDim.x;
@@ -118,6 +136,11 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   const int n_items = (int)(it1 - it0);
   const int nMt = p.nMt;
 
+  constexpr bool UPF = upfront_v<SPREAD>;
+  if constexpr (UPF) {  // whole warpgroups (4 warps) move registers: 0-3 epilogue, 4-6 everything else
+    if (warp < EPI_WARPS) setmaxnreg_inc<BF_K64_EPI_REGS>();
+    else setmaxnreg_dec<BF_K64_OTHER_REGS>();
+  }
   if (warp < EPI_WARPS) {
     // =========================================================================== epilogue
     // 16 warps: warp w owns TMEM lanes 32*(w&3).. and columns 64*(w>>2).. of EVERY accumulator tile.
@@ -189,8 +212,8 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
             epilogue_beams_tile(t_lane + ACC * TILE_T, bptr + (size_t)m * BF_TILE_BEAMS * p.nsamp, (bok >> m) & 1, nvalid,
                                 bvec_ok, p.beam_scale, lane >= 16, b_full + 16 + 8 * ACC, lane0);
           else
-            epilogue_tile<NINT_T>(t_lane + ACC * TILE_T, out + m * mstride, (wr >> m) & 1, nvalid, NINT_T != 0 && vec_ok,
-                                  b_full + 16 + 8 * ACC, lane0);
+            epilogue_tile<NINT_T, UPF>(t_lane + ACC * TILE_T, out + m * mstride, (wr >> m) & 1, nvalid, NINT_T != 0 && vec_ok,
+                                       b_full + 16 + 8 * ACC, lane0);
         };
         if constexpr (GROUP == 1) {
           if (i & 1) one(std::integral_constant<int, 1>{}, 0);
@@ -248,31 +271,39 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         const int rs = i % NRAW, st = i % NSTAGE;
         const uint32_t raw = raw0 + rs * RAW_STAGE_BYTES, dst = dst0 + st * B_STAGE_BYTES;
         mbar_wait(bar_r_full + 8 * rs, (uint32_t)((i / NRAW) & 1));
-        uint4 x[GP];
+        constexpr int RP = UPF ? 4 : GP;   // pieces per round (a round's pieces live in registers: 40-register budget)
+        uint4 x[RP];
 #pragma unroll
-        for (int k = 0; k < GP; ++k) x[k] = ld_shared_v4(raw + k * (16 * GT));
+        for (int k = 0; k < RP; ++k) x[k] = ld_shared_v4(raw + k * (16 * GT));
         mbar_wait(bar_b_empty + 8 * st, (uint32_t)(((i / NSTAGE) & 1) ^ 1));
-        if (IN == BF_CI4) {
-          const uint32_t d1 = dst ^ 16u, d2 = dst ^ 32u, d3 = dst ^ 48u;
 #pragma unroll
-          for (int k = 0; k < GP; ++k) {
-            uint32_t h[4];
-            cvt_i4x8_f16x8(x[k].x, h); st_shared_v4(dst + k * KSTEP, h[0], h[1], h[2], h[3]);
-            cvt_i4x8_f16x8(x[k].y, h); st_shared_v4(d1 + k * KSTEP, h[0], h[1], h[2], h[3]);
-            cvt_i4x8_f16x8(x[k].z, h); st_shared_v4(d2 + k * KSTEP, h[0], h[1], h[2], h[3]);
-            cvt_i4x8_f16x8(x[k].w, h); st_shared_v4(d3 + k * KSTEP, h[0], h[1], h[2], h[3]);
+        for (int r0 = 0; r0 < GP; r0 += RP) {
+          if (r0 > 0) {
+#pragma unroll
+            for (int k = 0; k < RP; ++k) x[k] = ld_shared_v4(raw + (r0 + k) * (16 * GT));
           }
-        } else {
-          const uint32_t d1 = dst ^ 16u;
+          if (IN == BF_CI4) {
+            const uint32_t d1 = dst ^ 16u, d2 = dst ^ 32u, d3 = dst ^ 48u;
 #pragma unroll
-          for (int k = 0; k < GP; ++k) {
-            uint32_t h[8];
-            cvt_i8x4_f16x4(x[k].x, h[0], h[1]);
-            cvt_i8x4_f16x4(x[k].y, h[2], h[3]);
-            cvt_i8x4_f16x4(x[k].z, h[4], h[5]);
-            cvt_i8x4_f16x4(x[k].w, h[6], h[7]);
-            st_shared_v4(dst + k * KSTEP, h[0], h[1], h[2], h[3]);
-            st_shared_v4(d1 + k * KSTEP, h[4], h[5], h[6], h[7]);
+            for (int k = 0; k < RP; ++k) {
+              uint32_t h[4];
+              cvt_i4x8_f16x8(x[k].x, h); st_shared_v4(dst + (r0 + k) * KSTEP, h[0], h[1], h[2], h[3]);
+              cvt_i4x8_f16x8(x[k].y, h); st_shared_v4(d1 + (r0 + k) * KSTEP, h[0], h[1], h[2], h[3]);
+              cvt_i4x8_f16x8(x[k].z, h); st_shared_v4(d2 + (r0 + k) * KSTEP, h[0], h[1], h[2], h[3]);
+              cvt_i4x8_f16x8(x[k].w, h); st_shared_v4(d3 + (r0 + k) * KSTEP, h[0], h[1], h[2], h[3]);
+            }
+          } else {
+            const uint32_t d1 = dst ^ 16u;
+#pragma unroll
+            for (int k = 0; k < RP; ++k) {
+              uint32_t h[8];
+              cvt_i8x4_f16x4(x[k].x, h[0], h[1]);
+              cvt_i8x4_f16x4(x[k].y, h[2], h[3]);
+              cvt_i8x4_f16x4(x[k].z, h[4], h[5]);
+              cvt_i8x4_f16x4(x[k].w, h[6], h[7]);
+              st_shared_v4(dst + (r0 + k) * KSTEP, h[0], h[1], h[2], h[3]);
+              st_shared_v4(d1 + (r0 + k) * KSTEP, h[4], h[5], h[6], h[7]);
+            }
           }
         }
         fence_proxy_async_smem();
@@ -384,6 +415,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   tc_fence_before();
   __syncthreads();
   if (mw == 0) tmem_dealloc(tmem_base, 512);
+  probe_mark(p.probe, 1);
 }
 
 template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD, int IN, bool BEAMS = false>
@@ -401,7 +433,7 @@ cudaError_t launch_k64(const BfParams &p, int sm_count, cudaStream_t st) {
     if (e != cudaSuccess) return e;
   }
   const int grid = (int)(total < sm_count ? total : sm_count);
-  kern<<<grid, SPREAD ? 1024 : (EPI_WARPS + CONV_WARPS + 3) * 32, smem, st>>>(p, total, nG, nTt, nks);
+  kern<<<grid, k64_threads_v<SPREAD, CONV_WARPS>, smem, st>>>(p, total, nG, nTt, nks);
   return cudaGetLastError();
 }
 

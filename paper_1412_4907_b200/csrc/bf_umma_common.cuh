@@ -104,7 +104,7 @@ __device__ __forceinline__ void convert_store_ci4(uint32_t s_dst, const uint32_t
 // that it can be hoisted out of the tile loop.
 // NINT_T: integration length if a power of two <= 64; 0 = a larger multiple of 64: the partial sum of
 // the warp's 64 columns is added atomically into the (zeroed) bin `out` points at.
-template <int NINT_T>
+template <int NINT_T, bool UPFRONT = false>
 __device__ __forceinline__ void epilogue_tile(uint32_t taddr, float *out, bool writer, int nvalid, bool vec_ok,
                                               uint32_t bar_empty, bool lane0) {
   constexpr int CPW = TILE_T / (EPI_WARPS / 4);                          // columns per warp (64)
@@ -119,15 +119,28 @@ __device__ __forceinline__ void epilogue_tile(uint32_t taddr, float *out, bool w
   float2 a[NACC];  // packed running sums of squares; live across the chunks of one bin
 #pragma unroll
   for (int q = 0; q < NACC; ++q) a[q] = make_float2(0.f, 0.f);
+  uint32_t vv[UPFRONT ? NCH : 1][32];
+  if constexpr (UPFRONT) {
+    // the accumulator ring is the critical loop (MMA -> commit -> tcgen05.ld -> arrive -> next MMA): request ALL of this
+    // warp's columns at once and hand the stage back after ONE wait, before any arithmetic
+#pragma unroll
+    for (int ch = 0; ch < NCH; ++ch) BF_TMEM_LD_32x32b_X32(taddr + 32 * ch, vv[ch]);
+    tc_wait_ld();
+    tc_fence_before();
+    __syncwarp();
+    if (lane0) mbar_arrive(bar_empty);
+  }
 #pragma unroll
   for (int ch = 0; ch < NCH; ++ch) {
-    uint32_t v[32];
-    BF_TMEM_LD_32x32b_X32(taddr + 32 * ch, v);
-    tc_wait_ld();
-    if (ch == NCH - 1) {  // all of this warp's columns are in registers: release the stage
-      tc_fence_before();
-      __syncwarp();
-      if (lane0) mbar_arrive(bar_empty);
+    uint32_t (&v)[32] = vv[UPFRONT ? ch : 0];
+    if constexpr (!UPFRONT) {
+      BF_TMEM_LD_32x32b_X32(taddr + 32 * ch, v);
+      tc_wait_ld();
+      if (ch == NCH - 1) {  // all of this warp's columns are in registers: release the stage
+        tc_fence_before();
+        __syncwarp();
+        if (lane0) mbar_arrive(bar_empty);
+      }
     }
 #pragma unroll
     for (int s = 0; s < NSUB; ++s) {

@@ -104,6 +104,7 @@ bf_umma_i8_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(s_tmem));
   tmem_base = __shfl_sync(0xffffffffu, tmem_base, 0);
+  probe_mark(p.probe, 0);
 
   // this CTA's contiguous range of super-tiles (super-tile = G tiles of 128 samples = 4 bins of 32 G samples,
   // or 128 / nint bins for nint <= 32)
@@ -247,6 +248,7 @@ bf_umma_i8_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
   tc_fence_before();
   __syncthreads();
   if (warp == L_MMA_WARP) tmem_dealloc(tmem_base, 512);
+  probe_mark(p.probe, 1);
 }
 
 // ---- WIDE variant (nant = 32 exactly, nsamp even): shared-memory rows of 128 bytes = TWO samples --------------
@@ -293,6 +295,7 @@ bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(s_tmem));
   tmem_base = __shfl_sync(0xffffffffu, tmem_base, 0);
+  probe_mark(p.probe, 0);
 
   const long long s0 = total_super * blockIdx.x / gridDim.x;
   const long long s1 = total_super * (blockIdx.x + 1) / gridDim.x;
@@ -495,6 +498,7 @@ bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
   tc_fence_before();
   __syncthreads();
   if (warp == L_MMA_WARP) tmem_dealloc(tmem_base, 512);
+  probe_mark(p.probe, 1);
 }
 
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,

@@ -75,6 +75,7 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(s_tmem));
   tmem_base = __shfl_sync(0xffffffffu, tmem_base, 0);
+  probe_mark(p.probe, 0);
 
   const long long it0 = blockIdx.x, it_step = gridDim.x;  // round-robin item assignment
   const int n_items = (int)((total_items - it0 + it_step - 1) / it_step);
@@ -217,6 +218,7 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
   tc_fence_before();
   __syncthreads();
   if (warp == MMA_WARP) tmem_dealloc(tmem_base, 512);
+  probe_mark(p.probe, 1);
 }
 
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,

@@ -21,6 +21,16 @@ BF_DEVI bool elect_one() {
   return pred != 0;
 }
 
+// bf_set_clock_probe: CTA 0 stamps (clock64, globaltimer) at slot 0 = kernel start, 1 = kernel end
+BF_DEVI void probe_mark(unsigned long long *probe, int slot) {
+  if (probe != nullptr && blockIdx.x == 0 && threadIdx.x == 0) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    probe[2 * slot] = (unsigned long long)clock64();
+    probe[2 * slot + 1] = t;
+  }
+}
+
 // ---- mbarrier ----------------------------------------------------------------------------------
 BF_DEVI void mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
@@ -76,16 +86,31 @@ BF_DEVI bool mbar_try_wait_hint(uint32_t bar, uint32_t parity, uint32_t ns) {
 }
 // Bounded wait: a mis-phased pipeline must fail (trap), not hang the GPU.  The poll loop is two
 // instructions; the clock is looked at once per 4096 polls and the wait gives up after ~2 s.
+#ifndef BF_WAIT_HINT_NS
+#define BF_WAIT_HINT_NS 0
+#endif
 BF_DEVI void mbar_wait(uint32_t bar, uint32_t parity) {
+#if BF_WAIT_HINT_NS > 0
+  if (mbar_try_wait_hint(bar, parity, BF_WAIT_HINT_NS)) return;
+#else
   if (mbar_try_wait(bar, parity)) return;
+#endif
   const long long t0 = clock64();
   for (;;) {
 #pragma unroll 1
-    for (int k = 0; k < 4096; ++k)
+    for (int k = 0; k < 4096; ++k) {
+#if BF_WAIT_HINT_NS > 0
+      if (mbar_try_wait_hint(bar, parity, BF_WAIT_HINT_NS)) return;
+#else
       if (mbar_try_wait(bar, parity)) return;
-    if (clock64() - t0 > 4000000000LL) asm volatile("trap;");
+#endif
+    }
+    // ~20 s at 2 GHz: long enough for a time-sliced or profiled GPU, short enough to fail instead of hanging
+    if (clock64() - t0 > 40000000000LL) asm volatile("trap;");
   }
 }
+template <int N> BF_DEVI void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> BF_DEVI void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 
 // ---- tcgen05 -----------------------------------------------------------------------------------
 BF_DEVI void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }

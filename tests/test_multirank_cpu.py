@@ -84,3 +84,27 @@ def test_single_process_aggregate_is_identity():
     import bench
     assert bench.aggregate(3.5, 7.0) == (3.5, 7.0)
     assert bench.rank_seed(1, 0) == 1 and bench.rank_seed(1, 3) == 301
+
+
+def test_bench_gpus_flag_starts_the_ranks_itself():
+    """`python bench.py --gpus 2` with no torchrun environment must start two ranks:
+    the launcher path is driven end to end with gloo ranks that do no GPU work (--selftest-launcher)."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--selftest-launcher"],
+                       capture_output=True, text=True, timeout=300, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [json.loads(ln) for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1                          # rank 0 alone prints
+    d = lines[0]
+    assert d["n_gpus"] == 2 and d["requested_gpus"] == 2
+    assert d["max_ms"] == 2.0 and d["units"] == 3.0  # max over ranks of (rank + 1) ms, sum of (rank + 1) units
+
+
+def test_launcher_command_shape():
+    import bench
+    cmd = bench.launcher_command(4, ["--gpus", "4", "--steps", "2"], port=29999)
+    assert cmd[1:3] == ["-m", "torch.distributed.run"] and "--nproc-per-node=4" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29999"
+    assert cmd[-4:] == ["--gpus", "4", "--steps", "2"] and cmd[-5].endswith("bench.py")
