@@ -25,6 +25,7 @@
 // (MMA <-> epilogue).
 #include <type_traits>
 
+#include "bf_tmap.h"
 #include "bf_umma_common.cuh"
 
 namespace {
@@ -33,22 +34,7 @@ using namespace bfk;
 
 constexpr int MAX_INPUT_PIECES = TILE_T * 4;  // 16-byte input pieces per tile at nant = 32
 
-// BF_K64_UPFRONT: the epilogue warps request all their TMEM columns of a tile at once (64 registers of data) and
-// hand the accumulator stage back after one wait.  The registers come from the other roles: 28 warps are launched
-// at 72 registers, the four epilogue warpgroups grow to 96, the convert / MMA / TMA warpgroups shrink to 40
-// (setmaxnreg; 16*32*96 + 12*32*40 = 28*32*72).
-#ifndef BF_K64_UPFRONT
-#define BF_K64_UPFRONT 1
-#endif
-#ifndef BF_K64_EPI_REGS
-#define BF_K64_EPI_REGS 96
-#endif
-#ifndef BF_K64_OTHER_REGS
-#define BF_K64_OTHER_REGS 40
-#endif
-template <bool SPREAD> constexpr bool upfront_v = BF_K64_UPFRONT && !SPREAD;
-template <bool SPREAD, int CONV_WARPS> constexpr int k64_threads_v =
-    SPREAD ? 1024 : (upfront_v<SPREAD> ? (EPI_WARPS + CONV_WARPS + 4) * 32 : (EPI_WARPS + CONV_WARPS + 3) * 32);
+template <bool SPREAD, int CONV_WARPS> constexpr int k64_threads_v = SPREAD ? 1024 : (EPI_WARPS + CONV_WARPS + 3) * 32;
 
 struct Item { int c, g, tt; };
 
@@ -96,12 +82,18 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   // runs on the uniform datapath: descriptors in uniform registers, no per-lane waterfall loops)
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
   // role table: cw = convert-warp index (0..7) or -1, mw = MMA-warp index (0/1) or -1
-  int cw = -1, mw = -1;
+  int cw = -1, mw = -1, ew = -1;     // ew = epilogue-warp index (0..15) or -1
   bool is_tma = false;
-  if (!SPREAD) {  // warps 16-23 convert, 24/25 MMA, 26 TMA
-    if (warp >= EPI_WARPS && warp < EPI_WARPS + 8) cw = warp - EPI_WARPS;
-    else if (warp == EPI_WARPS + 8 || warp == EPI_WARPS + 9) mw = warp - (EPI_WARPS + 8);
-    else if (warp == EPI_WARPS + 10) is_tma = true;
+  if (!SPREAD) {
+    // The warp scheduler favours the higher warp index among eligible warps, and the epilogue warps are the chain
+    // everything else waits for: convert warps sit at the bottom (0-7), the epilogue above them (8-23; 8 % 4 == 0, so
+    // warp & 3 is still the TMEM lane quadrant), the MMA and TMA warps on top (24-26).
+    if (warp < 8) cw = warp;
+    else if (warp < 8 + EPI_WARPS) ew = warp - 8;
+    else if (warp < 8 + EPI_WARPS + 2) mw = warp - (8 + EPI_WARPS);
+    else if (warp == 8 + EPI_WARPS + 2) is_tma = true;
+  } else if (warp < EPI_WARPS) {
+    ew = warp;
   } else if (warp >= EPI_WARPS && (warp & 3) != 0) {  // 32 warps; nothing but epilogue on sub-partition 0
     const int r = (warp - EPI_WARPS) >> 2, q = warp & 3;   // r = 0..3, q = 1..3
     if (r < 3) { const int k = r * 3 + (q - 1); if (k < 8) cw = k; }   // 17,18,19,21,22,23,25,26
@@ -136,12 +128,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   const int n_items = (int)(it1 - it0);
   const int nMt = p.nMt;
 
-  constexpr bool UPF = upfront_v<SPREAD>;
-  if constexpr (UPF) {  // whole warpgroups (4 warps) move registers: 0-3 epilogue, 4-6 everything else
-    if (warp < EPI_WARPS) setmaxnreg_inc<BF_K64_EPI_REGS>();
-    else setmaxnreg_dec<BF_K64_OTHER_REGS>();
-  }
-  if (warp < EPI_WARPS) {
+  if (ew >= 0) {
     // =========================================================================== epilogue
     // 16 warps: warp w owns TMEM lanes 32*(w&3).. and columns 64*(w>>2).. of EVERY accumulator tile.
     // The TMEM stage is handed back to the MMA warp as soon as this warp's last tcgen05.ld has
@@ -152,7 +139,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     // tile m of an item uses stage m & 1 (GROUP even), item i uses stage i & 1 (GROUP == 1).
     constexpr int BPW = NINT_T == 0 ? 1 : 64 / NINT_T;       // bins per warp and tile
     constexpr int BPT = NINT_T == 0 ? 0 : TILE_T / NINT_T;   // bins per tile
-    const int quad = warp & 3, slot = warp >> 2;
+    const int quad = ew & 3, slot = ew >> 2;
     const bool lane0 = lane == 0;
     uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16) + slot * 64;
     uint32_t b_full = bar_t_full;
@@ -166,6 +153,9 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     Item it = decode_item(it0, nG, nTt);
     uint32_t par0 = 0, par1 = 0;                             // parity of the next completion of t_full[0/1]
     int i = 0;
+    constexpr bool DEFER = !BEAMS;
+    EpiPend<NINT_T> pend;
+    epi_pend_init<NINT_T>(pend);
     while (i < n_items) {
       // ---- one run: the items of one (chan, beam group) inside my range; time tiles it.tt ..
       const int run = min(n_items - i, nTt - it.tt);
@@ -186,7 +176,34 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
       for (int m = 0; m < GROUP; ++m)
         if (m < gm && beam0 + m * BF_TILE_BEAMS < nbeam) bok |= 1u << m;
       int tt = it.tt;
-      for (int k = 0; k < run; ++k, ++i, ++tt, ptr += BPT, bptr += TILE_T) {
+      int k = 0;
+      if constexpr (DEFER && NINT_T != 0 && EpiPend<NINT_T>::DEFER) {
+        // ---- lean loop: the interior of a run (every quadrant holds real rows, every bin of the tile exists).  The
+        // kernel's time follows the instructions the SM sub-partitions issue (profiles/), and the general loop below
+        // spends more of them on predicates, pointer arithmetic and re-convergence than on squares; here a tile is
+        // wait -> tcgen05.ld x2 -> 32 FFMA2 -> add tree, with everything else hoisted to the run.
+        const bool all_rows = rows == (1u << GROUP) - 1;       // implies gm == GROUP
+        const int n_lean = all_rows ? ((ragged && it.tt + run == nTt) ? run - 1 : run) : 0;
+        bool wrm[GROUP];
+#pragma unroll
+        for (int m = 0; m < GROUP; ++m) wrm[m] = (wr >> m) & 1;
+        const bool vec = vec_ok;
+        for (; k < n_lean; ++k, ++i, ptr += BPT) {
+#pragma unroll
+          for (int m = 0; m < GROUP; ++m) {
+            const uint32_t acc = GROUP == 1 ? (uint32_t)(i & 1) : (uint32_t)(m & 1);
+            uint32_t par;
+            if (GROUP == 1) { par = acc ? par1 : par0; if (acc) par1 ^= 1; else par0 ^= 1; }
+            else if (m & 1) { par = par1; par1 ^= 1; }
+            else { par = par0; par0 ^= 1; }
+            mbar_wait_tight(b_full + 8 * acc, par);
+            tc_fence_after();
+            epilogue_tile_defer<NINT_T>(t_lane + acc * TILE_T, ptr + m * mstride, wrm[m], 1 << 30, vec, b_full + 16 + 8 * acc, lane0, pend);
+          }
+        }
+        tt += n_lean;
+      }
+      for (; k < run; ++k, ++i, ++tt, ptr += BPT, bptr += TILE_T) {
         int nvalid = 1 << 30;
         float *out = ptr;
         if (BEAMS) {
@@ -201,7 +218,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         auto one = [&](auto acc_c, int m) {
           constexpr int ACC = decltype(acc_c)::value;
           uint32_t &par = ACC ? par1 : par0;
-          mbar_wait(b_full + 8 * ACC, par);
+          mbar_wait_tight(b_full + 8 * ACC, par);
           par ^= 1;
           tc_fence_after();
           if (!((rows >> m) & 1)) {                          // warp-uniform: only padding rows in this quadrant
@@ -211,9 +228,12 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
           if constexpr (BEAMS)
             epilogue_beams_tile(t_lane + ACC * TILE_T, bptr + (size_t)m * BF_TILE_BEAMS * p.nsamp, (bok >> m) & 1, nvalid,
                                 bvec_ok, p.beam_scale, lane >= 16, b_full + 16 + 8 * ACC, lane0);
+          else if constexpr (DEFER)
+            epilogue_tile_defer<NINT_T>(t_lane + ACC * TILE_T, out + m * mstride, (wr >> m) & 1, nvalid, NINT_T != 0 && vec_ok,
+                                        b_full + 16 + 8 * ACC, lane0, pend);
           else
-            epilogue_tile<NINT_T, UPF>(t_lane + ACC * TILE_T, out + m * mstride, (wr >> m) & 1, nvalid, NINT_T != 0 && vec_ok,
-                                       b_full + 16 + 8 * ACC, lane0);
+            epilogue_tile<NINT_T>(t_lane + ACC * TILE_T, out + m * mstride, (wr >> m) & 1, nvalid, NINT_T != 0 && vec_ok,
+                                  b_full + 16 + 8 * ACC, lane0);
         };
         if constexpr (GROUP == 1) {
           if (i & 1) one(std::integral_constant<int, 1>{}, 0);
@@ -230,6 +250,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
       it.tt = 0;
       if (++it.g == nG) { it.g = 0; ++it.c; }
     }
+    if constexpr (DEFER) epi_pend_flush<NINT_T>(pend);     // the tail of this CTA's last tile
   } else if (cw >= 0) {
     // =========================================================================== convert
     // 16-byte input pieces per thread per tile: int8 rows are 2*nant bytes, 4-bit rows nant bytes
@@ -271,17 +292,12 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         const int rs = i % NRAW, st = i % NSTAGE;
         const uint32_t raw = raw0 + rs * RAW_STAGE_BYTES, dst = dst0 + st * B_STAGE_BYTES;
         mbar_wait(bar_r_full + 8 * rs, (uint32_t)((i / NRAW) & 1));
-        constexpr int RP = UPF ? 4 : GP;   // pieces per round (a round's pieces live in registers: 40-register budget)
-        uint4 x[RP];
+        constexpr int RP = GP, r0 = 0;
+        uint4 x[GP];
 #pragma unroll
-        for (int k = 0; k < RP; ++k) x[k] = ld_shared_v4(raw + k * (16 * GT));
+        for (int k = 0; k < GP; ++k) x[k] = ld_shared_v4(raw + k * (16 * GT));
         mbar_wait(bar_b_empty + 8 * st, (uint32_t)(((i / NSTAGE) & 1) ^ 1));
-#pragma unroll
-        for (int r0 = 0; r0 < GP; r0 += RP) {
-          if (r0 > 0) {
-#pragma unroll
-            for (int k = 0; k < RP; ++k) x[k] = ld_shared_v4(raw + (r0 + k) * (16 * GT));
-          }
+        {
           if (IN == BF_CI4) {
             const uint32_t d1 = dst ^ 16u, d2 = dst ^ 32u, d3 = dst ^ 48u;
 #pragma unroll
@@ -426,7 +442,8 @@ cudaError_t launch_k64(const BfParams &p, int sm_count, cudaStream_t st) {
   const int nks = (2 * p.nant + 15) / 16;
   const size_t smem = 1024 + 2 * GROUP * A_TILE_BYTES + NSTAGE * B_STAGE_BYTES + NRAW * RAW_STAGE_BYTES + 256;
   auto kern = bf_umma_k64_kernel<NINT_T, GROUP, NSTAGE, NRAW, CONV_WARPS, SPREAD, IN, BEAMS>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  static thread_local int attr_dev = -1;   // once per instantiation and device
+  cudaError_t e = bf_set_smem_once(kern, smem, &attr_dev);
   if (e != cudaSuccess) return e;
   if (NINT_T == 0 && !BEAMS) {
     e = cudaMemsetAsync(p.pow, 0, (size_t)p.nchan_run * p.nbeam * p.nbin * sizeof(float), st);

@@ -104,7 +104,7 @@ __device__ __forceinline__ void convert_store_ci4(uint32_t s_dst, const uint32_t
 // that it can be hoisted out of the tile loop.
 // NINT_T: integration length if a power of two <= 64; 0 = a larger multiple of 64: the partial sum of
 // the warp's 64 columns is added atomically into the (zeroed) bin `out` points at.
-template <int NINT_T, bool UPFRONT = false>
+template <int NINT_T>
 __device__ __forceinline__ void epilogue_tile(uint32_t taddr, float *out, bool writer, int nvalid, bool vec_ok,
                                               uint32_t bar_empty, bool lane0) {
   constexpr int CPW = TILE_T / (EPI_WARPS / 4);                          // columns per warp (64)
@@ -119,28 +119,15 @@ __device__ __forceinline__ void epilogue_tile(uint32_t taddr, float *out, bool w
   float2 a[NACC];  // packed running sums of squares; live across the chunks of one bin
 #pragma unroll
   for (int q = 0; q < NACC; ++q) a[q] = make_float2(0.f, 0.f);
-  uint32_t vv[UPFRONT ? NCH : 1][32];
-  if constexpr (UPFRONT) {
-    // the accumulator ring is the critical loop (MMA -> commit -> tcgen05.ld -> arrive -> next MMA): request ALL of this
-    // warp's columns at once and hand the stage back after ONE wait, before any arithmetic
-#pragma unroll
-    for (int ch = 0; ch < NCH; ++ch) BF_TMEM_LD_32x32b_X32(taddr + 32 * ch, vv[ch]);
-    tc_wait_ld();
-    tc_fence_before();
-    __syncwarp();
-    if (lane0) mbar_arrive(bar_empty);
-  }
 #pragma unroll
   for (int ch = 0; ch < NCH; ++ch) {
-    uint32_t (&v)[32] = vv[UPFRONT ? ch : 0];
-    if constexpr (!UPFRONT) {
-      BF_TMEM_LD_32x32b_X32(taddr + 32 * ch, v);
-      tc_wait_ld();
-      if (ch == NCH - 1) {  // all of this warp's columns are in registers: release the stage
-        tc_fence_before();
-        __syncwarp();
-        if (lane0) mbar_arrive(bar_empty);
-      }
+    uint32_t v[32];
+    BF_TMEM_LD_32x32b_X32(taddr + 32 * ch, v);
+    tc_wait_ld();
+    if (ch == NCH - 1) {  // all of this warp's columns are in registers: release the stage
+      tc_fence_before();
+      __syncwarp();
+      if (lane0) mbar_arrive(bar_empty);
     }
 #pragma unroll
     for (int s = 0; s < NSUB; ++s) {
@@ -177,6 +164,102 @@ __device__ __forceinline__ void epilogue_tile(uint32_t taddr, float *out, bool w
         }
       }
     }
+  }
+}
+// ---- deferred tail ----------------------------------------------------------------------------------------------
+// The epilogue warps are the critical chain of the resident kernel (profiles/: busy ~90 % of the time while every
+// other role waits), and a fifth of that chain was the tail of each tile: add tree -> SHFL -> FADD -> STG, the FADD
+// stalled on the shuffle, which queues behind the other warps' tcgen05.ld / LDS / STS in the same memory pipe.
+// Here the tail of tile i is carried into tile i+1 and issued right after that tile's first tcgen05.ld, so its
+// latency hides under the load.  EpiPend = the per-lane bin sums of the previous tile (re^2 and im^2 rows still
+// apart), where they go, and whether this lane stores them.
+template <int NINT_T>
+struct EpiPend {
+  static constexpr int NBIN = NINT_T == 0 ? 1 : (TILE_T / (EPI_WARPS / 4)) / NINT_T;   // bins per warp and tile
+  static constexpr bool DEFER = NBIN <= 4;
+  float s[DEFER ? NBIN : 1];
+  float *out;
+  int nvalid;
+  bool writer, vec;
+};
+template <int NINT_T>
+__device__ __forceinline__ void epi_pend_init(EpiPend<NINT_T> &pd) {
+#pragma unroll
+  for (int j = 0; j < (EpiPend<NINT_T>::DEFER ? EpiPend<NINT_T>::NBIN : 1); ++j) pd.s[j] = 0.f;
+  pd.out = nullptr; pd.nvalid = 0; pd.writer = false; pd.vec = false;
+}
+template <int NINT_T>
+__device__ __forceinline__ void epi_pend_flush(EpiPend<NINT_T> &pd) {
+  constexpr int NBIN = EpiPend<NINT_T>::NBIN;
+  if constexpr (EpiPend<NINT_T>::DEFER) {
+    float tot[NBIN];
+#pragma unroll
+    for (int j = 0; j < NBIN; ++j) tot[j] = pd.s[j] + __shfl_xor_sync(0xffffffffu, pd.s[j], 16);  // re^2 rows + im^2 rows
+    if (NINT_T == 0) {
+      if (pd.writer && pd.nvalid > 0) atomicAdd(pd.out, tot[0]);
+    } else if (NBIN == 4 && pd.vec) {
+      if (pd.writer && pd.nvalid >= 4) *reinterpret_cast<float4 *>(pd.out) = make_float4(tot[0], tot[1], tot[2], tot[3]);
+      else if (pd.writer) {
+#pragma unroll
+        for (int j = 0; j < NBIN; ++j) if (j < pd.nvalid) pd.out[j] = tot[j];
+      }
+    } else if (pd.writer) {
+#pragma unroll
+      for (int j = 0; j < NBIN; ++j) if (j < pd.nvalid) pd.out[j] = tot[j];
+    }
+    pd.writer = false;
+  }
+}
+// One accumulator tile for one warp, tail deferred (see above).  Same contract as epilogue_tile; `pd` carries the
+// previous tile's tail in and this tile's tail out.  Bins of <= 8 samples (more than 4 bins per warp) fall back to
+// the immediate form.
+template <int NINT_T>
+__device__ __forceinline__ void epilogue_tile_defer(uint32_t taddr, float *out, bool writer, int nvalid, bool vec_ok,
+                                                    uint32_t bar_empty, bool lane0, EpiPend<NINT_T> &pd) {
+  if constexpr (!EpiPend<NINT_T>::DEFER) {
+    epilogue_tile<NINT_T>(taddr, out, writer, nvalid, vec_ok, bar_empty, lane0);
+  } else {
+    constexpr int CPW = TILE_T / (EPI_WARPS / 4);
+    constexpr int NCH = CPW / 32;
+    constexpr int SUB = (NINT_T == 0 || NINT_T > 32) ? 32 : NINT_T;
+    constexpr int NSUB = 32 / SUB;
+    constexpr int CPB = NINT_T == 0 ? NCH : (NINT_T <= 32 ? 1 : NINT_T / 32);
+    constexpr int NACC = SUB >= 8 ? 4 : (SUB >= 2 ? SUB / 2 : 1);
+    float2 a[NACC];
+#pragma unroll
+    for (int q = 0; q < NACC; ++q) a[q] = make_float2(0.f, 0.f);
+    float sums[EpiPend<NINT_T>::NBIN];
+#pragma unroll
+    for (int ch = 0; ch < NCH; ++ch) {
+      uint32_t v[32];
+      BF_TMEM_LD_32x32b_X32(taddr + 32 * ch, v);
+      if (ch == 0) epi_pend_flush<NINT_T>(pd);   // the previous tile's shuffles and stores, under this load
+      tc_wait_ld();
+      if (ch == NCH - 1) {  // all of this warp's columns are in registers: release the stage
+        tc_fence_before();
+        __syncwarp();
+        if (lane0) mbar_arrive(bar_empty);
+      }
+#pragma unroll
+      for (int s = 0; s < NSUB; ++s) {
+#pragma unroll
+        for (int j = 0; j < SUB / 2; ++j) {
+          const float2 d = make_float2(__uint_as_float(v[s * SUB + 2 * j]), __uint_as_float(v[s * SUB + 2 * j + 1]));
+          a[j % NACC] = ffma2(d, d, a[j % NACC]);
+        }
+        if (CPB > 1 && (ch + 1) % CPB != 0) continue;  // bin continues in the next chunk
+#pragma unroll
+        for (int w = NACC / 2; w >= 1; w >>= 1)        // packed add tree
+#pragma unroll
+          for (int q = 0; q < w; ++q) a[q] = fadd2(a[q], a[q + w]);
+        sums[NINT_T == 0 ? 0 : (ch / CPB) * NSUB + s] = a[0].x + a[0].y;
+#pragma unroll
+        for (int q = 0; q < NACC; ++q) a[q] = make_float2(0.f, 0.f);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < EpiPend<NINT_T>::NBIN; ++j) pd.s[j] = sums[j];
+    pd.out = out; pd.nvalid = nvalid; pd.writer = writer; pd.vec = vec_ok;
   }
 }
 // Voltage-beam epilogue ("electric-field ... beams ... output as 16-bit complex-valued

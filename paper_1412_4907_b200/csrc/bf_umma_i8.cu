@@ -30,6 +30,7 @@
 #include <cuda.h>
 
 #include "bf_internal.h"
+#include "bf_tmap.h"
 #include "ptx.cuh"
 
 namespace {
@@ -315,6 +316,8 @@ bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
       if (lane & (LB >> (k + 1))) beam_off += 8 >> (k + 1);
     const bool writer = (lane & ((LB >> HALVINGS) - 1)) == 0;
     const int nbeam = p.nbeam, nbin = p.nbin;
+    // 8-byte stores (two samples per lane) need an 8-byte aligned output; nsamp is even in this variant
+    const bool vec8 = ((reinterpret_cast<uintptr_t>(BEAMS ? p.beams : (void *)p.pow)) & 7) == 0;
     int c = c0, sp = sp0;
     int ti = 0;                                                   // tile counter of this CTA (all roles count alike)
     for (int s = 0; s < n_super; ++s) {
@@ -345,9 +348,16 @@ bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
             const int io = ((int)u[4 * i + 1] << 7) + (int)u[4 * i + 3];
             const __half2 ye = __floats2half2_rn((float)re * sc, (float)im * sc);
             const __half2 yo = __floats2half2_rn((float)ro * sc, (float)io * sc);
-            if (8 * ch + i < nbeam && t < p.nsamp)
-              *reinterpret_cast<uint2 *>(yrow + (size_t)(8 * ch + i) * p.nsamp) =
-                  make_uint2(*reinterpret_cast<const uint32_t *>(&ye), *reinterpret_cast<const uint32_t *>(&yo));
+            if (8 * ch + i < nbeam && t < p.nsamp) {
+              __half2 *dst = yrow + (size_t)(8 * ch + i) * p.nsamp;
+              if (vec8) {
+                *reinterpret_cast<uint2 *>(dst) =
+                    make_uint2(*reinterpret_cast<const uint32_t *>(&ye), *reinterpret_cast<const uint32_t *>(&yo));
+              } else {  // output pointer only 4-byte aligned (bf.h allows it): two scalar stores
+                dst[0] = ye;
+                dst[1] = yo;
+              }
+            }
           }
         }
         ++ti;
@@ -397,9 +407,15 @@ bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
             for (int ch = 0; ch < NCH; ++ch)
 #pragma unroll
               for (int i = 0; i < 8; ++i)
-                if (8 * ch + i < nbeam)
-                  *reinterpret_cast<float2 *>(p.pow + ((size_t)c * nbeam + 8 * ch + i) * nbin + bin) =
-                      make_float2(acc[ch][i] * sc2, acc1[ch][i] * sc2);
+                if (8 * ch + i < nbeam) {
+                  float *dst = p.pow + ((size_t)c * nbeam + 8 * ch + i) * nbin + bin;
+                  if (vec8) {
+                    *reinterpret_cast<float2 *>(dst) = make_float2(acc[ch][i] * sc2, acc1[ch][i] * sc2);
+                  } else {  // powers pointer only 4-byte aligned: two scalar stores
+                    dst[0] = acc[ch][i] * sc2;
+                    dst[1] = acc1[ch][i] * sc2;
+                  }
+                }
           }
         } else {
           const int bin = (32 / LB) * (4 * sp + quad) + lane / LB;
@@ -501,47 +517,10 @@ bf_umma_i8w_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
   probe_mark(p.probe, 1);
 }
 
-typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-PFN_encodeTiled get_encode() {
-  static PFN_encodeTiled fn = nullptr;
-  if (!fn) {
-    void *ptr = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
-        qres == cudaDriverEntryPointSuccess)
-      fn = reinterpret_cast<PFN_encodeTiled>(ptr);
-  }
-  return fn;
-}
-
-// The tensor maps depend only on (pointer, nant, nsamp, nchan, view): a streaming caller alternates between a few
-// buffers, so the last few encodings are kept (host-side cost only; launch-bound shapes like `tiny` notice).
-struct TmapKey { const void *ptr; int nant, nsamp, nchan, wide, rows; };
-struct TmapSlot { TmapKey k; CUtensorMap tm; bool used; };
-thread_local TmapSlot g_tmaps[8];
-thread_local int g_tmap_next = 0;
-
-template <typename F>
-cudaError_t cached_tmap(CUtensorMap *tm, const BfParams &p, int wide, int rows, F make) {
-  const TmapKey k = {p.volt, p.nant, p.nsamp, p.nchan_run, wide, rows};
-  for (TmapSlot &s : g_tmaps)
-    if (s.used && s.k.ptr == k.ptr && s.k.nant == k.nant && s.k.nsamp == k.nsamp && s.k.nchan == k.nchan &&
-        s.k.wide == k.wide && s.k.rows == k.rows) { *tm = s.tm; return cudaSuccess; }
-  cudaError_t e = make(tm, p, rows);
-  if (e != cudaSuccess) return e;
-  TmapSlot &s = g_tmaps[g_tmap_next];
-  g_tmap_next = (g_tmap_next + 1) % 8;
-  s.k = k; s.tm = *tm; s.used = true;
-  return cudaSuccess;
-}
-
 // 3-D view of the int8 voltages as bytes: {2 nant, nsamp, nchan}; box {64, 32, 1}, 64-byte swizzle; bytes past
 // 2 nant and samples past nsamp are zero-filled
 cudaError_t make_tmap(CUtensorMap *tm, const BfParams &p, int box_rows) {
-  PFN_encodeTiled enc = get_encode();
+  PFN_encodeTiled enc = bf_get_encode();
   if (!enc) return cudaErrorNotSupported;
   cuuint64_t dims[3] = {(cuuint64_t)2 * p.nant, (cuuint64_t)p.nsamp, (cuuint64_t)p.nchan_run};
   cuuint64_t strides[2] = {dims[0], dims[0] * (cuuint64_t)p.nsamp};
@@ -555,7 +534,7 @@ cudaError_t make_tmap(CUtensorMap *tm, const BfParams &p, int box_rows) {
 
 // WIDE view: rows of 128 bytes = two samples of 32 antennas: {128, nsamp / 2, nchan}; box {128, box_rows, 1}, 128-byte swizzle
 cudaError_t make_tmap_wide(CUtensorMap *tm, const BfParams &p, int box_rows) {
-  PFN_encodeTiled enc = get_encode();
+  PFN_encodeTiled enc = bf_get_encode();
   if (!enc) return cudaErrorNotSupported;
   cuuint64_t dims[3] = {128, (cuuint64_t)p.nsamp / 2, (cuuint64_t)p.nchan_run};
   cuuint64_t strides[2] = {128, (cuuint64_t)64 * p.nsamp};
@@ -571,8 +550,8 @@ template <int NCOL, int LBIN, bool BEAMS = false>
 cudaError_t launch_i8w(const BfParams &p, int sm_count, cudaStream_t st) {
   constexpr int NST = 12;
   CUtensorMap tm, tm32;
-  cudaError_t e = cached_tmap(&tm, p, 1, 128, make_tmap_wide);
-  if (e == cudaSuccess) e = cached_tmap(&tm32, p, 1, 32, make_tmap_wide);
+  cudaError_t e = bf_cached_tmap(&tm, p, 1, 128, make_tmap_wide);
+  if (e == cudaSuccess) e = bf_cached_tmap(&tm32, p, 1, 32, make_tmap_wide);
   if (e != cudaSuccess) return e;
   const int G = BEAMS || p.nint <= 64 ? 1 : p.nint / 64;
   const int n_super_chan = (p.nsamp + 256 * G - 1) / (256 * G);
@@ -580,13 +559,7 @@ cudaError_t launch_i8w(const BfParams &p, int sm_count, cudaStream_t st) {
   const size_t smem = 1024 + 2 * NCOL * L_ROW_BYTES + NST * W_STAGE_BYTES + 1024;
   auto kern = bf_umma_i8w_kernel<NCOL, LBIN, NST, BEAMS>;
   static thread_local int attr_dev = -1;   // once per instantiation and device
-  int dev = 0;
-  cudaGetDevice(&dev);
-  if (attr_dev != dev) {
-    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    attr_dev = dev;
-  }
+  if ((e = bf_set_smem_once(kern, smem, &attr_dev)) != cudaSuccess) return e;
   const int grid = (int)(total < sm_count ? total : sm_count);
   kern<<<grid, L_THREADS + 32, smem, st>>>(p, tm, tm32, total, n_super_chan, G);
   return cudaGetLastError();
@@ -609,8 +582,8 @@ template <int NCOL, int LBIN>
 cudaError_t launch_i8(const BfParams &p, int sm_count, cudaStream_t st) {
   constexpr int NST = 24;
   CUtensorMap tm, tm32;
-  cudaError_t e = cached_tmap(&tm, p, 0, L_TILE_T, make_tmap);
-  if (e == cudaSuccess) e = cached_tmap(&tm32, p, 0, L_BOX_ROWS, make_tmap);
+  cudaError_t e = bf_cached_tmap(&tm, p, 0, L_TILE_T, make_tmap);
+  if (e == cudaSuccess) e = bf_cached_tmap(&tm32, p, 0, L_BOX_ROWS, make_tmap);
   if (e != cudaSuccess) return e;
   const int G = p.nint <= 32 ? 1 : p.nint / 32;
   const int n_super_chan = (p.nsamp + L_TILE_T * G - 1) / (L_TILE_T * G);
@@ -618,8 +591,8 @@ cudaError_t launch_i8(const BfParams &p, int sm_count, cudaStream_t st) {
   const int nks = (2 * p.nant + 31) / 32;
   const size_t smem = 1024 + 2 * NCOL * L_ROW_BYTES + NST * L_STAGE_BYTES + 1024;
   auto kern = bf_umma_i8_kernel<NCOL, LBIN, NST>;
-  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
+  static thread_local int attr_dev = -1;
+  if ((e = bf_set_smem_once(kern, smem, &attr_dev)) != cudaSuccess) return e;
   const int grid = (int)(total < sm_count ? total : sm_count);
   kern<<<grid, L_THREADS, smem, st>>>(p, tm, tm32, total, n_super_chan, G, nks);
   return cudaGetLastError();

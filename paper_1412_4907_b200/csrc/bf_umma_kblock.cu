@@ -19,6 +19,7 @@
 // would be live at once and DRAM traffic was 3-14x the algorithmic bytes).
 #include <cuda.h>
 
+#include "bf_tmap.h"
 #include "bf_umma_common.cuh"
 
 namespace {
@@ -221,25 +222,11 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
   probe_mark(p.probe, 1);
 }
 
-typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-PFN_encodeTiled get_encode() {
-  static PFN_encodeTiled fn = nullptr;
-  if (!fn) {
-    void *ptr = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
-        qres == cudaDriverEntryPointSuccess)
-      fn = reinterpret_cast<PFN_encodeTiled>(ptr);
-  }
-  return fn;
-}
-
 // 3-D view of the voltages: {K' elements, nsamp, nchan}, box {64, 256, 1}
-cudaError_t make_tmap(CUtensorMap *tm, const BfParams &p, int dtype) {
-  PFN_encodeTiled enc = get_encode();
+template <bool F16>
+cudaError_t make_tmap(CUtensorMap *tm, const BfParams &p, int) {
+  constexpr int dtype = F16 ? BF_CF16 : BF_CI8;
+  PFN_encodeTiled enc = bf_get_encode();
   if (!enc) return cudaErrorNotSupported;
   const bool f16 = dtype == BF_CF16;
   const cuuint64_t esz = f16 ? 2 : 1;
@@ -258,15 +245,15 @@ template <int NINT_T, bool IS_F16, bool BEAMS = false>
 cudaError_t launch_kb(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
   constexpr int NA = 3, NB = IS_F16 ? 3 : 2, NR = IS_F16 ? 0 : 3;
   CUtensorMap tm;
-  cudaError_t e = make_tmap(&tm, p, dtype);
+  cudaError_t e = bf_cached_tmap(&tm, p, IS_F16 ? 101 : 100, TILE_T, make_tmap<IS_F16>);
   if (e != cudaSuccess) return e;
   const int nG = (p.nMt + KB_GROUP - 1) / KB_GROUP;
   const int nTt = (p.nsamp + TILE_T - 1) / TILE_T;
   const long long total = (long long)p.nchan_run * nTt * nG;
   const size_t smem = 1024 + NA * A_STAGE_BYTES + NB * B_STAGE_BYTES + NR * RAW_STAGE_BYTES + 512;
   auto kern = bf_umma_kblock_kernel<NINT_T, IS_F16, NA, NB, NR, BEAMS>;
-  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
+  static thread_local int attr_dev = -1;   // once per instantiation and device
+  if ((e = bf_set_smem_once(kern, smem, &attr_dev)) != cudaSuccess) return e;
   if (NINT_T == 0 && !BEAMS) {
     e = cudaMemsetAsync(p.pow, 0, (size_t)p.nchan_run * p.nbeam * p.nbin * sizeof(float), st);
     if (e != cudaSuccess) return e;

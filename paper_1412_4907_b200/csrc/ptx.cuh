@@ -109,8 +109,30 @@ BF_DEVI void mbar_wait(uint32_t bar, uint32_t parity) {
     if (clock64() - t0 > 40000000000LL) asm volatile("trap;");
   }
 }
-template <int N> BF_DEVI void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
-template <int N> BF_DEVI void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+// Tight bounded wait for roles on the critical chain (the epilogue): two instructions per failed poll, trap after
+// 2^26 polls (a try_wait blocks for a hardware-defined slice, so this is seconds, not a hang).
+BF_DEVI void mbar_wait_tight(uint32_t bar, uint32_t parity) {
+  // four polls per trip of the bounding counter: a failed poll costs two issue slots, and every slot a waiting
+  // warp takes is one a working warp of the same sub-partition does not get
+  asm volatile(
+      "{\n\t.reg .pred p, q;\n\t.reg .u32 n;\n\tmov.u32 n, 0;\n"
+      "BFW_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra BFD_%=;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra BFD_%=;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra BFD_%=;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra BFD_%=;\n\t"
+      "add.u32 n, n, 1;\n\t"
+      "setp.lt.u32 q, n, 0x1000000;\n\t"
+      "@q bra BFW_%=;\n\t"
+      "trap;\n"
+      "BFD_%=:\n\t}" ::"r"(bar), "r"(parity)
+      : "memory");
+}
+
 
 // ---- tcgen05 -----------------------------------------------------------------------------------
 BF_DEVI void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -138,6 +160,29 @@ BF_DEVI void mma_f16_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_
       "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
       : "memory");
 }
+
+// D[tmem] (+)= A[tmem] * B[smem]: the A operand (M = 128 rows = TMEM lanes, 16 fp16 along K = 8 columns) read from
+// tensor memory, B from shared memory
+BF_DEVI void mma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+BF_DEVI void tc_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// 32 lanes x 32 consecutive 32-bit columns, registers -> TMEM: thread l of the warp writes lane (base lane + l)
+#define BF_TMEM_ST_32x32b_X32(taddr, r)                                                           \
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "                                     \
+               "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"                          \
+               "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"                 \
+               ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]),     \
+                 "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]),   \
+                 "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]),           \
+                 "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]),           \
+                 "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]),           \
+                 "r"(r[31])                                                                        \
+               : "memory")
 
 // Shared-memory matrix descriptor, K-major operand, 128-byte swizzle:
 //   bits [0,14) start address >> 4 | [16,30) leading byte offset >> 4 (unused for swizzled K-major,
