@@ -78,6 +78,7 @@ extern "C" bf_ctx *bf_create(int nant, int nchan, int nbeam, int nsamp, int nint
   c->have_events = false;
   c->nwbuf = 1; c->active = 0; c->pending = -1;
   c->geom_buf[0] = c->geom_buf[1] = nullptr; c->wop_buf[0] = c->wop_buf[1] = nullptr;
+  c->wop_lo_buf[0] = c->wop_lo_buf[1] = nullptr; c->d_wop_lo = nullptr;
   c->wop8_buf[0] = c->wop8_buf[1] = nullptr; c->d_wop8 = nullptr; c->d_i8scale = nullptr;
   c->have_wevents = false; c->used[0] = c->used[1] = false;
   c->d_probe = nullptr;
@@ -166,10 +167,11 @@ extern "C" const char *bf_kernel_name(const bf_ctx *c) {
 extern "C" long long bf_launch_count(const bf_ctx *c) { return c ? c->launches : 0; }
 
 static size_t wop_bytes(const bf_ctx *c) { return align_up((size_t)c->nchan * bf_wop_bytes_per_chan(c), BF_ALIGN); }
+static size_t wop_lo_bytes(const bf_ctx *c) { return c->nint < BF_LO_NINT ? wop_bytes(c) : 0; }
 
 extern "C" size_t bf_workspace_bytes(const bf_ctx *c) {
   if (!c) return 0;
-  return (size_t)c->nwbuf * (geom_bytes(c) + wop_bytes(c) + wop8_bytes(c));
+  return (size_t)c->nwbuf * (geom_bytes(c) + wop_bytes(c) + wop8_bytes(c) + wop_lo_bytes(c));
 }
 
 extern "C" int bf_set_weight_buffers(bf_ctx *c, int n) {
@@ -189,6 +191,7 @@ static void select_buffer(bf_ctx *c, int i) {
   c->d_gain = c->d_dir + 3 * (size_t)c->nbeam;
   c->d_i8scale = c->d_gain + 2 * (size_t)c->nchan * c->nant;
   c->d_wop = c->wop_buf[i];
+  c->d_wop_lo = c->wop_lo_buf[i];
   c->d_wop8 = c->wop8_buf[i];
 }
 
@@ -223,6 +226,8 @@ extern "C" int bf_set_workspace(bf_ctx *c, void *dev_ptr, size_t bytes) {
   for (int i = 0; i < c->nwbuf; ++i) {
     c->geom_buf[i] = p + (size_t)i * geom_bytes(c);
     c->wop_buf[i] = (__half *)(p + (size_t)c->nwbuf * geom_bytes(c) + (size_t)i * wop_bytes(c));
+    c->wop_lo_buf[i] = wop_lo_bytes(c) ? (__half *)(p + (size_t)c->nwbuf * (geom_bytes(c) + wop_bytes(c) + wop8_bytes(c)) + (size_t)i * wop_lo_bytes(c))
+                                       : nullptr;
     c->wop8_buf[i] = wop8_bytes(c) ? (signed char *)(p + (size_t)c->nwbuf * (geom_bytes(c) + wop_bytes(c)) + (size_t)i * wop8_bytes(c))
                                    : nullptr;
   }
@@ -380,7 +385,8 @@ extern "C" int bf_get_weights(bf_ctx *c, float *host_out, void *stream) {
   float *d = nullptr;  // verification helper: the one place the library allocates device memory itself
   cudaError_t e = cudaMalloc(&d, bytes);
   if (e != cudaSuccess) return cuda_fail(c, e, "cudaMalloc (bf_get_weights)");
-  e = bf_launch_decode_weights(c, d, st);
+  const char *why;
+  e = bf_launch_decode_weights(c, d, pick_kernel(c, BF_MODE_POWER, &why) == BF_KERNEL_UMMA_I8, st);
   if (e == cudaSuccess) { c->launches += 1; e = cudaMemcpyAsync(host_out, d, bytes, cudaMemcpyDeviceToHost, st); }
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   cudaFree(d);
@@ -402,6 +408,7 @@ static int launch_range(bf_ctx *c, const void *volt, void *out, int chan0, int n
   p.beam_scale = scale;
   p.mode = mode;
   p.wop = c->d_wop + (size_t)chan0 * (bf_wop_bytes_per_chan(c) / sizeof(__half));
+  p.wop_lo = c->d_wop_lo ? c->d_wop_lo + (size_t)chan0 * (bf_wop_bytes_per_chan(c) / sizeof(__half)) : nullptr;
   p.wop8 = c->d_wop8 ? c->d_wop8 + (size_t)chan0 * bf_i8_ncol(c->nbeam) * 64 : nullptr;
   p.i8scale = c->d_i8scale + chan0;
   p.probe = c->d_probe;

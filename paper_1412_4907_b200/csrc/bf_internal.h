@@ -20,6 +20,12 @@
 // (chan, mt, kb) block is one contiguous 16 KiB K-major tile, stored as the exact shared-memory image
 // tcgen05.mma wants (128-byte swizzle: the 16-byte chunk index of a row is XORed with row & 7), so one
 // cp.async.bulk per tile brings it in with no fix-up.
+// Two-term coefficients: one fp16 rounding of a coefficient (|error| <= 2^-12) is independent from sample to
+// sample, so it averages out over a bin -- measured worst row 4.0e-4 of the bin mean at nint = 16, but 1.45e-3 at
+// nint = 1, above BASELINE.json's 1e-3.  Below BF_LO_NINT the generator therefore also stores the rounding
+// residual lo = fp16(a - fp16(a)) in a second operand plane of the same layout and every kernel contracts both
+// (hi + lo carries 22 bits); the extra MMAs hide under the output traffic, which dominates at such short bins.
+#define BF_LO_NINT 16
 #define BF_TILE_ROWS 128
 #define BF_TILE_BEAMS 64
 #define BF_KBLOCK 64
@@ -43,6 +49,7 @@ struct BfParams {
   float beam_scale;     // voltage-beam mode: y is multiplied by this before rounding to fp16
   int mode;             // BF_MODE_POWER (|y|^2 integrated over nint -> pow) or BF_MODE_BEAMS (y -> beams)
   const __half *wop;    // device, weight operand of the first channel of this launch
+  const __half *wop_lo; // second fp16 term of every coefficient (same layout), or NULL: see BF_LO_NINT
   const signed char *wop8;  // int8 two-limb weight operand of the first channel (bf_umma_i8.cu), or NULL
   const double *i8scale;    // per channel: y = (128 hi + lo) * i8scale[c]
   unsigned long long *probe;  // bf_set_clock_probe: 4 words written by CTA 0, or NULL
@@ -70,6 +77,8 @@ struct bf_ctx {
   bool have_gains;         // false = all ones (d_gain not read)
   std::vector<double> h_gain, h_i8scale;
   __half *d_wop;
+  __half *d_wop_lo;        // residual plane (nint < BF_LO_NINT), else NULL
+  __half *wop_lo_buf[2];
   signed char *d_wop8;     // int8 two-limb operand (NULL when the shape never takes the int8 kernel)
   double *d_i8scale;       // [nchan]
   bool have_geom;
@@ -97,7 +106,7 @@ size_t bf_wop_bytes_per_chan(const bf_ctx *c);
 
 // kernels (each returns a cudaError_t from the launch)
 cudaError_t bf_launch_weights(const bf_ctx *c, cudaStream_t st);
-cudaError_t bf_launch_decode_weights(const bf_ctx *c, float *d_out, cudaStream_t st);
+cudaError_t bf_launch_decode_weights(const bf_ctx *c, float *d_out, bool int8_operand, cudaStream_t st);
 cudaError_t bf_launch_simt(const BfParams &p, int dtype, cudaStream_t st);
 bool bf_umma_supported(const bf_ctx *c, const char **why);
 bool bf_umma_shape_supported(const bf_ctx *c, const char **why);  // ignoring nint (voltage-beam mode)

@@ -40,6 +40,7 @@ __global__ void __launch_bounds__(SIMT_BEAMS) bf_simt_kernel(BfParams p, int sam
   const int t_end = min(p.nsamp, t_begin + samples_per_block);
   const size_t wop_chan = (size_t)p.nMt * p.nKb * BF_TILE_ROWS * BF_KBLOCK;
   const __half *wc = p.wop + (size_t)c * wop_chan;
+  const __half *wl = p.wop_lo ? p.wop_lo + (size_t)c * wop_chan : nullptr;   // second coefficient term (BF_LO_NINT)
   float binacc = 0.f;
   for (int t0 = t_begin; t0 < t_end; t0 += SIMT_TT) {
     float2 acc[SIMT_TT];
@@ -64,6 +65,10 @@ __global__ void __launch_bounds__(SIMT_BEAMS) bf_simt_kernel(BfParams p, int sam
           size_t base = ((size_t)mt * p.nKb + kb) * (BF_TILE_ROWS * BF_KBLOCK);
           w.x = __half2float(wc[base + bf_tile_off(bf_beam_row(bt, 0), kk)]);
           w.y = __half2float(wc[base + bf_tile_off(bf_beam_row(bt, 1), kk)]);
+          if (wl) {
+            w.x += __half2float(wl[base + bf_tile_off(bf_beam_row(bt, 0), kk)]);
+            w.y += __half2float(wl[base + bf_tile_off(bf_beam_row(bt, 1), kk)]);
+          }
         }
         Ws[n][bl] = w;
       }

@@ -60,7 +60,9 @@ __device__ __forceinline__ void next_item(Item &it, int nG, int nTt) {
 // read by warps w with w % 4 == quadrant -- which all sit on SM sub-partition `quadrant`.  For <= 16
 // beams the whole epilogue therefore lands on sub-partition 0; SPREAD launches 32 warps and puts the
 // convert / MMA / TMA warps on sub-partitions 1-3 only, so that sub-partition 0 does nothing else.
-template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD, int IN, bool BEAMS>
+// LO: two-term coefficients (bf_internal.h, BF_LO_NINT): every coefficient buffer holds GROUP "hi" tiles followed by
+// GROUP "lo" tiles and a voltage tile is contracted against both (8 MMAs per accumulator tile instead of 4).
+template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD, int IN, bool BEAMS, bool LO>
 __global__ void __launch_bounds__(k64_threads_v<SPREAD, CONV_WARPS>, 1)
 bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, const int nTt, const int nks) {
   extern __shared__ uint8_t smem_raw[];
@@ -68,8 +70,9 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   static_assert(CONV_WARPS == 8, "role table below assumes 8 convert warps");
 
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t sA = smem_base;                                  // 2 buffers x GROUP coefficient tiles
-  const uint32_t sB = sA + 2 * GROUP * A_TILE_BYTES;              // NSTAGE fp16 operand stages
+  constexpr int APB = (LO ? 2 : 1) * GROUP;                       // coefficient tiles per buffer
+  const uint32_t sA = smem_base;                                  // 2 buffers x APB coefficient tiles
+  const uint32_t sB = sA + 2 * APB * A_TILE_BYTES;                // NSTAGE fp16 operand stages
   const uint32_t sR = sB + NSTAGE * B_STAGE_BYTES;                // NRAW raw int8 stages
   const uint32_t sBar = sR + NRAW * RAW_STAGE_BYTES;              // barriers
   const uint32_t bar_b_full = sBar, bar_b_empty = sBar + 8 * NSTAGE;
@@ -385,10 +388,16 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
           te_par ^= 1;
           tc_fence_after();
           if (elect_one()) {
-            const uint64_t adesc = adesc0 + (uint64_t)((ab * GROUP + m) * (A_TILE_BYTES >> 4));
+            const uint64_t adesc = adesc0 + (uint64_t)((ab * APB + m) * (A_TILE_BYTES >> 4));
 #pragma unroll
             for (int k = 0; k < 4; ++k)  // advance 16 fp16 = 32 bytes along K inside the swizzle atom
               if (k < nks) mma_f16_ss(d, adesc + 2 * k, bdesc + 2 * k, idesc, k > 0);
+            if constexpr (LO) {          // the residual term of the coefficients against the same voltages
+              const uint64_t ldesc = adesc + (uint64_t)(GROUP * (A_TILE_BYTES >> 4));
+#pragma unroll
+              for (int k = 0; k < 4; ++k)
+                if (k < nks) mma_f16_ss(d, ldesc + 2 * k, bdesc + 2 * k, idesc, 1);
+            }
             tc_commit(bar_t_full + 8 * id);
             if (m + 2 >= gm) {
               tc_commit(bar_b_empty + 8 * st);
@@ -414,8 +423,12 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         mbar_wait(bar_a_empty + 8 * ab, ((ag >> 1) & 1) ^ 1);
         const int gm = min(GROUP, nMt - it.g * GROUP);
         const char *wsrc = reinterpret_cast<const char *>(p.wop) + ((size_t)it.c * nMt + (size_t)it.g * GROUP) * A_TILE_BYTES;
-        mbar_arrive_expect_tx(bar_a_full + 8 * ab, gm * A_TILE_BYTES);
-        bulk_g2s(sA + ab * GROUP * A_TILE_BYTES, wsrc, gm * A_TILE_BYTES, bar_a_full + 8 * ab);
+        mbar_arrive_expect_tx(bar_a_full + 8 * ab, (LO ? 2 : 1) * gm * A_TILE_BYTES);
+        bulk_g2s(sA + ab * APB * A_TILE_BYTES, wsrc, gm * A_TILE_BYTES, bar_a_full + 8 * ab);
+        if constexpr (LO) {
+          const char *lsrc = reinterpret_cast<const char *>(p.wop_lo) + ((size_t)it.c * nMt + (size_t)it.g * GROUP) * A_TILE_BYTES;
+          bulk_g2s(sA + (ab * APB + GROUP) * A_TILE_BYTES, lsrc, gm * A_TILE_BYTES, bar_a_full + 8 * ab);
+        }
         ++ag;
       }
       const int rs = i % NRAW;
@@ -434,14 +447,14 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   probe_mark(p.probe, 1);
 }
 
-template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD, int IN, bool BEAMS = false>
+template <int NINT_T, int GROUP, int NSTAGE, int NRAW, int CONV_WARPS, bool SPREAD, int IN, bool BEAMS = false, bool LO = false>
 cudaError_t launch_k64(const BfParams &p, int sm_count, cudaStream_t st) {
   const int nG = (p.nMt + GROUP - 1) / GROUP;
   const int nTt = (p.nsamp + TILE_T - 1) / TILE_T;
   const long long total = (long long)p.nchan_run * nG * nTt;
   const int nks = (2 * p.nant + 15) / 16;
-  const size_t smem = 1024 + 2 * GROUP * A_TILE_BYTES + NSTAGE * B_STAGE_BYTES + NRAW * RAW_STAGE_BYTES + 256;
-  auto kern = bf_umma_k64_kernel<NINT_T, GROUP, NSTAGE, NRAW, CONV_WARPS, SPREAD, IN, BEAMS>;
+  const size_t smem = 1024 + 2 * (LO ? 2 : 1) * GROUP * A_TILE_BYTES + NSTAGE * B_STAGE_BYTES + NRAW * RAW_STAGE_BYTES + 256;
+  auto kern = bf_umma_k64_kernel<NINT_T, GROUP, NSTAGE, NRAW, CONV_WARPS, SPREAD, IN, BEAMS, LO>;
   static thread_local int attr_dev = -1;   // once per instantiation and device
   cudaError_t e = bf_set_smem_once(kern, smem, &attr_dev);
   if (e != cudaSuccess) return e;
@@ -456,6 +469,13 @@ cudaError_t launch_k64(const BfParams &p, int sm_count, cudaStream_t st) {
 
 template <int NINT_T, int IN>
 cudaError_t launch_k64_nint(const BfParams &p, int sm_count, cudaStream_t st) {
+  if constexpr (NINT_T != 0 && NINT_T < BF_LO_NINT) {
+    // short bins: two-term coefficients (the output stream, 4 bytes per beam and bin, hides the second set of MMAs)
+    if (p.wop_lo != nullptr) {
+      if (p.nMt == 1) return launch_k64<NINT_T, 1, 2, 4, 8, false, IN, false, true>(p, sm_count, st);
+      return launch_k64<NINT_T, 2, 2, 2, 8, false, IN, false, true>(p, sm_count, st);
+    }
+  }
   // <= 64 beams: HBM-bound.  A raw slot is held for the whole HBM latency plus the conversion (~3 us
   // measured), so the bytes in flight per SM decide the bandwidth: 8 raw slots of 16 KiB.
   if (p.nbeam <= 32) return launch_k64<NINT_T, 1, 2, 8, 8, true, IN>(p, sm_count, st);   // rows only in lane quadrants 0-1

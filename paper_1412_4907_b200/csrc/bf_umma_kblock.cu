@@ -32,7 +32,7 @@ constexpr int CONV_THREADS = CONV_WARPS * 32;
 constexpr int MMA_WARP = EPI_WARPS + CONV_WARPS;
 constexpr int TMA_WARP = MMA_WARP + 2;  // two MMA-issuing warps, one per accumulator
 constexpr int NTHREADS = (EPI_WARPS + CONV_WARPS + 3) * 32;
-constexpr int A_STAGE_BYTES = KB_GROUP * A_TILE_BYTES;
+template <bool LO> constexpr int a_stage_bytes_v = (LO ? 2 : 1) * KB_GROUP * A_TILE_BYTES;   // [hi tiles][lo tiles]
 
 struct KItem { int c, tt, g; };
 __device__ __forceinline__ KItem kdecode(long long idx, int nG, int nTt) {
@@ -44,13 +44,16 @@ __device__ __forceinline__ KItem kdecode(long long idx, int nG, int nTt) {
   return it;
 }
 
-template <int NINT_T, bool IS_F16, int NA, int NB, int NR, bool BEAMS>
+// LO: two-term coefficients (bf_internal.h, BF_LO_NINT): a coefficient stage holds the "hi" tiles followed by the "lo"
+// tiles of the K-block and every voltage K-block is contracted against both.
+template <int NINT_T, bool IS_F16, int NA, int NB, int NR, bool BEAMS, bool LO>
 __global__ void __launch_bounds__(NTHREADS, 1)
 bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, const long long total_items,
                       const int nG, const int nTt) {
   extern __shared__ uint8_t smem_raw[];
+  constexpr int A_STAGE_BYTES = a_stage_bytes_v<LO>;
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t sA = smem_base;                              // NA stages x 2 coefficient tiles
+  const uint32_t sA = smem_base;                              // NA stages x 2 (x 2) coefficient tiles
   const uint32_t sB = sA + NA * A_STAGE_BYTES;                // NB fp16 operand stages
   const uint32_t sR = sB + NB * B_STAGE_BYTES;                // NR raw int8 stages (int8 input only)
   const uint32_t sBar = sR + NR * RAW_STAGE_BYTES;
@@ -177,6 +180,11 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
             const uint64_t adesc = adesc0 + (uint64_t)(sa * (A_STAGE_BYTES >> 4));
 #pragma unroll
             for (int k = 0; k < 4; ++k) mma_f16_ss(d, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+            if constexpr (LO) {   // the residual term of the coefficients against the same voltage K-block
+              const uint64_t ldesc = adesc + (uint64_t)(KB_GROUP * (A_TILE_BYTES >> 4));
+#pragma unroll
+              for (int k = 0; k < 4; ++k) mma_f16_ss(d, ldesc + 2 * k, bdesc + 2 * k, idesc, 1);
+            }
             tc_commit(bar_a_empty + 8 * sa);
             tc_commit(bar_b_empty + 8 * sb);
             if (gm == 1) { tc_commit(bar_a_empty + 8 * sa); tc_commit(bar_b_empty + 8 * sb); }  // other warp idle
@@ -201,11 +209,14 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
       const int gm = min(KB_GROUP, nMt - it.g * KB_GROUP);
       for (int kb = 0; kb < nKb; ++kb) {
         mbar_wait(bar_a_empty + 8 * sa, apar);
-        mbar_arrive_expect_tx(bar_a_full + 8 * sa, gm * A_TILE_BYTES);
+        mbar_arrive_expect_tx(bar_a_full + 8 * sa, (LO ? 2 : 1) * gm * A_TILE_BYTES);
         for (int m = 0; m < gm; ++m) {
-          const char *src = reinterpret_cast<const char *>(p.wop) +
-                            (((size_t)it.c * nMt + (size_t)(it.g * KB_GROUP + m)) * nKb + kb) * A_TILE_BYTES;
-          bulk_g2s(sA + (sa * KB_GROUP + m) * A_TILE_BYTES, src, A_TILE_BYTES, bar_a_full + 8 * sa);
+          const size_t off = (((size_t)it.c * nMt + (size_t)(it.g * KB_GROUP + m)) * nKb + kb) * A_TILE_BYTES;
+          bulk_g2s(sA + sa * A_STAGE_BYTES + m * A_TILE_BYTES, reinterpret_cast<const char *>(p.wop) + off, A_TILE_BYTES,
+                   bar_a_full + 8 * sa);
+          if constexpr (LO)
+            bulk_g2s(sA + sa * A_STAGE_BYTES + (KB_GROUP + m) * A_TILE_BYTES, reinterpret_cast<const char *>(p.wop_lo) + off,
+                     A_TILE_BYTES, bar_a_full + 8 * sa);
         }
         mbar_wait(bar_v_empty + 8 * sv, vpar);
         mbar_arrive_expect_tx(bar_v_full + 8 * sv, VBYTES);
@@ -241,9 +252,10 @@ cudaError_t make_tmap(CUtensorMap *tm, const BfParams &p, int) {
   return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-template <int NINT_T, bool IS_F16, bool BEAMS = false>
+template <int NINT_T, bool IS_F16, bool BEAMS = false, bool LO = false>
 cudaError_t launch_kb(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
-  constexpr int NA = 3, NB = IS_F16 ? 3 : 2, NR = IS_F16 ? 0 : 3;
+  constexpr int NA = LO ? 2 : 3, NB = LO ? 2 : (IS_F16 ? 3 : 2), NR = IS_F16 ? 0 : (LO ? 2 : 3);
+  constexpr int A_STAGE_BYTES = a_stage_bytes_v<LO>;
   CUtensorMap tm;
   cudaError_t e = bf_cached_tmap(&tm, p, IS_F16 ? 101 : 100, TILE_T, make_tmap<IS_F16>);
   if (e != cudaSuccess) return e;
@@ -251,7 +263,7 @@ cudaError_t launch_kb(const BfParams &p, int dtype, int sm_count, cudaStream_t s
   const int nTt = (p.nsamp + TILE_T - 1) / TILE_T;
   const long long total = (long long)p.nchan_run * nTt * nG;
   const size_t smem = 1024 + NA * A_STAGE_BYTES + NB * B_STAGE_BYTES + NR * RAW_STAGE_BYTES + 512;
-  auto kern = bf_umma_kblock_kernel<NINT_T, IS_F16, NA, NB, NR, BEAMS>;
+  auto kern = bf_umma_kblock_kernel<NINT_T, IS_F16, NA, NB, NR, BEAMS, LO>;
   static thread_local int attr_dev = -1;   // once per instantiation and device
   if ((e = bf_set_smem_once(kern, smem, &attr_dev)) != cudaSuccess) return e;
   if (NINT_T == 0 && !BEAMS) {
@@ -266,6 +278,15 @@ cudaError_t launch_kb(const BfParams &p, int dtype, int sm_count, cudaStream_t s
 template <bool IS_F16>
 cudaError_t launch_kb_nint(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
   if (p.mode == BF_MODE_BEAMS) return launch_kb<64, IS_F16, true>(p, dtype, sm_count, st);
+  if (p.wop_lo != nullptr) {   // short bins: two-term coefficients
+    switch (p.nint) {
+      case 1: return launch_kb<1, IS_F16, false, true>(p, dtype, sm_count, st);
+      case 2: return launch_kb<2, IS_F16, false, true>(p, dtype, sm_count, st);
+      case 4: return launch_kb<4, IS_F16, false, true>(p, dtype, sm_count, st);
+      case 8: return launch_kb<8, IS_F16, false, true>(p, dtype, sm_count, st);
+      default: break;
+    }
+  }
   switch (p.nint) {
     case 1: return launch_kb<1, IS_F16>(p, dtype, sm_count, st);
     case 2: return launch_kb<2, IS_F16>(p, dtype, sm_count, st);

@@ -29,7 +29,7 @@ __device__ __forceinline__ void steering_weight(const double *__restrict__ ant, 
 
 __global__ void bf_weights_kernel(const double *__restrict__ ant, const double *__restrict__ freq,
                                   const double *__restrict__ dir, const double *__restrict__ gain,
-                                  __half *__restrict__ wop, int nant,
+                                  __half *__restrict__ wop, __half *__restrict__ wop_lo, int nant,
                                   int nchan, int nbeam, int nMt, int nKb) {
   // one thread per (chan, mt, row, n-slot) where n-slot covers the padded K' / 2
   const int npad = nKb * (BF_KBLOCK / 2);
@@ -44,16 +44,20 @@ __global__ void bf_weights_kernel(const double *__restrict__ ant, const double *
   int c = (int)(t / nMt);
   int b = bf_row_beam(mt, r);
   int part = bf_row_part(r);
-  float a0 = 0.f, a1 = 0.f;
+  double a0 = 0.0, a1 = 0.0;
   if (b < nbeam && n < nant) {
     double wre, wim;
     steering_weight(ant, freq, dir, gain, nant, c, b, n, wre, wim);
-    if (part == 0) { a0 = (float)wre; a1 = (float)(-wim); }
-    else           { a0 = (float)wim; a1 = (float)wre; }
+    if (part == 0) { a0 = wre; a1 = -wim; }
+    else           { a0 = wim; a1 = wre; }
   }
   int kb = (2 * n) / BF_KBLOCK, kk = (2 * n) % BF_KBLOCK;
   size_t o = (((size_t)c * nMt + mt) * nKb + kb) * (BF_TILE_ROWS * BF_KBLOCK) + bf_tile_off(r, kk);
-  *reinterpret_cast<__half2 *>(wop + o) = __floats2half2_rn(a0, a1);
+  const __half2 hi = __floats2half2_rn((float)a0, (float)a1);
+  *reinterpret_cast<__half2 *>(wop + o) = hi;
+  if (wop_lo)  // the rounding residual as a second fp16 term (bf_internal.h, BF_LO_NINT)
+    *reinterpret_cast<__half2 *>(wop_lo + o) =
+        __floats2half2_rn((float)(a0 - (double)__low2float(hi)), (float)(a1 - (double)__high2float(hi)));
 }
 
 // the same weights as two int8 limbs in the bf_umma_i8.cu operand layout (bf_internal.h); one thread per
@@ -89,7 +93,7 @@ cudaError_t bf_launch_weights(const bf_ctx *c, cudaStream_t st) {
   int threads = 256;
   long long blocks = (total + threads - 1) / threads;
   bf_weights_kernel<<<(unsigned)blocks, threads, 0, st>>>(c->d_ant, c->d_freq, c->d_dir,
-                                                          c->have_gains ? c->d_gain : nullptr, c->d_wop, c->nant,
+                                                          c->have_gains ? c->d_gain : nullptr, c->d_wop, c->d_wop_lo, c->nant,
                                                           c->nchan, c->nbeam, c->nMt, c->nKb);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess || !c->d_wop8) return e;
@@ -103,7 +107,8 @@ cudaError_t bf_launch_weights(const bf_ctx *c, cudaStream_t st) {
 }
 
 // operand layout -> logical fp32 [chan][beam][ant][2] (for bf_get_weights)
-__global__ void bf_decode_weights_kernel(const __half *__restrict__ wop, float *__restrict__ out, int nant,
+__global__ void bf_decode_weights_kernel(const __half *__restrict__ wop, const __half *__restrict__ wop_lo,
+                                         float *__restrict__ out, int nant,
                                          int nchan, int nbeam, int nMt, int nKb) {
   long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   long long total = (long long)nchan * nbeam * nant;
@@ -117,6 +122,10 @@ __global__ void bf_decode_weights_kernel(const __half *__restrict__ wop, float *
   size_t base = (((size_t)c * nMt + mt) * nKb + kb) * (BF_TILE_ROWS * BF_KBLOCK);
   float wre = __half2float(wop[base + bf_tile_off(bf_beam_row(bl, 0), kk)]);
   float wim = __half2float(wop[base + bf_tile_off(bf_beam_row(bl, 1), kk)]);
+  if (wop_lo) {
+    wre += __half2float(wop_lo[base + bf_tile_off(bf_beam_row(bl, 0), kk)]);
+    wim += __half2float(wop_lo[base + bf_tile_off(bf_beam_row(bl, 1), kk)]);
+  }
   out[2 * idx] = wre;
   out[2 * idx + 1] = wim;
 }
@@ -138,17 +147,17 @@ __global__ void bf_decode_weights_i8_kernel(const signed char *__restrict__ wop8
   out[2 * idx + 1] = (float)((128 * at(row0 + 1) + at(row0 + 3)) * scale[c]);
 }
 
-cudaError_t bf_launch_decode_weights(const bf_ctx *c, float *d_out, cudaStream_t st) {
+cudaError_t bf_launch_decode_weights(const bf_ctx *c, float *d_out, bool int8_operand, cudaStream_t st) {
   long long total = (long long)c->nchan * c->nbeam * c->nant;
   int threads = 256;
   long long blocks = (total + threads - 1) / threads;
-  if (c->d_wop8 && c->kernel_forced != BF_KERNEL_SIMT && c->kernel_forced != BF_KERNEL_UMMA_F16) {
-    // the int8 kernel is the one that runs: report ITS operand
+  if (int8_operand && c->d_wop8) {
+    // the int8 kernel is the one bf_run launches: report ITS operand
     bf_decode_weights_i8_kernel<<<(unsigned)blocks, threads, 0, st>>>(c->d_wop8, c->d_i8scale, d_out, c->nant, c->nchan,
                                                                       c->nbeam, bf_i8_ncol(c->nbeam));
     return cudaGetLastError();
   }
-  bf_decode_weights_kernel<<<(unsigned)blocks, threads, 0, st>>>(c->d_wop, d_out, c->nant, c->nchan, c->nbeam,
+  bf_decode_weights_kernel<<<(unsigned)blocks, threads, 0, st>>>(c->d_wop, c->d_wop_lo, d_out, c->nant, c->nchan, c->nbeam,
                                                                  c->nMt, c->nKb);
   return cudaGetLastError();
 }

@@ -116,3 +116,32 @@ def test_mode_entry_points_validate_without_gpu(bf):
     assert bf.bf_set_workspace(ctx, 0x10000, 1 << 30) == bf.BF_OK
     assert bf.bf_set_weight_buffers(ctx, 2) == bf.BF_EINVAL        # too late: the workspace is laid out
     bf.bf_destroy(ctx)
+
+
+def test_dtype_is_fixed_once_the_workspace_is_set(bf):
+    """The workspace layout depends on the element type (which weight operands exist): bf_set_dtype after
+    bf_set_workspace must be refused, not silently leave a kernel without its operand."""
+    ctx = bf.bf_create(32, 4, 16, 256, 16)
+    assert bf.bf_set_dtype(ctx, bf.BF_CF16) == bf.BF_OK
+    n = bf.bf_workspace_bytes(ctx)
+    assert bf.bf_set_workspace(ctx, 0x10000, n) == bf.BF_OK          # pointer is only recorded (no CUDA call)
+    assert bf.bf_set_dtype(ctx, bf.BF_CF16) == bf.BF_OK              # same type: fine
+    assert bf.bf_set_dtype(ctx, bf.BF_CI8) == bf.BF_EINVAL
+    assert "before bf_set_workspace" in bf.bf_last_error(ctx)
+    bf.bf_destroy(ctx)
+
+
+def test_workspace_grows_with_the_second_coefficient_term(bf):
+    """nint < 16 carries a second fp16 term per coefficient (bf_internal.h BF_LO_NINT): the workspace says so."""
+    a = bf.bf_create(64, 4, 40, 256, 16)
+    b = bf.bf_create(64, 4, 40, 256, 8)
+    assert bf.bf_workspace_bytes(b) > bf.bf_workspace_bytes(a) * 1.8
+    bf.bf_destroy(a); bf.bf_destroy(b)
+
+
+def test_clock_probe_argument(bf):
+    ctx = bf.bf_create(32, 4, 16, 256, 16)
+    assert bf.bf_set_clock_probe(ctx, None) == bf.BF_OK
+    assert bf.bf_set_clock_probe(ctx, 0x1004) == bf.BF_EINVAL        # 8-byte alignment
+    assert bf.bf_set_clock_probe(ctx, 0x1008) == bf.BF_OK
+    bf.bf_destroy(ctx)

@@ -46,6 +46,43 @@ def test_weight_quarter_turn_is_minus_i():
     np.testing.assert_allclose(W[0, 1], [1.0, 1.0, 1.0], atol=1e-15)  # zenith beam of a planar array
 
 
+def test_weight_z_term_hand_values():
+    """The z component of r . s (every other closed-form pin is planar).  One antenna a quarter
+    wavelength ABOVE the reference: the zenith beam sees a quarter turn (W = -i), a horizon beam none; a beam
+    30 deg from zenith sees cos(30 deg)/4 turn from height alone."""
+    f = 150e6
+    lam = C0 / f
+    r = [[0, 0, 0], [0, 0, lam / 4], [0, 0, -lam / 2]]
+    th = np.deg2rad(30.0)
+    s = [[0, 0, 1.0], [1.0, 0, 0], [math.sin(th), 0, math.cos(th)]]
+    W = oracle.weights(r, [f], s)
+    np.testing.assert_allclose(W[0, 0], [1.0, -1j, -1.0], atol=1e-12)          # zenith: -i at +lam/4, e^{+i pi} at -lam/2
+    np.testing.assert_allclose(W[0, 1], [1.0, 1.0, 1.0], atol=1e-12)           # horizon beam: height is invisible
+    np.testing.assert_allclose(W[0, 2], [1.0, np.exp(-2j * np.pi * math.cos(th) / 4), np.exp(+2j * np.pi * math.cos(th) / 2)],
+                               atol=1e-12)
+
+
+def test_tilted_plane_grid_array_factor():
+    """Closed form with z != 0: a uniform line of N antennas climbing a slope (spacing d along x, rise h per step).
+    r_n . (s_b - s_src) = n (d (l_b - l_s) + h (n_b - n_s)), so the pattern is the Dirichlet kernel in
+    psi = 2 pi f/c0 (d dl + h dn) -- drop the z term (or swap it with y) and psi, hence every power, changes."""
+    N, f, d, h, A, I = 12, 200e6, 0.9, 0.35, 1.5, 4
+    r = np.stack([np.arange(N) * d, np.zeros(N), np.arange(N) * h], axis=1)
+    def unit(l):
+        return np.array([l, 0.0, math.sqrt(1.0 - l * l)])
+    src = unit(0.2)
+    beams = np.stack([unit(l) for l in np.linspace(-0.6, 0.6, 25)])
+    x = plane_wave(r, np.array([f]), src, A, I)
+    P = oracle.beamform(r, [f], beams, x, I)
+    dl = beams[:, 0] - src[0]
+    dn = beams[:, 2] - src[2]
+    psi = 2.0 * np.pi * f / C0 * (d * dl + h * dn)
+    np.testing.assert_allclose(P[0, :, 0], I * A * A * dirichlet_sq(N, psi), rtol=1e-9, atol=1e-9)
+    # and the slope matters: the planar formula (h = 0) is off by far more than the tolerance
+    psi0 = 2.0 * np.pi * f / C0 * (d * dl)
+    assert np.abs(I * A * A * dirichlet_sq(N, psi0) - P[0, :, 0]).max() > 1.0
+
+
 def test_weights_unit_modulus_and_conjugate_symmetry():
     rng = np.random.default_rng(5)
     r = rng.normal(size=(7, 3)) * 20
