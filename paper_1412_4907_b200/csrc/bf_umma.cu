@@ -191,17 +191,31 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
 #pragma unroll
         for (int m = 0; m < GROUP; ++m) wrm[m] = (wr >> m) & 1;
         const bool vec = vec_ok;
-        for (; k < n_lean; ++k, ++i, ptr += BPT) {
+        if (n_lean > 0) epi_pend_flush<NINT_T>(pend);           // a tail left by the general loop: the lean flush below assumes whole tiles
+        // one tile on accumulator stage ACC (a compile-time constant, so its barriers and TMEM columns are immediates)
+        auto lean_tile = [&](auto acc_c, int m) {
+          constexpr int ACC = decltype(acc_c)::value;
+          uint32_t &par = ACC ? par1 : par0;
+          mbar_wait_tight(b_full + 8 * ACC, par);
+          par ^= 1;
+          tc_fence_after();
+          epilogue_tile_defer<NINT_T, true>(t_lane + ACC * TILE_T, ptr + m * mstride, wrm[m], 1 << 30, vec, b_full + 16 + 8 * ACC, lane0,
+                                            pend);
+        };
+        if constexpr (GROUP == 1) {   // items alternate between the two stages: walk them in (even, odd) pairs
+          if ((i & 1) && k < n_lean) { lean_tile(std::integral_constant<int, 1>{}, 0); ++k; ++i; ptr += BPT; }
+          for (; k + 1 < n_lean; k += 2, i += 2) {
+            lean_tile(std::integral_constant<int, 0>{}, 0); ptr += BPT;
+            lean_tile(std::integral_constant<int, 1>{}, 0); ptr += BPT;
+          }
+          if (k < n_lean) { lean_tile(std::integral_constant<int, 0>{}, 0); ++k; ++i; ptr += BPT; }
+        } else {
+          for (; k < n_lean; ++k, ++i, ptr += BPT) {
 #pragma unroll
-          for (int m = 0; m < GROUP; ++m) {
-            const uint32_t acc = GROUP == 1 ? (uint32_t)(i & 1) : (uint32_t)(m & 1);
-            uint32_t par;
-            if (GROUP == 1) { par = acc ? par1 : par0; if (acc) par1 ^= 1; else par0 ^= 1; }
-            else if (m & 1) { par = par1; par1 ^= 1; }
-            else { par = par0; par0 ^= 1; }
-            mbar_wait_tight(b_full + 8 * acc, par);
-            tc_fence_after();
-            epilogue_tile_defer<NINT_T>(t_lane + acc * TILE_T, ptr + m * mstride, wrm[m], 1 << 30, vec, b_full + 16 + 8 * acc, lane0, pend);
+            for (int m = 0; m < GROUP; ++m) {
+              if (m & 1) lean_tile(std::integral_constant<int, 1>{}, m);
+              else lean_tile(std::integral_constant<int, 0>{}, m);
+            }
           }
         }
         tt += n_lean;
@@ -362,9 +376,10 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
     // stage of a tile (the epilogue uses the same compile-time rule): GROUP even -> tile m of an item
     // goes to stage m & 1; GROUP == 1 -> item i goes to stage i & 1
     constexpr uint32_t idesc = make_idesc_f16(BF_TILE_ROWS, TILE_T);
-    const uint64_t adesc0 = make_sdesc_k_sw128(sA);
-    const uint64_t bdesc0 = make_sdesc_k_sw128(sB);
+    constexpr uint32_t dhi = sdesc_k_sw128_hi();
+    const uint32_t a_lo0 = sdesc_k_sw128_lo(sA), b_lo0 = sdesc_k_sw128_lo(sB);   // descriptor low words: address >> 4
     const uint32_t d = tmem_base + id * TILE_T;
+    const uint32_t t_full = bar_t_full + 8 * id, t_empty = bar_t_empty + 8 * id;
     Item it = decode_item(it0, nG, nTt);
     int ag = 0, ab = 0;
     int st = 0;                 // operand stage and the parity its "full" barrier completes next
@@ -381,27 +396,28 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
       }
       const bool mine = GROUP == 1 ? ((i & 1) == id) : (id < gm);
       if (mine) {
-        mbar_wait(bar_b_full + 8 * st, st_par);
-        const uint64_t bdesc = bdesc0 + (uint64_t)(st * (B_STAGE_BYTES >> 4));
+        const uint32_t b_full = bar_b_full + 8 * st, b_empty = bar_b_empty + 8 * st;
+        mbar_wait(b_full, st_par);
+        const uint32_t b_lo = b_lo0 + st * (B_STAGE_BYTES >> 4);
         for (int m = (GROUP == 1 ? 0 : id); m < gm; m += 2) {
-          mbar_wait(bar_t_empty + 8 * id, te_par);
+          mbar_wait(t_empty, te_par);
           te_par ^= 1;
           tc_fence_after();
+          const uint32_t a_lo = a_lo0 + (ab * APB + m) * (A_TILE_BYTES >> 4);
+          const bool last = m + 2 >= gm;
           if (elect_one()) {
-            const uint64_t adesc = adesc0 + (uint64_t)((ab * APB + m) * (A_TILE_BYTES >> 4));
 #pragma unroll
             for (int k = 0; k < 4; ++k)  // advance 16 fp16 = 32 bytes along K inside the swizzle atom
-              if (k < nks) mma_f16_ss(d, adesc + 2 * k, bdesc + 2 * k, idesc, k > 0);
+              if (k < nks) mma_f16_ss_lo(d, a_lo + 2 * k, b_lo + 2 * k, dhi, idesc, k > 0);
             if constexpr (LO) {          // the residual term of the coefficients against the same voltages
-              const uint64_t ldesc = adesc + (uint64_t)(GROUP * (A_TILE_BYTES >> 4));
 #pragma unroll
               for (int k = 0; k < 4; ++k)
-                if (k < nks) mma_f16_ss(d, ldesc + 2 * k, bdesc + 2 * k, idesc, 1);
+                if (k < nks) mma_f16_ss_lo(d, a_lo + GROUP * (A_TILE_BYTES >> 4) + 2 * k, b_lo + 2 * k, dhi, idesc, 1);
             }
-            tc_commit(bar_t_full + 8 * id);
-            if (m + 2 >= gm) {
-              tc_commit(bar_b_empty + 8 * st);
-              if (gm == 1) tc_commit(bar_b_empty + 8 * st);  // the other warp has no tile in this item
+            tc_commit(t_full);
+            if (last) {
+              tc_commit(b_empty);
+              if (gm == 1) tc_commit(b_empty);  // the other warp has no tile in this item
             }
           }
         }

@@ -188,13 +188,24 @@ __device__ __forceinline__ void epi_pend_init(EpiPend<NINT_T> &pd) {
   for (int j = 0; j < (EpiPend<NINT_T>::DEFER ? EpiPend<NINT_T>::NBIN : 1); ++j) pd.s[j] = 0.f;
   pd.out = nullptr; pd.nvalid = 0; pd.writer = false; pd.vec = false;
 }
-template <int NINT_T>
+// WHOLE: the pending tile is known to have all its bins (the lean loop): no per-bin bounds
+template <int NINT_T, bool WHOLE = false>
 __device__ __forceinline__ void epi_pend_flush(EpiPend<NINT_T> &pd) {
   constexpr int NBIN = EpiPend<NINT_T>::NBIN;
   if constexpr (EpiPend<NINT_T>::DEFER) {
     float tot[NBIN];
 #pragma unroll
     for (int j = 0; j < NBIN; ++j) tot[j] = pd.s[j] + __shfl_xor_sync(0xffffffffu, pd.s[j], 16);  // re^2 rows + im^2 rows
+    if constexpr (WHOLE && NINT_T != 0) {
+      if (NBIN == 4 && pd.vec) {
+        if (pd.writer) *reinterpret_cast<float4 *>(pd.out) = make_float4(tot[0], tot[1], tot[2], tot[3]);
+      } else if (pd.writer) {
+#pragma unroll
+        for (int j = 0; j < NBIN; ++j) pd.out[j] = tot[j];
+      }
+      pd.writer = false;
+      return;
+    }
     if (NINT_T == 0) {
       if (pd.writer && pd.nvalid > 0) atomicAdd(pd.out, tot[0]);
     } else if (NBIN == 4 && pd.vec) {
@@ -213,7 +224,7 @@ __device__ __forceinline__ void epi_pend_flush(EpiPend<NINT_T> &pd) {
 // One accumulator tile for one warp, tail deferred (see above).  Same contract as epilogue_tile; `pd` carries the
 // previous tile's tail in and this tile's tail out.  Bins of <= 8 samples (more than 4 bins per warp) fall back to
 // the immediate form.
-template <int NINT_T>
+template <int NINT_T, bool WHOLE = false>
 __device__ __forceinline__ void epilogue_tile_defer(uint32_t taddr, float *out, bool writer, int nvalid, bool vec_ok,
                                                     uint32_t bar_empty, bool lane0, EpiPend<NINT_T> &pd) {
   if constexpr (!EpiPend<NINT_T>::DEFER) {
@@ -233,7 +244,7 @@ __device__ __forceinline__ void epilogue_tile_defer(uint32_t taddr, float *out, 
     for (int ch = 0; ch < NCH; ++ch) {
       uint32_t v[32];
       BF_TMEM_LD_32x32b_X32(taddr + 32 * ch, v);
-      if (ch == 0) epi_pend_flush<NINT_T>(pd);   // the previous tile's shuffles and stores, under this load
+      if (ch == 0) epi_pend_flush<NINT_T, WHOLE>(pd);   // the previous tile's shuffles and stores, under this load
       tc_wait_ld();
       if (ch == NCH - 1) {  // all of this warp's columns are in registers: release the stage
         tc_fence_before();

@@ -161,6 +161,23 @@ BF_DEVI void mma_f16_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_
       : "memory");
 }
 
+// The same with the two descriptors given as 32-bit low words plus their common high word: all operand tiles of a
+// kernel share the high word (stride, version, swizzle), and advancing along K or to another stage only changes the
+// 14-bit address field, so the issuing warp does 32-bit arithmetic instead of 64-bit adds with carries.
+BF_DEVI void mma_f16_ss_lo(uint32_t d_tmem, uint32_t adesc_lo, uint32_t bdesc_lo, uint32_t desc_hi, uint32_t idesc,
+                           uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\t"
+      "mov.b64 da, {%1, %5};\n\tmov.b64 db, {%2, %5};\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, p;\n\t}" ::"r"(d_tmem),
+      "r"(adesc_lo), "r"(bdesc_lo), "r"(idesc), "r"(accumulate), "r"(desc_hi)
+      : "memory");
+}
+// low / high word of make_sdesc_k_sw128
+BF_DEVI uint32_t sdesc_k_sw128_lo(uint32_t saddr) { return ((saddr >> 4) & 0x3FFFu) | (1u << 16); }
+__host__ __device__ constexpr uint32_t sdesc_k_sw128_hi() { return (1024u >> 4) | (1u << 14) | (2u << 29); }
+
 // D[tmem] (+)= A[tmem] * B[smem]: the A operand (M = 128 rows = TMEM lanes, 16 fp16 along K = 8 columns) read from
 // tensor memory, B from shared memory
 BF_DEVI void mma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
