@@ -510,11 +510,12 @@ static int umma_variant(int dtype, int nant) {
   if (dtype == BF_CI4 && nant % 16 == 0 && nant <= 32) return 1;  // bulk copies need rows of 16 bytes
   if (dtype == BF_CI8 && nant % 8 == 0) return 2;   // TMA rows must be multiples of 16 bytes
   if (dtype == BF_CF16 && nant % 4 == 0) return 2;
+  if (dtype == BF_CI4 && nant % 16 == 0) return 2;  // K-blocks of 32 antennas = 32 bytes per sample
   return 0;
 }
 
 bool bf_umma_shape_supported(const bf_ctx *c, const char **why) {
-  if (!umma_variant(c->dtype, c->nant)) { *why = "needs nant % 8 == 0 (int8), % 4 == 0 (fp16), or 16 / 32 (4-bit)"; return false; }
+  if (!umma_variant(c->dtype, c->nant)) { *why = "needs nant % 8 == 0 (int8), % 4 == 0 (fp16) or % 16 == 0 (4-bit)"; return false; }
   return true;
 }
 

@@ -31,7 +31,7 @@ constexpr int CONV_WARPS = 8;
 constexpr int CONV_THREADS = CONV_WARPS * 32;
 constexpr int MMA_WARP = EPI_WARPS + CONV_WARPS;
 constexpr int TMA_WARP = MMA_WARP + 2;  // two MMA-issuing warps, one per accumulator
-constexpr int NTHREADS = (EPI_WARPS + CONV_WARPS + 3) * 32;
+constexpr int NTHREADS = (EPI_WARPS + CONV_WARPS + 4) * 32;   // + 2 MMA warps + 2 producer warps
 template <bool LO> constexpr int a_stage_bytes_v = (LO ? 2 : 1) * KB_GROUP * A_TILE_BYTES;   // [hi tiles][lo tiles]
 
 struct KItem { int c, tt, g; };
@@ -46,11 +46,14 @@ __device__ __forceinline__ KItem kdecode(long long idx, int nG, int nTt) {
 
 // LO: two-term coefficients (bf_internal.h, BF_LO_NINT): a coefficient stage holds the "hi" tiles followed by the "lo"
 // tiles of the K-block and every voltage K-block is contracted against both.
-template <int NINT_T, bool IS_F16, int NA, int NB, int NR, bool BEAMS, bool LO>
+// IN: BF_CI8 / BF_CF16 / BF_CI4 (the paper's 4+4-bit bytes: a K-block of 32 antennas is 32 raw bytes per
+// sample, unpacked by the convert warps).
+template <int NINT_T, int IN, int NA, int NB, int NR, bool BEAMS, bool LO>
 __global__ void __launch_bounds__(NTHREADS, 1)
 bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, const long long total_items,
                       const int nG, const int nTt) {
   extern __shared__ uint8_t smem_raw[];
+  constexpr bool IS_F16 = IN == BF_CF16, IS_CI4 = IN == BF_CI4;
   constexpr int A_STAGE_BYTES = a_stage_bytes_v<LO>;
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sA = smem_base;                              // NA stages x 2 (x 2) coefficient tiles
@@ -126,14 +129,17 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
   } else if (warp < MMA_WARP) {
     // =========================================================================== convert (int8 input only)
     if (!IS_F16) {
-      constexpr int PIECES = (TILE_T * 4) / CONV_THREADS;
+      // 16-byte input pieces per K-block: int8 rows are 64 bytes (4 pieces, 2 output chunks each), 4-bit rows 32 bytes
+      // (2 pieces of 16 antennas, 4 output chunks each)
+      constexpr int PPR = IS_CI4 ? 2 : 4, CPP = IS_CI4 ? 4 : 2;
+      constexpr int PIECES = (TILE_T * PPR) / CONV_THREADS;
       const int ctid = threadIdx.x - EPI_WARPS * 32;
       uint32_t p_dst[PIECES];
 #pragma unroll
       for (int k = 0; k < PIECES; ++k) {
         const int pc = ctid + k * CONV_THREADS;
-        const int t = pc >> 2, q = pc & 3;
-        p_dst[k] = (uint32_t)((t >> 3) * 1024 + (t & 7) * 128 + (((2 * q) ^ (t & 7)) << 4));
+        const int t = pc / PPR, q = pc % PPR;
+        p_dst[k] = (uint32_t)((t >> 3) * 1024 + (t & 7) * 128 + (((CPP * q) ^ (t & 7)) << 4));
       }
       const long long nblk = (long long)n_items * nKb;
       int rs = 0, bs = 0;
@@ -143,7 +149,8 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
         uint4 x[PIECES];
         convert_load<PIECES, CONV_THREADS>(sR + rs * RAW_STAGE_BYTES, ctid, p_dst, x);
         mbar_wait(bar_b_empty + 8 * bs, bpar);
-        convert_store<PIECES>(sB + bs * B_STAGE_BYTES, p_dst, x);
+        if constexpr (IS_CI4) convert_store_ci4<PIECES>(sB + bs * B_STAGE_BYTES, p_dst, x);
+        else convert_store<PIECES>(sB + bs * B_STAGE_BYTES, p_dst, x);
         fence_proxy_async_smem();
         __syncwarp();
         if (lane == 0) {
@@ -196,32 +203,46 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
       }
     }
   } else if (warp == TMA_WARP && lane == 0) {
-    // =========================================================================== TMA producer (one thread)
+    // =========================================================================== producer 1 of 2: coefficient tiles
+    // Two producer threads, one per operand, each with its own ring: a single thread that issued all three copies of
+    // a K-block and polled both "empty" barriers was itself the slowest stage of the pipeline (anything added to its
+    // loop slowed the whole kernel; the tensor pipe sat at 70-74 %).
+    int sa = 0;
+    uint32_t apar = 1;
+    for (int i = 0; i < n_items; ++i) {
+      const KItem it = kdecode(it0 + i * it_step, nG, nTt);
+      const int gm = min(KB_GROUP, nMt - it.g * KB_GROUP);
+      const char *src = reinterpret_cast<const char *>(p.wop) + ((size_t)it.c * nMt + (size_t)(it.g * KB_GROUP)) * nKb * A_TILE_BYTES;
+      const char *src_lo = LO ? reinterpret_cast<const char *>(p.wop_lo) + ((size_t)it.c * nMt + (size_t)(it.g * KB_GROUP)) * nKb * A_TILE_BYTES
+                              : nullptr;
+      const size_t mstep = (size_t)nKb * A_TILE_BYTES;     // from M-tile m to m + 1 at the same K-block
+      for (int kb = 0; kb < nKb; ++kb, src += A_TILE_BYTES, src_lo += A_TILE_BYTES) {
+        mbar_wait(bar_a_empty + 8 * sa, apar);
+        mbar_arrive_expect_tx(bar_a_full + 8 * sa, (LO ? 2 : 1) * gm * A_TILE_BYTES);
+        for (int m = 0; m < gm; ++m) {
+          bulk_g2s(sA + sa * A_STAGE_BYTES + m * A_TILE_BYTES, src + m * mstep, A_TILE_BYTES, bar_a_full + 8 * sa);
+          if constexpr (LO)
+            bulk_g2s(sA + sa * A_STAGE_BYTES + (KB_GROUP + m) * A_TILE_BYTES, src_lo + m * mstep, A_TILE_BYTES, bar_a_full + 8 * sa);
+        }
+        if (++sa == NA) { sa = 0; apar ^= 1; }
+      }
+    }
+  } else if (warp == TMA_WARP + 1 && lane == 0) {
+    // =========================================================================== producer 2 of 2: voltage K-blocks
     tma_prefetch_desc(&tmap);
-    int sa = 0, sv = 0;  // sv: voltage stage (operand stage for fp16, raw stage for int8)
-    uint32_t apar = 1, vpar = 1;
+    int sv = 0;  // voltage stage (operand stage for fp16, raw stage for int8)
+    uint32_t vpar = 1;
     constexpr int NV = IS_F16 ? NB : NR;
-    constexpr uint32_t VBYTES = IS_F16 ? B_STAGE_BYTES : RAW_STAGE_BYTES;
+    constexpr uint32_t VBYTES = IS_F16 ? B_STAGE_BYTES : (IS_CI4 ? RAW_STAGE_BYTES / 2 : RAW_STAGE_BYTES);
+    constexpr int XSTEP = IS_CI4 ? BF_KBLOCK / 2 : BF_KBLOCK;   // tensor-map elements (bytes / fp16) per K-block
     const uint32_t sV = IS_F16 ? sB : sR;
     const uint32_t bar_v_full = IS_F16 ? bar_b_full : bar_r_full, bar_v_empty = IS_F16 ? bar_b_empty : bar_r_empty;
     for (int i = 0; i < n_items; ++i) {
       const KItem it = kdecode(it0 + i * it_step, nG, nTt);
-      const int gm = min(KB_GROUP, nMt - it.g * KB_GROUP);
       for (int kb = 0; kb < nKb; ++kb) {
-        mbar_wait(bar_a_empty + 8 * sa, apar);
-        mbar_arrive_expect_tx(bar_a_full + 8 * sa, (LO ? 2 : 1) * gm * A_TILE_BYTES);
-        for (int m = 0; m < gm; ++m) {
-          const size_t off = (((size_t)it.c * nMt + (size_t)(it.g * KB_GROUP + m)) * nKb + kb) * A_TILE_BYTES;
-          bulk_g2s(sA + sa * A_STAGE_BYTES + m * A_TILE_BYTES, reinterpret_cast<const char *>(p.wop) + off, A_TILE_BYTES,
-                   bar_a_full + 8 * sa);
-          if constexpr (LO)
-            bulk_g2s(sA + sa * A_STAGE_BYTES + (KB_GROUP + m) * A_TILE_BYTES, reinterpret_cast<const char *>(p.wop_lo) + off,
-                     A_TILE_BYTES, bar_a_full + 8 * sa);
-        }
         mbar_wait(bar_v_empty + 8 * sv, vpar);
         mbar_arrive_expect_tx(bar_v_full + 8 * sv, VBYTES);
-        tma_load_3d(sV + sv * VBYTES, &tmap, kb * BF_KBLOCK, it.tt * TILE_T, it.c, bar_v_full + 8 * sv);
-        if (++sa == NA) { sa = 0; apar ^= 1; }
+        tma_load_3d(sV + sv * (IS_F16 ? B_STAGE_BYTES : RAW_STAGE_BYTES), &tmap, kb * XSTEP, it.tt * TILE_T, it.c, bar_v_full + 8 * sv);
         if (++sv == NV) { sv = 0; vpar ^= 1; }
       }
     }
@@ -234,16 +255,16 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
 }
 
 // 3-D view of the voltages: {K' elements, nsamp, nchan}, box {64, 256, 1}
-template <bool F16>
-cudaError_t make_tmap(CUtensorMap *tm, const BfParams &p, int) {
-  constexpr int dtype = F16 ? BF_CF16 : BF_CI8;
+template <int IN>
+cudaError_t make_tmap(CUtensorMap *tm, const BfParams &p, int box_rows) {
   PFN_encodeTiled enc = bf_get_encode();
   if (!enc) return cudaErrorNotSupported;
-  const bool f16 = dtype == BF_CF16;
+  const bool f16 = IN == BF_CF16;
   const cuuint64_t esz = f16 ? 2 : 1;
-  cuuint64_t dims[3] = {(cuuint64_t)2 * p.nant, (cuuint64_t)p.nsamp, (cuuint64_t)p.nchan_run};
+  // elements per sample row: 2 nant (re, im) values, or nant bytes for the 4+4-bit format
+  cuuint64_t dims[3] = {(cuuint64_t)(IN == BF_CI4 ? p.nant : 2 * p.nant), (cuuint64_t)p.nsamp, (cuuint64_t)p.nchan_run};
   cuuint64_t strides[2] = {dims[0] * esz, dims[0] * esz * (cuuint64_t)p.nsamp};
-  cuuint32_t box[3] = {BF_KBLOCK, (cuuint32_t)TILE_T, 1};
+  cuuint32_t box[3] = {(cuuint32_t)(IN == BF_CI4 ? BF_KBLOCK / 2 : BF_KBLOCK), (cuuint32_t)box_rows, 1};
   cuuint32_t estr[3] = {1, 1, 1};
   CUresult r = enc(tm, f16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8, 3,
                    const_cast<void *>(p.volt), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -252,18 +273,20 @@ cudaError_t make_tmap(CUtensorMap *tm, const BfParams &p, int) {
   return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-template <int NINT_T, bool IS_F16, bool BEAMS = false, bool LO = false>
+template <int NINT_T, int IN, bool BEAMS = false, bool LO = false>
 cudaError_t launch_kb(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
+  (void)dtype;
+  constexpr bool IS_F16 = IN == BF_CF16;
   constexpr int NA = LO ? 2 : 3, NB = LO ? 2 : (IS_F16 ? 3 : 2), NR = IS_F16 ? 0 : (LO ? 2 : 3);
   constexpr int A_STAGE_BYTES = a_stage_bytes_v<LO>;
   CUtensorMap tm;
-  cudaError_t e = bf_cached_tmap(&tm, p, IS_F16 ? 101 : 100, TILE_T, make_tmap<IS_F16>);
+  cudaError_t e = bf_cached_tmap(&tm, p, 100 + IN, TILE_T, make_tmap<IN>);
   if (e != cudaSuccess) return e;
   const int nG = (p.nMt + KB_GROUP - 1) / KB_GROUP;
   const int nTt = (p.nsamp + TILE_T - 1) / TILE_T;
   const long long total = (long long)p.nchan_run * nTt * nG;
   const size_t smem = 1024 + NA * A_STAGE_BYTES + NB * B_STAGE_BYTES + NR * RAW_STAGE_BYTES + 512;
-  auto kern = bf_umma_kblock_kernel<NINT_T, IS_F16, NA, NB, NR, BEAMS, LO>;
+  auto kern = bf_umma_kblock_kernel<NINT_T, IN, NA, NB, NR, BEAMS, LO>;
   static thread_local int attr_dev = -1;   // once per instantiation and device
   if ((e = bf_set_smem_once(kern, smem, &attr_dev)) != cudaSuccess) return e;
   if (NINT_T == 0 && !BEAMS) {
@@ -275,33 +298,34 @@ cudaError_t launch_kb(const BfParams &p, int dtype, int sm_count, cudaStream_t s
   return cudaGetLastError();
 }
 
-template <bool IS_F16>
+template <int IN>
 cudaError_t launch_kb_nint(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
-  if (p.mode == BF_MODE_BEAMS) return launch_kb<64, IS_F16, true>(p, dtype, sm_count, st);
+  if (p.mode == BF_MODE_BEAMS) return launch_kb<64, IN, true>(p, dtype, sm_count, st);
   if (p.wop_lo != nullptr) {   // short bins: two-term coefficients
     switch (p.nint) {
-      case 1: return launch_kb<1, IS_F16, false, true>(p, dtype, sm_count, st);
-      case 2: return launch_kb<2, IS_F16, false, true>(p, dtype, sm_count, st);
-      case 4: return launch_kb<4, IS_F16, false, true>(p, dtype, sm_count, st);
-      case 8: return launch_kb<8, IS_F16, false, true>(p, dtype, sm_count, st);
+      case 1: return launch_kb<1, IN, false, true>(p, dtype, sm_count, st);
+      case 2: return launch_kb<2, IN, false, true>(p, dtype, sm_count, st);
+      case 4: return launch_kb<4, IN, false, true>(p, dtype, sm_count, st);
+      case 8: return launch_kb<8, IN, false, true>(p, dtype, sm_count, st);
       default: break;
     }
   }
   switch (p.nint) {
-    case 1: return launch_kb<1, IS_F16>(p, dtype, sm_count, st);
-    case 2: return launch_kb<2, IS_F16>(p, dtype, sm_count, st);
-    case 4: return launch_kb<4, IS_F16>(p, dtype, sm_count, st);
-    case 8: return launch_kb<8, IS_F16>(p, dtype, sm_count, st);
-    case 16: return launch_kb<16, IS_F16>(p, dtype, sm_count, st);
-    case 32: return launch_kb<32, IS_F16>(p, dtype, sm_count, st);
-    case 64: return launch_kb<64, IS_F16>(p, dtype, sm_count, st);
-    default: return launch_kb<0, IS_F16>(p, dtype, sm_count, st);
+    case 1: return launch_kb<1, IN>(p, dtype, sm_count, st);
+    case 2: return launch_kb<2, IN>(p, dtype, sm_count, st);
+    case 4: return launch_kb<4, IN>(p, dtype, sm_count, st);
+    case 8: return launch_kb<8, IN>(p, dtype, sm_count, st);
+    case 16: return launch_kb<16, IN>(p, dtype, sm_count, st);
+    case 32: return launch_kb<32, IN>(p, dtype, sm_count, st);
+    case 64: return launch_kb<64, IN>(p, dtype, sm_count, st);
+    default: return launch_kb<0, IN>(p, dtype, sm_count, st);
   }
 }
 
 }  // namespace
 
 cudaError_t bf_launch_umma_kblock(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
-  if (dtype == BF_CF16) return launch_kb_nint<true>(p, dtype, sm_count, st);
-  return launch_kb_nint<false>(p, dtype, sm_count, st);
+  if (dtype == BF_CF16) return launch_kb_nint<BF_CF16>(p, dtype, sm_count, st);
+  if (dtype == BF_CI4) return launch_kb_nint<BF_CI4>(p, dtype, sm_count, st);
+  return launch_kb_nint<BF_CI8>(p, dtype, sm_count, st);
 }

@@ -222,6 +222,15 @@ def make_workload(name: str, nbeam: Optional[int] = None) -> Workload:
         # the medium geometry with the paper's own 4+4-bit wire format
         w = make_workload("medium")
         return dataclasses.replace(w, name=name, dtype="ci4", sigma=2.0, sources=[(w.sources[0][0], 1.0)])
+    if name == "sweep-ci4":
+        # the beam-count sweep on the paper's 4+4-bit wire format (halves the input bytes, which moves the
+        # bandwidth -> compute crossover to fewer beams)
+        w = make_workload("sweep", nbeam=nbeam)
+        return dataclasses.replace(w, name=w.name.replace("sweep", "sweep-ci4"), dtype="ci4", sigma=2.0)
+    if name == "streaming-ci4":
+        # the 1024-antenna aperture array fed 4+4-bit samples: half the PCIe bytes per antenna-sample
+        w = make_workload("streaming")
+        return dataclasses.replace(w, name=name, dtype="ci4", sigma=2.0)
     if name == "sweep":
         N, C, T, I = 32, 512, 16384, 16
         B = 64 if nbeam is None else nbeam

@@ -123,6 +123,13 @@ SMALL = [
     (32, 1, 130, 512, 64, "ci4"),
     (16, 2, 5, 256, 1, "ci4"),       # K' = 32: half a K-block
     (24, 2, 7, 128, 16, "ci4"),      # rows of 24 bytes: generic kernel only
+    (64, 3, 256, 992, 32, "ci8"),    # K-blocked, two beam groups: CTA pairs with multicast voltages (int8: raw stages), ragged tail
+    (128, 2, 200, 528, 16, "cf16"),  # the same for fp16 input (operand stages are the multicast target), last M-tile partial
+    (72, 5, 300, 704, 64, "cf16"),   # three beam groups... odd: no pairs; 5 channels
+    (64, 7, 512, 512, 64, "ci8"),    # four beam groups, 7 x 2 x 4 = 56 items on 56 CTAs
+    (1024, 1, 16, 256, 64, "ci4"),   # 4-bit input on the K-blocked kernel: the streaming array's antenna count
+    (48, 2, 70, 608, 16, "ci4"),     # K-blocked, second K-block half full (TMA zero-fills), two M-tiles, ragged tail
+    (64, 2, 9, 512, 4, "ci4"),       # K-blocked with two-term coefficients
     (32, 40, 64, 5000, 8, "ci8"),    # 800 items: 5-6 per CTA, both convert groups busy, ragged tail (5000 = 19*256 + 136)
     (32, 30, 100, 3000, 4, "ci4"),   # same for the 4-bit unpack, two M-tiles per item
 ]
@@ -241,7 +248,7 @@ def test_coherent_gain_property(bf):
 
 
 # ------------------------------------------------------------------ full BASELINE.json sizes, EVERY channel
-FULL = [("medium", None), ("medium-ci4", None), ("sweep", 1), ("sweep", 4), ("sweep", 16), ("sweep", 64), ("sweep", 256),
+FULL = [("medium", None), ("medium-ci4", None), ("streaming-ci4", None), ("sweep-ci4", 16), ("sweep", 1), ("sweep", 4), ("sweep", 16), ("sweep", 64), ("sweep", 256),
         ("sweep", 1024), ("large-N", None), ("streaming", None)]
 
 
@@ -287,6 +294,7 @@ EXTREME_CASES = [
     (32, 2, 64, 1024, 16, "ci4", "auto"),                 # 4-bit unpack in the resident kernel: nibble flip at 0x8
     (16, 2, 5, 512, 8, "ci4", "auto"),
     (24, 2, 7, 128, 16, "ci4", "auto"),                   # CUDA-core kernel's nibble decode
+    (64, 2, 33, 512, 32, "ci4", "auto"),                  # K-blocked kernel's nibble unpack
     (32, 2, 16, 1024, 16, "ci4", "simt"),
 ]
 
