@@ -494,7 +494,10 @@ cudaError_t launch_k64_nint(const BfParams &p, int sm_count, cudaStream_t st) {
   }
   // <= 64 beams: HBM-bound.  A raw slot is held for the whole HBM latency plus the conversion (~3 us
   // measured), so the bytes in flight per SM decide the bandwidth: 8 raw slots of 16 KiB.
-  if (p.nbeam <= 32) return launch_k64<NINT_T, 1, 2, 8, 8, true, IN>(p, sm_count, st);   // rows only in lane quadrants 0-1
+  // <= 32 beams: rows only in lane quadrants 0-1, the epilogue gets those sub-partitions to itself (SPREAD).  Not for the
+  // 4-bit format: its unpack is three instructions per antenna and needs all four sub-partitions (measured on the
+  // sweep at 16 beams: 0.220 ms SPREAD, 0.195 ms plain)
+  if (p.nbeam <= 32 && IN != BF_CI4) return launch_k64<NINT_T, 1, 2, 8, 8, true, IN>(p, sm_count, st);
   if (p.nMt == 1) return launch_k64<NINT_T, 1, 2, 8, 8, false, IN>(p, sm_count, st);
   if (p.nMt <= 2) return launch_k64<NINT_T, 2, 3, 4, 8, false, IN>(p, sm_count, st);
   return launch_k64<NINT_T, 4, 2, 2, 8, false, IN>(p, sm_count, st);                  // many beams: MMA-bound, big A group

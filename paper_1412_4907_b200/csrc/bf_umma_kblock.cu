@@ -104,7 +104,7 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
       const int gm = min(KB_GROUP, nMt - it.g * KB_GROUP);
       const int t_first = it.tt * TILE_T + slot * 64;
       for (int m = 0; m < gm; ++m) {
-        mbar_wait(bar_t_full + 8 * m, (tpar >> m) & 1);
+        mbar_wait_backoff(bar_t_full + 8 * m, (tpar >> m) & 1, 128);   // a K loop away: do not spin
         tpar ^= 1u << m;
         tc_fence_after();
         const int beam = (it.g * KB_GROUP + m) * BF_TILE_BEAMS + bl;

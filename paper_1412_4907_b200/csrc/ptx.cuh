@@ -109,6 +109,17 @@ BF_DEVI void mbar_wait(uint32_t bar, uint32_t parity) {
     if (clock64() - t0 > 40000000000LL) asm volatile("trap;");
   }
 }
+// Wait for roles that wait LONG (the K-blocked kernel's epilogue sits out a whole K loop): sleep between polls, so
+// that the waiting warps stop taking issue slots from the working ones (ncu: 56 % of the streaming kernel's
+// instructions were such polls).  Bounded like the others.
+BF_DEVI void mbar_wait_backoff(uint32_t bar, uint32_t parity, uint32_t sleep_ns) {
+  if (mbar_try_wait(bar, parity)) return;
+  for (uint32_t n = 0;; ++n) {
+    asm volatile("nanosleep.u32 %0;" ::"r"(sleep_ns));
+    if (mbar_try_wait(bar, parity)) return;
+    if (n > (1u << 26)) asm volatile("trap;");
+  }
+}
 // Tight bounded wait for roles on the critical chain (the epilogue): two instructions per failed poll, trap after
 // 2^26 polls (a try_wait blocks for a hardware-defined slice, so this is seconds, not a hang).
 BF_DEVI void mbar_wait_tight(uint32_t bar, uint32_t parity) {
