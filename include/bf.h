@@ -55,7 +55,11 @@ enum bf_dtype {
 };
 
 enum bf_kernel {
-  BF_KERNEL_AUTO = 0, /* pick the fastest kernel that supports the shape */
+  BF_KERNEL_AUTO = 0, /* pick the fastest kernel that supports the shape.  NOTE: for shapes no tensor-core kernel takes (nant
+                         not a multiple of 8 (int8) / 4 (fp16) / 16 (4+4-bit), nint neither 2^k <= 64 nor a multiple of 64 / 32)
+                         AUTO falls through to BF_KERNEL_SIMT without an error -- about 30x slower on the `tiny` shape;
+                         bf_kernel_name / bf_selected_kernel say which family will run, and BF_KERNEL_UMMA turns the
+                         fall-through into BF_EUNSUPPORTED */
   BF_KERNEL_SIMT = 1, /* generic fp32 CUDA-core kernel (any shape; Algorithm 1's structure) */
   BF_KERNEL_UMMA = 2, /* tcgen05/TMEM tensor-core kernels with the fused |.|^2 + integrate epilogue (the library
                          picks the variant) */
@@ -74,24 +78,31 @@ bf_ctx *bf_create(int nant, int nchan, int nbeam, int nsamp, int nint);
 /* Free the context (host state only; caller-owned device memory is untouched).  NULL is allowed. */
 void bf_destroy(bf_ctx *ctx);
 
-/* Select the voltage element type (enum bf_dtype).  Call before bf_workspace_bytes. */
+/* Select the voltage element type (enum bf_dtype): complex int8 (BASELINE.json configs), complex fp16, or the paper's
+ * F-engine wire format, "4-bit, two's complement ... real and imaginary components ... a single byte".
+ * Call before bf_workspace_bytes / bf_set_workspace: the workspace layout depends on it, and a different type after
+ * bf_set_workspace is refused with BF_EINVAL. */
 int bf_set_dtype(bf_ctx *ctx, int dtype);
 
-/* Force a kernel (enum bf_kernel); default BF_KERNEL_AUTO.  BF_EUNSUPPORTED is reported by bf_run
+/* Force a kernel (enum bf_kernel); default BF_KERNEL_AUTO.  All kernels compute the same operation (Sec. 2.1,
+ * PAPER.md:60-64); BF_KERNEL_SIMT keeps the structure of the paper's Algorithm 1.  BF_EUNSUPPORTED is reported by bf_run
  * if the forced kernel cannot run the context's shape. */
 int bf_set_kernel(bf_ctx *ctx, int kernel);
 
-/* Which kernel family bf_run will launch for this context: BF_KERNEL_SIMT or BF_KERNEL_UMMA. */
+/* Which kernel family bf_run will launch for this context: BF_KERNEL_SIMT (CUDA cores, Algorithm 1's structure,
+ * PAPER.md:66-98) or BF_KERNEL_UMMA (tensor cores: the N_b x N_a matrix product of PAPER.md:62). */
 int bf_selected_kernel(const bf_ctx *ctx);
 
 /* Name of the kernel bf_run will launch: "simt", "umma-f16-resident", "umma-f16-kblock", "umma-i8". */
 const char *bf_kernel_name(const bf_ctx *ctx);
 
-/* Number of kernels this context has launched so far (all streams), for accounting. */
+/* Number of kernels this context has launched so far (all streams), for accounting (the bench line's
+ * gpu_launches). */
 long long bf_launch_count(const bf_ctx *ctx);
 
 /*
- * Device workspace: geometry copy + the weight operand.  The caller allocates `bytes` >=
+ * Device workspace: geometry copy + the weight operand(s) -- the beam coefficients of Eq. 1, kept on
+ * the device because they "do not need to change within small time frames".  The caller allocates `bytes` >=
  * bf_workspace_bytes(ctx) of DEVICE memory, 1024-byte aligned, and keeps it alive while the
  * context is used.  Returns BF_EINVAL on NULL / misaligned pointer, BF_ENOMEM if too small.
  */
@@ -209,10 +220,11 @@ int bf_run_streaming(bf_ctx *ctx, const void *const *host_blocks, int nblocks, f
  */
 int bf_set_clock_probe(bf_ctx *ctx, void *dev_u64x4);
 
-/* Message for the last error on this context ("" if none).  Valid until the next call on ctx. */
+/* Message for the last error on this context ("" if none).  Valid until the next call on ctx.  (Error reporting of the
+ * ABI itself; no passage of the paper.) */
 const char *bf_last_error(const bf_ctx *ctx);
 
-/* Library version string. */
+/* Library version string (names the target architecture, sm_100a). */
 const char *bf_version(void);
 
 #ifdef __cplusplus

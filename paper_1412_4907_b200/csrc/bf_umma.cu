@@ -196,6 +196,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         auto lean_tile = [&](auto acc_c, int m) {
           constexpr int ACC = decltype(acc_c)::value;
           uint32_t &par = ACC ? par1 : par0;
+          // (sleeping between polls was measured at 64 beams: 0.188 vs 0.172 ms -- the wake-up latency is on the chain)
           mbar_wait_tight(b_full + 8 * ACC, par);
           par ^= 1;
           tc_fence_after();

@@ -10,6 +10,8 @@ Tolerances (DESIGN.md 'Tolerance'):
   fp16 inputs are summed in fp32 (rel ~ sqrt(n) 2^-24): bar 1e-5.
 * tracking: the power bar of test_gpu_parity.py (1e-3 per row), for every block with ITS geometry.
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -178,3 +180,42 @@ def test_update_geometry_needs_two_buffers(bf):
         B.update_geometry(w.ant_xyz, w.freqs, w.beam_dir)
     assert e.value.code == bf.BF_EINVAL
     B.close()
+
+
+# ------------------------------------------------------------------ boundary: a failing stream-ordering call is reported
+def test_stream_ordering_failures_surface_as_bf_ecuda():
+    """every cudaStreamWaitEvent / cudaEventRecord of the library is checked.  The compute stream
+    handed to bf_run_host is put into graph-capture mode first: waiting there on the "copy landed" event, which is
+    recorded on the (non-capturing) copy stream, is illegal, so the library's cudaStreamWaitEvent fails and the call must
+    come back with BF_ECUDA.  (A destroyed stream handle is not a usable injection: the runtime accepted it.)  Run in a
+    subprocess: the broken capture must not leak into the other tests."""
+    import subprocess
+    import sys
+    code = r'''
+import ctypes, sys, numpy as np, torch
+sys.path.insert(0, ".")
+import synthetic, paper_1412_4907_b200 as bf
+w = synthetic.make_workload("tiny").sub(nchan=4, nsamp=256)
+B = bf.Beamformer(w.nant, w.nchan, w.nbeam, w.nsamp, w.nint)
+B.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
+hv = torch.from_numpy(w.make_voltages()).pin_memory()
+hp = torch.empty((w.nchan, w.nbeam, w.nbin), dtype=torch.float32).pin_memory()
+try:
+    rt = ctypes.CDLL("libcudart.so.12")
+except OSError:
+    rt = ctypes.CDLL("/usr/local/cuda/lib64/libcudart.so.12")
+cs, xs = torch.cuda.Stream(), torch.cuda.Stream()
+B.run_host(hv, hp, 2, cs, xs)                      # the same call is fine on ordinary streams
+cs.synchronize(); xs.synchronize()
+assert rt.cudaStreamBeginCapture(ctypes.c_void_p(cs.cuda_stream), 0) == 0
+try:
+    B.run_host(hv, hp, 2, cs, xs)
+    print("RESULT no-error")
+except bf.BfError as e:
+    print("RESULT", e.code, str(e)[:120])
+'''
+    r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300,
+                       cwd=os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("RESULT")]
+    assert lines, (r.returncode, r.stdout[-500:], r.stderr[-1500:])
+    assert lines[0].split()[1] == "-3", lines[0]          # BF_ECUDA
