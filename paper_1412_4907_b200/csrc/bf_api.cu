@@ -49,7 +49,9 @@ static size_t geom_bytes(const bf_ctx *c) {  // positions, frequencies, directio
 }
 // the int8 two-limb operand exists whenever the shape could take bf_umma_i8.cu (any nint)
 static bool i8_shape(const bf_ctx *c) {
-  return c->dtype == BF_CI8 && c->nant % 8 == 0 && c->nant <= 32 && c->nbeam <= BF_I8_MAX_BEAMS;
+  if (c->nbeam > BF_I8_MAX_BEAMS) return false;
+  if (c->dtype == BF_CI4) return c->nant == 32;       // 4+4-bit rows unpack to int8 operands in bf_umma_i8b.cu
+  return c->dtype == BF_CI8 && c->nant % 8 == 0 && c->nant <= 32;
 }
 static size_t wop8_bytes(const bf_ctx *c) {
   return i8_shape(c) ? align_up((size_t)c->nchan * bf_i8_ncol(c->nbeam) * 64, BF_ALIGN) : 0;
@@ -135,7 +137,8 @@ static int pick_kernel(const bf_ctx *c, int mode, const char **why) {
   if (k == BF_KERNEL_SIMT) return BF_KERNEL_SIMT;
   const bool i8_ok = i8_shape(c) && bf_umma_i8_supported(c, mode) && (c->d_wop8 != nullptr || c->ws == nullptr);
   if (k == BF_KERNEL_UMMA_I8) {
-    if (!i8_ok) *why = "int8 kernel needs complex int8 input, nant % 8 == 0 and <= 32, <= 32 beams, nint 2^k <= 32 or % 32 == 0";
+    if (!i8_ok) *why = "int8-operand kernel needs int8 input with nant % 8 == 0 and <= 32 (4-bit: nant = 32, nint % 4 == 0), <= 32 beams, "
+                       "nint 2^k <= 32, % 32 == 0, or even with nbin % 128 == 0 or >= 512";
     return i8_ok ? BF_KERNEL_UMMA_I8 : 0;
   }
   if (k != BF_KERNEL_UMMA_F16 && i8_ok && c->nbeam <= BF_I8_AUTO_BEAMS) return BF_KERNEL_UMMA_I8;
@@ -415,7 +418,7 @@ static int launch_range(bf_ctx *c, const void *volt, void *out, int chan0, int n
   const char *why = "";
   const int k = pick_kernel(c, mode, &why);
   if (k == 0) return fail(c, BF_EUNSUPPORTED, "tensor-core kernel cannot run this shape: %s", why);
-  cudaError_t e = k == BF_KERNEL_UMMA_I8    ? bf_launch_umma_i8(p, c->sm_count, st)
+  cudaError_t e = k == BF_KERNEL_UMMA_I8    ? bf_launch_umma_i8(p, c->dtype, c->sm_count, st)
                   : k == BF_KERNEL_UMMA_F16 ? bf_launch_umma(p, c->dtype, c->sm_count, st)
                                             : bf_launch_simt(p, c->dtype, st);
   if (e != cudaSuccess) return cuda_fail(c, e, k == BF_KERNEL_SIMT ? "SIMT kernel launch" : "tensor-core kernel launch");

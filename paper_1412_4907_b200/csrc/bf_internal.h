@@ -111,7 +111,9 @@ cudaError_t bf_launch_simt(const BfParams &p, int dtype, cudaStream_t st);
 bool bf_umma_supported(const bf_ctx *c, const char **why);
 bool bf_umma_shape_supported(const bf_ctx *c, const char **why);  // ignoring nint (voltage-beam mode)
 bool bf_umma_i8_supported(const bf_ctx *c, int mode);
-cudaError_t bf_launch_umma_i8(const BfParams &p, int sm_count, cudaStream_t st);
+cudaError_t bf_launch_umma_i8(const BfParams &p, int dtype, int sm_count, cudaStream_t st);
+bool bf_umma_i8b_takes(const BfParams &p, int dtype);   // bf_umma_i8b.cu: one output bin per TMEM lane
+cudaError_t bf_launch_umma_i8b(const BfParams &p, int dtype, int sm_count, cudaStream_t st);
 cudaError_t bf_launch_incoherent(const bf_ctx *c, const void *volt, float *out, cudaStream_t st);
 cudaError_t bf_launch_umma(const BfParams &p, int dtype, int sm_count, cudaStream_t st);
 cudaError_t bf_launch_umma_kblock(const BfParams &p, int dtype, int sm_count, cudaStream_t st);

@@ -1,0 +1,446 @@
+// bf_umma_i8b.cu -- the int8-operand few-beam kernel with ONE OUTPUT BIN PER TMEM LANE (hot-path rows a2..a5,
+// <= 32 beams, 32 antennas, complex int8 or 4+4-bit input, even nint).
+//
+// bf_umma_i8.cu puts TIME on the M axis of tcgen05.mma kind::i8 (so that TMEM holds only real beams) and then has
+// to integrate ACROSS the lanes of a warp: a transposing butterfly of shuffles, selects and adds that costs as much
+// as the detection itself (profiles/r02_roles.md, sweep-B32: 2723 epilogue instructions per 256 samples, of which
+// FSEL + SHFL + FADD are 450 and the rest is six instructions per beam and sample).  Here the TMA engine does the
+// transposition on the way in: the voltages of one channel are viewed as a 4-D tensor
+//      { 128 bytes = two samples of 32 antennas,  nint / 2 rows per bin,  nbin,  nchan }
+// and a tile is the box {128, 1, 128, 1}: row g of 128 CONSECUTIVE BINS.  Row r of the A operand (= TMEM lane r)
+// therefore belongs to bin 128 sp + r in every one of the G = nint / 2 tiles of a super-tile, and the integration
+// P[c][b][j] = sum_t |y|^2 is a plain running sum in the registers of the thread that owns the
+// lane: no shuffle, no select, and the stores of a warp are 32 consecutive bins of one beam (128 bytes).
+//   a3 contraction  as in bf_umma_i8.cu (WIDE form): four MMAs per tile slice the 128-byte rows along K, even
+//                   sample -> accumulator E, odd sample -> accumulator O; two-limb 15-bit weights (A21)
+//   a4 detection    re = 128 hi + lo (IMAD), I2F, then ONE packed FFMA2 squares (re, im) into a float2 running sum:
+//                   five instructions per beam and sample
+//   a5 integration  in registers over the G tiles, (x + y) * scale^2, one coalesced fp32 store per beam
+// 4+4-bit input (row f1): the raw byte masked to its high nibble IS the int8 number 16 re, shifted
+// left by four it is 16 im -- three ALU instructions per four antennas turn a raw row of 128 bytes (four samples)
+// into two int8 operand rows, which the same MMAs and the same epilogue consume (scale / 16).
+//
+// Warp roles (one persistent CTA per SM over a contiguous range of (channel, super-tile)): warps 0-7 epilogue in
+// two sets that split the 8-beam column chunks of EVERY tile between them (set 1 idles for <= 8 beams), warp 8 MMA
+// issue + TMEM allocation, warps 9-10 one TMA thread each (tiles of even / odd index), warps 11-14 (4-bit input
+// only) unpack.
+#include <cuda.h>
+#include <stdlib.h>
+
+#include "bf_internal.h"
+#include "bf_tmap.h"
+#include "ptx.cuh"
+
+namespace {
+
+constexpr int B_ROW_BYTES = 128;                       // one operand row: two samples x 32 antennas x (re, im)
+constexpr int B_STAGE_BYTES = 128 * B_ROW_BYTES;       // 16 KiB: 128 bins x two samples
+constexpr int B_W_ROW_BYTES = 64;                      // coefficient rows (bf_internal.h: int8 two-limb operand)
+#ifndef B_SETS_MAX
+#define B_SETS_MAX 4
+#endif
+constexpr int B_UNPACK_WARPS = 4;
+// epilogue sets of four warps (one per TMEM lane quadrant): CS column sets split the 8-beam chunks of a tile, TS tile
+// sets take alternate tiles of a super-tile (their partial sums meet in shared memory at its end).  A warp's work on
+// a tile is one chain -- barrier, tcgen05.ld, 5 instructions per beam and sample -- of 300-400 clk whatever the beam
+// count, so up to 16 beams (one chunk per warp) two tile sets are needed to keep up with 4-bit input.
+__host__ __device__ constexpr int b_csets(int ncol) { return ncol / 32 >= 4 ? 4 : (ncol / 32 >= 2 ? 2 : 1); }
+__host__ __device__ constexpr int b_tsets(int ncol) { return ncol / 32 >= 4 ? 1 : 2; }
+__host__ __device__ constexpr int b_nsets(int ncol) { return b_csets(ncol) * b_tsets(ncol); }
+
+__host__ __device__ constexpr int b_ilog2(int x) { return x <= 1 ? 0 : 1 + b_ilog2(x >> 1); }
+
+BF_DEVI void tma_load_5d(uint32_t dst_smem, const void *tmap, int x, int y, int z, int w, int v, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];"
+      ::"r"(dst_smem), "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(w), "r"(v), "r"(bar) : "memory");
+}
+
+// unpack groups (4-bit input): groups of four warps on alternate raw tiles (a tile's unpack is one chain of dependent
+// latencies -- barrier, LDS, barrier, STS, proxy fence, arrive -- that a group walks once per tile); one group only
+// next to four epilogue sets (registers)
+__host__ __device__ constexpr int b_ugroups(int ncol) { return 1; }   // measured: a second group changes nothing (0.0741 / 0.0725 ms)
+template <int NCOL, int IN> constexpr int i8b_threads_v = (4 * b_nsets(NCOL) + 3 + (IN == BF_CI4 ? B_UNPACK_WARPS * b_ugroups(NCOL) : 0)) * 32;
+
+// NCOL: accumulator columns = 4 * beam capacity (32 / 64 / 128 -> 8 / 16 / 32 beams).  NST: operand stages (int8:
+// filled by TMA; 4-bit: filled by the unpack warps from NRAW raw stages).
+template <int NCOL, int NST, int NRAW, int IN, int LPB>
+__global__ void __launch_bounds__(i8b_threads_v<NCOL, IN>, 1)
+bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, const long long total_super,
+                   const int n_super_chan, const int G, const int l2pf) {
+  extern __shared__ uint8_t smem_raw[];
+  constexpr bool CI4 = IN == BF_CI4;
+  constexpr int W_BYTES = NCOL * B_W_ROW_BYTES;
+  constexpr int NACC = 512 / (2 * NCOL);                    // accumulator PAIRS (even, odd sample) in TMEM
+  constexpr int NCH = NCOL / 32;                            // 8-beam column chunks
+  constexpr int NSETS = b_nsets(NCOL), CS = b_csets(NCOL), TS = b_tsets(NCOL);
+  constexpr int B_MMA_WARP = 4 * NSETS, B_TMA_WARP = B_MMA_WARP + 1, B_UNPACK_WARP = B_MMA_WARP + 3;
+  constexpr int CPS = NCH / CS;                             // chunks per column set
+  constexpr int BPS = 128 / LPB;                            // bins per super-tile
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sW = smem_base;                            // 2 coefficient buffers
+  const uint32_t sA = sW + 2 * W_BYTES;                     // NST operand stages (W_BYTES is a multiple of 1024)
+  const uint32_t sR = sA + NST * B_STAGE_BYTES;             // NRAW raw stages (4-bit input)
+  const uint32_t sX = sR + NRAW * B_STAGE_BYTES;            // tile-set exchange: [2][4 quadrants][CS][8 CPS][32 lanes] floats
+  constexpr int X_BYTES = TS > 1 ? 2 * 4 * CS * 8 * CPS * 32 * 4 : 0;
+  const uint32_t sBar = sX + X_BYTES;
+  const uint32_t bar_a_full = sBar, bar_a_empty = bar_a_full + 8 * NST;
+  const uint32_t bar_r_full = bar_a_empty + 8 * NST, bar_r_empty = bar_r_full + 8 * (NRAW + 1);
+  const uint32_t bar_w_full = bar_r_empty + 8 * (NRAW + 1), bar_w_empty = bar_w_full + 16;
+  const uint32_t bar_t_full = bar_w_empty + 16, bar_t_empty = bar_t_full + 8 * NACC;
+  const uint32_t s_tmem = bar_t_empty + 8 * NACC;
+
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    // operand stage "full": one TMA transaction (int8) or the unpack warps (4-bit); "empty": the MMA's commit
+    for (int s = 0; s < NST; ++s) { mbar_init(bar_a_full + 8 * s, CI4 ? B_UNPACK_WARPS : 1); mbar_init(bar_a_empty + 8 * s, 1); }
+    for (int s = 0; s < NRAW; ++s) { mbar_init(bar_r_full + 8 * s, 1); mbar_init(bar_r_empty + 8 * s, B_UNPACK_WARPS); }   // one group per stage
+    for (int s = 0; s < 2; ++s) { mbar_init(bar_w_full + 8 * s, 1); mbar_init(bar_w_empty + 8 * s, 1); }
+    for (int s = 0; s < NACC; ++s) { mbar_init(bar_t_full + 8 * s, 1); mbar_init(bar_t_empty + 8 * s, 4 * CS); }
+    fence_barrier_init();
+  }
+  if (warp == B_MMA_WARP) tmem_alloc(s_tmem, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(s_tmem));
+  tmem_base = __shfl_sync(0xffffffffu, tmem_base, 0);
+  probe_mark(p.probe, 0);
+
+  // this CTA's contiguous range of super-tiles (super-tile = 128 bins of one channel = G tiles; 4-bit input: G
+  // raw tiles of four samples per bin, each unpacked into two operand tiles)
+  const long long s0 = total_super * blockIdx.x / gridDim.x;
+  const long long s1 = total_super * (blockIdx.x + 1) / gridDim.x;
+  const int n_super = (int)(s1 - s0);
+  const int c0 = (int)(s0 / n_super_chan), sp0 = (int)(s0 % n_super_chan);
+  const int GT = CI4 ? 2 * G : G;                           // operand tiles per super-tile
+
+  if (warp < 4 * NSETS) {
+    // =========================================================================== epilogue
+    const int quad = warp & 3, set = (warp >> 2) % CS, tset = (warp >> 2) / CS;
+    const bool lane0 = lane == 0;
+    const uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16) + set * (CPS * 32);
+    const uint32_t xch = sX + (uint32_t)(((quad * CS + set) * 8 * CPS) * 32 + lane) * 4;   // + buffer, + 128 per value
+    const int nbeam = p.nbeam, nbin = p.nbin;
+    int c = c0, sp = sp0;
+    int ti = 0;                                             // operand-tile counter of this CTA (all roles count alike)
+    for (int s = 0; s < n_super; ++s) {
+      const int bin = BPS * sp + (32 * quad + lane) / LPB;
+      const bool live = BPS * sp + 32 * quad / LPB < nbin;  // warp-uniform: this quadrant holds real bins
+      // requested now, used after the G tiles: a load at the END of the super-tile would stall every warp for a
+      // DRAM round trip per super-tile
+      const float sc = (float)p.i8scale[c] * (CI4 ? 0.0625f : 1.0f);         // 4-bit operands carry 16 x
+      float2 acc[CPS][8];
+#pragma unroll
+      for (int k = 0; k < CPS; ++k)
+#pragma unroll
+        for (int i = 0; i < 8; ++i) acc[k][i] = make_float2(0.f, 0.f);
+      for (int g = 0; g < GT; ++g, ++ti) {
+        if (TS > 1 && (g & (TS - 1)) != tset) continue;     // the other tile set's
+        const int a = ti & (NACC - 1);
+        mbar_wait(bar_t_full + 8 * a, (uint32_t)((ti >> b_ilog2(NACC)) & 1));
+        tc_fence_after();
+        if (!live) {                                        // bins past the end of the channel (zero-filled rows)
+          __syncwarp();
+          if (lane0) mbar_arrive(bar_t_empty + 8 * a);
+          continue;
+        }
+#pragma unroll
+        for (int k = 0; k < CPS; ++k) {
+          uint32_t v[32], u[32];
+          BF_TMEM_LD_32x32b_X32(t_lane + a * 2 * NCOL + 32 * k, v);          // even samples
+          BF_TMEM_LD_32x32b_X32(t_lane + a * 2 * NCOL + NCOL + 32 * k, u);   // odd samples
+          tc_wait_ld();
+          if (k == CPS - 1) {  // all of this warp's columns are in registers: hand the accumulator pair back
+            tc_fence_before();
+            __syncwarp();
+            if (lane0) mbar_arrive(bar_t_empty + 8 * a);
+          }
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int re = ((int)v[4 * i] << 7) + (int)v[4 * i + 2];         // 128 hi + lo, exact
+            const int im = ((int)v[4 * i + 1] << 7) + (int)v[4 * i + 3];
+            const int ro = ((int)u[4 * i] << 7) + (int)u[4 * i + 2];
+            const int io = ((int)u[4 * i + 1] << 7) + (int)u[4 * i + 3];
+            const float2 e = make_float2((float)re, (float)im), o = make_float2((float)ro, (float)io);
+            acc[k][i] = ffma2(e, e, acc[k][i]);
+            acc[k][i] = ffma2(o, o, acc[k][i]);
+          }
+        }
+      }
+      if constexpr (TS > 1) {
+        // tile set 1 hands its partial sums to tile set 0 of the same (quadrant, column set): double-buffered by
+        // super-tile parity, one named barrier per pair of warps
+        const uint32_t xb = xch + (uint32_t)(s & 1) * (X_BYTES / 2);
+        if (tset == 1 && live) {
+#pragma unroll
+          for (int k = 0; k < CPS; ++k)
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+              asm volatile("st.shared.f32 [%0], %1;" ::"r"(xb + (k * 8 + i) * 128), "f"(acc[k][i].x + acc[k][i].y) : "memory");
+        }
+        asm volatile("bar.sync %0, 64;" ::"r"(1 + quad * CS + set) : "memory");
+        if (tset == 0 && live) {
+#pragma unroll
+          for (int k = 0; k < CPS; ++k)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              float o;
+              asm volatile("ld.shared.f32 %0, [%1];" : "=f"(o) : "r"(xb + (k * 8 + i) * 128) : "memory");
+              acc[k][i].x += o;
+            }
+        }
+      }
+      if (live && tset == 0) {
+        const float sc2 = sc * sc;
+        float *out = p.pow + (size_t)c * nbeam * nbin + bin;
+        const bool writer = (lane & (LPB - 1)) == 0 && bin < nbin;
+#pragma unroll
+        for (int k = 0; k < CPS; ++k)
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            float tot = acc[k][i].x + acc[k][i].y;
+#pragma unroll
+            for (int o = LPB / 2; o >= 1; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);   // the LPB lanes of a bin
+            const int beam = 8 * (set * CPS + k) + i;
+            if (writer && beam < nbeam) out[(size_t)beam * nbin] = tot * sc2;
+          }
+      }
+      if (++sp == n_super_chan) { sp = 0; ++c; }
+    }
+  } else if (warp == B_MMA_WARP) {
+    // =========================================================================== MMA issue
+    constexpr uint32_t idesc = make_idesc_i8(128, NCOL);
+    int c = c0, sp = sp0, prev_c = -1, wi = 0, wb = 0;
+    int ti = 0, st = 0;
+    uint32_t st_par = 0;
+    for (int s = 0; s < n_super; ++s) {
+      if (c != prev_c) {
+        if (wi > 0 && elect_one()) tc_commit(bar_w_empty + 8 * wb);   // my MMAs so far have left the old buffer
+        prev_c = c;
+        wb = wi & 1;
+        mbar_wait(bar_w_full + 8 * wb, (uint32_t)((wi >> 1) & 1));
+        ++wi;
+      }
+      const uint64_t bdesc = make_sdesc_k_sw64(sW + wb * W_BYTES);
+      for (int g = 0; g < GT; ++g, ++ti) {
+        const int a = ti & (NACC - 1);
+        mbar_wait(bar_a_full + 8 * st, st_par);
+        mbar_wait(bar_t_empty + 8 * a, (uint32_t)(((ti >> b_ilog2(NACC)) & 1) ^ 1));
+        tc_fence_after();
+        if (elect_one()) {
+          const uint64_t adesc = make_sdesc_k_sw128(sA + st * B_STAGE_BYTES);
+          const uint32_t d = tmem_base + a * 2 * NCOL;
+          mma_i8_ss(d, adesc, bdesc, idesc, 0);                  // even sample: row bytes 0..31
+          mma_i8_ss(d, adesc + 2, bdesc + 2, idesc, 1);          //              row bytes 32..63
+          mma_i8_ss(d + NCOL, adesc + 4, bdesc, idesc, 0);       // odd sample:  row bytes 64..95
+          mma_i8_ss(d + NCOL, adesc + 6, bdesc + 2, idesc, 1);   //              row bytes 96..127
+          tc_commit(bar_t_full + 8 * a);
+          tc_commit(bar_a_empty + 8 * st);
+        }
+        __syncwarp();
+        if (++st == NST) { st = 0; st_par ^= 1; }
+      }
+      if (++sp == n_super_chan) { sp = 0; ++c; }
+    }
+  } else if (warp == B_TMA_WARP || warp == B_TMA_WARP + 1) {
+    // =========================================================================== TMA producers (two warps)
+    // lane 0 of producer j issues the tiles of parity j; producer 0 also brings in the coefficients.  int8: the
+    // tiles are the operand stages themselves; 4-bit: raw stages for the unpack warps.
+    const int pj = warp - B_TMA_WARP;
+    constexpr int NRING = CI4 ? NRAW : NST;
+    static_assert(NRING % 2 == 0, "stages are dealt to the producers by parity");
+    const uint32_t ring = CI4 ? sR : sA, full = CI4 ? bar_r_full : bar_a_full, empty = CI4 ? bar_r_empty : bar_a_empty;
+    if (lane == 0) tma_prefetch_desc(&tmap);
+    int c = c0, sp = sp0, prev_c = -1, wi = 0;
+    int ti = 0, st = pj;
+    uint32_t st_par = 1;                 // parity of empty[st] to wait for (passes on the fresh barrier)
+    // A tile takes 128 LPB bytes out of every bin; the G tiles of a super-tile together cover one CONTIGUOUS region
+    // of BPS * nint samples, but spread over the super-tile's whole duration: DRAM would open every page G times
+    // (measured: 5.9 instead of 6.3 TB/s, while from a resident L2 the strided copies are FASTER than contiguous
+    // ones).  With every tile the whole producer warp therefore prefetches 16 KiB of the NEXT super-tile's region
+    // into the L2 (plain prefetch.global.L2: the TMA unit is busy with the boxes) -- sequential DRAM reads one
+    // super-tile ahead, and the strided tensor copies hit the L2.
+    const size_t samp_bytes = CI4 ? 32 : 64;
+    const size_t region = (size_t)BPS * p.nint * samp_bytes;             // = G pieces of 16 KiB
+    const bool l2_ahead = l2pf != 0 && G > 1 && region <= (256u << 10);
+    for (int s = 0; s < n_super; ++s) {
+      const char *nb = nullptr;          // the next super-tile's region and its length
+      uint32_t nbytes = 0;
+      if (l2_ahead && s + 1 < n_super) {
+        int cn = c, spn = sp + 1;
+        if (spn == n_super_chan) { spn = 0; ++cn; }
+        const size_t bins_left = (size_t)(p.nbin - BPS * spn);
+        nbytes = (uint32_t)((bins_left < (size_t)BPS ? bins_left : (size_t)BPS) * p.nint * samp_bytes);
+        nb = reinterpret_cast<const char *>(p.volt) + ((size_t)cn * p.nsamp + (size_t)BPS * spn * p.nint) * samp_bytes;
+      }
+      if (c != prev_c) {
+        prev_c = c;
+        if (pj == 0 && lane == 0) {
+          const int wb = wi & 1;
+          mbar_wait(bar_w_empty + 8 * wb, (uint32_t)(((wi >> 1) & 1) ^ 1));
+          mbar_arrive_expect_tx(bar_w_full + 8 * wb, W_BYTES);
+          bulk_g2s(sW + wb * W_BYTES, reinterpret_cast<const char *>(p.wop8) + (size_t)c * W_BYTES, W_BYTES, bar_w_full + 8 * wb);
+        }
+        ++wi;
+      }
+      for (int g = 0; g < G; ++g, ++ti) {
+        if ((ti & 1) != pj) continue;
+        if (nb != nullptr) {
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const uint32_t off = (uint32_t)g * B_STAGE_BYTES + (uint32_t)(k * 32 + lane) * 128u;
+            if (off < nbytes) asm volatile("prefetch.global.L2 [%0];" ::"l"(nb + off));
+          }
+        }
+        if (lane == 0) {
+          mbar_wait(empty + 8 * st, st_par);
+          mbar_arrive_expect_tx(full + 8 * st, B_STAGE_BYTES);
+          tma_load_5d(ring + st * B_STAGE_BYTES, &tmap, 0, 0, BPS * sp, g, c, full + 8 * st);   // rows LPB g .. of bins BPS sp ..
+        }
+        __syncwarp();
+        if ((st += 2) >= NRING) { st -= NRING; st_par ^= 1; }
+      }
+      if (++sp == n_super_chan) { sp = 0; ++c; }
+    }
+  } else if (CI4 && warp >= B_UNPACK_WARP) {
+    // =========================================================================== unpack (4-bit input, UG groups of 4 warps)
+    // A raw row is 128 bytes = FOUR samples of 32 antennas (high nibble re, low nibble im).  Masked
+    // to the high nibbles a byte is the int8 number 16 re, shifted left by four it is 16 im; PRMT interleaves the
+    // two into (re, im) byte pairs.  Samples 0, 1 of every row go to operand tile 2r, samples 2, 3 to tile 2r+1.
+    // Thread t of a group's 128 handles the 16-byte piece t & 7 of rows (t >> 3) + 16 k: piece q holds the antennas
+    // 16 (q & 1) .. of sample q >> 1, i.e. 32 bytes of operand row at byte 64 (q >> 1 & 1) + 32 (q & 1) of tile q >> 2.
+    constexpr int UG = b_ugroups(NCOL);
+    static_assert(NRAW % UG == 0, "raw stages are dealt to the unpack groups");
+    const int grp = (warp - B_UNPACK_WARP) >> 2;
+    const int ut = ((warp - B_UNPACK_WARP) & 3) * 32 + lane;
+    const int q = ut & 7, r0 = ut >> 3;
+    const uint32_t src0 = (uint32_t)(r0 * 128 + ((q ^ (r0 & 7)) << 4));              // raw stage is 128-byte swizzled by TMA
+    const uint32_t ch0 = (uint32_t)(4 * ((q >> 1) & 1) + 2 * (q & 1));               // first 16-byte chunk of the output
+    const uint32_t dst0 = (uint32_t)(r0 * 128 + ((ch0 ^ (r0 & 7)) << 4));            // second chunk: ^ 16
+    const uint32_t tsel = (uint32_t)(q >> 2);
+    int rs = grp, st = 2 * grp;            // group j: raw tiles j, j + UG, .. -> raw stage i % NRAW, operand stages 2 i % NST, + 1
+    uint32_t rpar = 0, spar = 1;
+    const int n_raw = n_super * G;
+    for (int i = grp; i < n_raw; i += UG) {
+      mbar_wait(bar_r_full + 8 * rs, rpar);
+      uint4 x[8];
+#pragma unroll
+      for (int k = 0; k < 8; ++k)   // rows r0 + 16 k: the swizzle term (row & 7) is the same for all of them
+        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(x[k].x), "=r"(x[k].y), "=r"(x[k].z), "=r"(x[k].w)
+                     : "r"(sR + rs * B_STAGE_BYTES + src0 + k * 2048));
+      // both operand tiles of this raw tile must be free
+      const int st1 = st + 1 == NST ? 0 : st + 1;
+      const uint32_t spar1 = st + 1 == NST ? spar ^ 1 : spar;
+      mbar_wait(bar_a_empty + 8 * st, spar);
+      mbar_wait(bar_a_empty + 8 * st1, spar1);
+      const uint32_t dst = sA + (tsel ? st1 : st) * B_STAGE_BYTES + dst0;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const uint32_t w[4] = {x[k].x, x[k].y, x[k].z, x[k].w};
+        uint32_t o[8];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t hi = w[j] & 0xF0F0F0F0u;             // 16 re of four antennas
+          const uint32_t lo = (w[j] << 4) & 0xF0F0F0F0u;      // 16 im
+          o[2 * j] = __byte_perm(hi, lo, 0x5140);             // (re0, im0, re1, im1)
+          o[2 * j + 1] = __byte_perm(hi, lo, 0x7362);         // (re2, im2, re3, im3)
+        }
+        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(dst + k * 2048), "r"(o[0]), "r"(o[1]), "r"(o[2]), "r"(o[3]) : "memory");
+        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"((dst ^ 16u) + k * 2048), "r"(o[4]), "r"(o[5]), "r"(o[6]), "r"(o[7]) : "memory");
+      }
+      fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) {
+        mbar_arrive(bar_r_empty + 8 * rs);
+        mbar_arrive(bar_a_full + 8 * st);
+        mbar_arrive(bar_a_full + 8 * st1);
+      }
+      if ((rs += UG) >= NRAW) { rs -= NRAW; rpar ^= 1; }
+      if ((st += 2 * UG) >= NST) { st -= NST; spar ^= 1; }
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == B_MMA_WARP) tmem_dealloc(tmem_base, 512);
+  probe_mark(p.probe, 1);
+}
+
+// 4-D view of one launch's voltages: {128 bytes, rows per bin, nbin, nchan}; box {128, 1, 128, 1}, 128-byte swizzle.
+// A row is two int8 samples (rows per bin = nint / 2) or four 4-bit samples (nint / 4); bins past nbin are zero-filled.
+template <int IN, int LPB>
+cudaError_t make_tmap_bins(CUtensorMap *tm, const BfParams &p, int nint) {
+  PFN_encodeTiled enc = bf_get_encode();
+  if (!enc) return cudaErrorNotSupported;
+  const int spr = IN == BF_CI4 ? 4 : 2;                                 // samples per 128-byte row
+  const cuuint64_t chan_bytes = (cuuint64_t)p.nsamp * (128 / spr);
+  // {byte in row, row in chunk, bin, chunk in bin, channel}: a tile = chunk g of 128 / LPB consecutive bins
+  cuuint64_t dims[5] = {128, LPB, (cuuint64_t)p.nbin, (cuuint64_t)(nint / spr / LPB), (cuuint64_t)p.nchan_run};
+  cuuint64_t strides[4] = {128, (cuuint64_t)nint * (128 / spr), 128 * LPB, chan_bytes};
+  cuuint32_t box[5] = {128, LPB, 128 / LPB, 1, 1};
+  cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 5, const_cast<void *>(p.volt), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+template <int NCOL, int IN, int LPB>
+cudaError_t launch_i8b_lpb(const BfParams &p, int sm_count, cudaStream_t st) {
+  constexpr bool CI4 = IN == BF_CI4;
+  constexpr int NST = CI4 ? 6 : 12, NRAW = CI4 ? 6 : 0;
+  CUtensorMap tm;
+  cudaError_t e = bf_cached_tmap(&tm, p, (CI4 ? 20 : 10) + LPB, p.nint, make_tmap_bins<IN, LPB>);
+  if (e != cudaSuccess) return e;
+  const int G = p.nint / (CI4 ? 4 : 2) / LPB;
+  const int n_super_chan = (p.nbin + 128 / LPB - 1) / (128 / LPB);
+  const long long total = (long long)p.nchan_run * n_super_chan;
+  constexpr int X_BYTES = b_tsets(NCOL) > 1 ? 2 * 4 * 8 * (NCOL / 32) * 32 * 4 : 0;   // tile-set exchange buffers
+  const size_t smem = 1024 + 2 * NCOL * B_W_ROW_BYTES + (size_t)(NST + NRAW) * B_STAGE_BYTES + X_BYTES + 1024;
+  auto kern = bf_umma_i8b_kernel<NCOL, NST, NRAW, IN, LPB>;
+  static thread_local int attr_dev = -1;   // once per instantiation and device
+  if ((e = bf_set_smem_once(kern, smem, &attr_dev)) != cudaSuccess) return e;
+  const int grid = (int)(total < sm_count ? total : sm_count);
+  static int l2pf = -1;
+  if (l2pf < 0) { const char *e = getenv("BF_I8B_L2PF"); l2pf = e ? atoi(e) : 1; }
+  kern<<<grid, i8b_threads_v<NCOL, IN>, smem, st>>>(p, tm, total, n_super_chan, G, l2pf);
+  return cudaGetLastError();
+}
+
+// LPB = lanes per bin.  1: every 128-byte row of a tile comes from another bin, no cross-lane sum at all.  2 / 4
+// (chunks of 256 / 512 contiguous bytes, one / two shuffle-adds per beam at the end of a super-tile) were measured
+// on the sweep and are slower at every beam count (32 beams: 0.117 / 0.156 / 0.237 ms for LPB 1 / 2 / 4): a
+// super-tile then has half / a quarter of the tiles to amortise its reduction and stores over.  Only 1 is built.
+template <int NCOL, int IN>
+cudaError_t launch_i8b(const BfParams &p, int sm_count, cudaStream_t st) {
+  return launch_i8b_lpb<NCOL, IN, 1>(p, sm_count, st);
+}
+
+}  // namespace
+
+// Shapes this kernel takes (the caller has checked int8 / 4-bit input, nant % 8 == 0, <= 32 beams): 32 antennas,
+// nint a multiple of the samples per 128-byte row, and enough bins that the 128 lanes of a super-tile are not
+// mostly padding (a channel's last super-tile is partial: at most a fifth wasted).
+bool bf_umma_i8b_takes(const BfParams &p, int dtype) {
+  static int off = -1;
+  if (off < 0) { const char *e = getenv("BF_I8B_OFF"); off = e ? atoi(e) : 0; }
+  if (off) return false;
+  if (p.mode != BF_MODE_POWER || p.nant != 32) return false;
+  if (p.nint % (dtype == BF_CI4 ? 4 : 2) != 0) return false;
+  if ((long long)p.nint * 64 >= (1ll << 32)) return false;
+  return p.nbin % 128 == 0 || p.nbin >= 512;
+}
+
+cudaError_t bf_launch_umma_i8b(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
+  if (dtype == BF_CI4) {
+    if (p.nbeam <= 8) return launch_i8b<32, BF_CI4>(p, sm_count, st);
+    if (p.nbeam <= 16) return launch_i8b<64, BF_CI4>(p, sm_count, st);
+    return launch_i8b<128, BF_CI4>(p, sm_count, st);
+  }
+  if (p.nbeam <= 8) return launch_i8b<32, BF_CI8>(p, sm_count, st);
+  if (p.nbeam <= 16) return launch_i8b<64, BF_CI8>(p, sm_count, st);
+  return launch_i8b<128, BF_CI8>(p, sm_count, st);
+}

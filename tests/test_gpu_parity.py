@@ -183,6 +183,14 @@ I8_SHAPES = [
     (32, 1, 4, 131, 1),        # odd nsamp: narrow variant
     (8, 1, 1, 1, 1),           # one sample
     (32, 2, 8, 66048, 32),     # 258 tiles per channel: super-tile ranges that straddle channels
+    # the bin-per-lane variant (bf_umma_i8b.cu): 32 antennas, even nint, nbin % 128 == 0 or >= 512
+    (32, 3, 32, 1280, 2),      # nint = 2: one tile per super-tile, 5 super-tiles per channel, 32 beams (both epilogue sets)
+    (32, 2, 5, 8192, 64),      # 128 bins: one super-tile of 32 tiles per channel, a single column chunk (set 1 idle)
+    (32, 1, 17, 20480, 32),    # 640 bins: the last super-tile of the channel is partial (TMA zero-fills bins >= nbin)
+    (32, 5, 9, 6144, 6),       # nint = 6: any even nint integrates in registers (1024 bins)
+    (32, 7, 16, 16384, 16),    # the sweep's per-channel shape: 8 super-tiles x 7 channels on 56 CTAs
+    (32, 2, 24, 33280, 4),     # 8320 bins = 65 super-tiles: CTA ranges straddle the channel boundary
+    (32, 1, 13, 66560, 130),   # nint = 130 = 65 tiles per super-tile, 512 bins
 ]
 
 
@@ -196,6 +204,34 @@ def test_i8_kernel_shapes(bf, shape):
     # 15-bit weights: far inside the 1e-3 bar even at nint = 1 (measured ~1e-4 there)
     worst = check_rows(out, ref, TOL)
     print(f"i8 {shape} worst={worst:.2e}")
+
+
+I8B_CI4_SHAPES = [
+    # nant nchan nbeam nsamp nint -- 4+4-bit input on the int8-operand kernel (bin-per-lane variant only): raw rows of
+    # four samples unpacked to two int8 operand tiles each
+    (32, 2, 16, 2048, 16),     # 128 bins, four raw tiles per super-tile
+    (32, 3, 5, 5120, 8),       # 640 bins: partial last super-tile, a single column chunk
+    (32, 2, 32, 8192, 64),     # 32 beams: four epilogue sets, 16 raw tiles per super-tile
+    (32, 1, 9, 2560, 4),       # one raw tile per super-tile
+    (32, 7, 16, 16384, 16),    # the sweep's per-channel shape
+    (32, 2, 24, 33280, 4),     # 65 super-tiles per channel: CTA ranges straddle the channel boundary
+    (32, 1, 13, 6144, 12),     # nint = 12: three raw rows per bin
+]
+
+
+@pytest.mark.parametrize("shape", I8B_CI4_SHAPES, ids=lambda s: "N%d-C%d-B%d-T%d-I%d" % s)
+def test_i8_kernel_ci4_shapes(bf, shape):
+    N, C, B, T, I = shape
+    w = synthetic.make_case(N, C, B, T, I, "ci4", seed=5)
+    v = w.make_voltages()
+    ref = oracle.beamform(w.ant_xyz, w.freqs, w.beam_dir, v, I)
+    out, _ = run_gpu(bf, w, v, bf.BF_KERNEL_UMMA_I8)
+    worst = check_rows(out, ref, TOL)
+    print(f"i8/ci4 {shape} worst={worst:.2e}")
+    # and it is the automatic choice for few beams on this format
+    Bf = bf.Beamformer(N, C, B, T, I, dtype=bf.BF_CI4)
+    assert Bf.kernel_name == "umma-i8"
+    Bf.close()
 
 
 def test_i8_kernel_is_the_auto_choice_for_few_beams_and_f16_can_be_forced(bf):
@@ -288,6 +324,8 @@ EXTREME_CASES = [
     (64, 2, 33, 512, 32, "ci8", "auto"),                  # K-blocked kernel, int8 input
     (32, 2, 16, 1024, 16, "ci8", "i8"),                   # int8-operand kernel, WIDE: kind::i8 with -128 x limb
     (32, 2, 32, 1024, 1, "ci8", "i8"),                    # WIDE, nint = 1
+    (32, 2, 16, 2048, 16, "ci8", "i8"),                   # bin-per-lane variant (128 bins)
+    (32, 1, 32, 8192, 64, "ci8", "i8"),                   # bin-per-lane, 32 tiles per super-tile
     (16, 2, 9, 300, 4, "ci8", "i8"),                      # int8-operand kernel, narrow rows
     (32, 1, 7, 960, 96, "ci8", "i8"),                     # nint = 96 = 3 x 32
     (32, 2, 16, 1024, 16, "ci8", "simt"),
@@ -296,6 +334,8 @@ EXTREME_CASES = [
     (24, 2, 7, 128, 16, "ci4", "auto"),                   # CUDA-core kernel's nibble decode
     (64, 2, 33, 512, 32, "ci4", "auto"),                  # K-blocked kernel's nibble unpack
     (32, 2, 16, 1024, 16, "ci4", "simt"),
+    (32, 2, 16, 2048, 16, "ci4", "i8"),                   # int8-operand kernel: nibble -> 16 x int8 by mask / shift (-8 -> -128)
+    (32, 1, 32, 4096, 32, "ci4", "i8"),
 ]
 
 
