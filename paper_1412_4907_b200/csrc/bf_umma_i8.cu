@@ -28,13 +28,10 @@
 // flight per SM.  All role loops keep 32-bit wrap counters: a 64-bit division per tile in the single producer
 // thread was measurably on the critical path.
 #include <cuda.h>
-#include <stdlib.h>
 
 #include "bf_internal.h"
 #include "bf_tmap.h"
 #include "ptx.cuh"
-
-static bool bf_i8b_forced() { static int f = -1; if (f < 0) { const char *e = getenv("BF_I8B_FORCE"); f = e ? atoi(e) : 0; } return f != 0; }
 
 namespace {
 
@@ -641,7 +638,7 @@ cudaError_t bf_launch_umma_i8(const BfParams &p, int dtype, int sm_count, cudaSt
   // 32 antennas, even nint and enough bins to fill the lanes: the bin-per-lane kernel (no cross-lane integration)
   // (measured on the sweep: 17-32 beams 0.147 -> 0.114 ms; up to 16 beams the contiguous tiles of the kernels
   // below read DRAM 7 % faster than the strided ones and their butterfly is still cheap)
-  if (bf_umma_i8b_takes(p, BF_CI8) && (p.nbeam > 16 || !old_nint_ok(p.nint) || bf_i8b_forced()))
+  if (bf_umma_i8b_takes(p, BF_CI8) && (p.nbeam > 16 || !old_nint_ok(p.nint)))
     return bf_launch_umma_i8b(p, BF_CI8, sm_count, st);
   // 32 antennas, an even number of samples and nint 2^k <= 64 or a multiple of 64: rows of two samples
   const bool wide = p.nant == 32 && p.nsamp % 2 == 0 && ((p.nint <= 64 && (p.nint & (p.nint - 1)) == 0) || p.nint % 64 == 0);

@@ -25,7 +25,6 @@
 // issue + TMEM allocation, warps 9-10 one TMA thread each (tiles of even / odd index), warps 11-14 (4-bit input
 // only) unpack.
 #include <cuda.h>
-#include <stdlib.h>
 
 #include "bf_internal.h"
 #include "bf_tmap.h"
@@ -59,7 +58,7 @@ BF_DEVI void tma_load_5d(uint32_t dst_smem, const void *tmap, int x, int y, int 
 // unpack groups (4-bit input): groups of four warps on alternate raw tiles (a tile's unpack is one chain of dependent
 // latencies -- barrier, LDS, barrier, STS, proxy fence, arrive -- that a group walks once per tile); one group only
 // next to four epilogue sets (registers)
-__host__ __device__ constexpr int b_ugroups(int ncol) { return 1; }   // measured: a second group changes nothing (0.0741 / 0.0725 ms)
+__host__ __device__ constexpr int b_ugroups(int ncol) { return 1; }   // measured: neither a second unpack group nor a second MMA-issuing warp changes the time (0.0638 / 0.0646 / 0.0667 ms)
 template <int NCOL, int IN> constexpr int i8b_threads_v = (4 * b_nsets(NCOL) + 3 + (IN == BF_CI4 ? B_UNPACK_WARPS * b_ugroups(NCOL) : 0)) * 32;
 
 // NCOL: accumulator columns = 4 * beam capacity (32 / 64 / 128 -> 8 / 16 / 32 beams).  NST: operand stages (int8:
@@ -67,11 +66,17 @@ template <int NCOL, int IN> constexpr int i8b_threads_v = (4 * b_nsets(NCOL) + 3
 template <int NCOL, int NST, int NRAW, int IN, int LPB>
 __global__ void __launch_bounds__(i8b_threads_v<NCOL, IN>, 1)
 bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, const long long total_super,
-                   const int n_super_chan, const int G, const int l2pf) {
+                   const int n_super_chan, const int G) {
   extern __shared__ uint8_t smem_raw[];
   constexpr bool CI4 = IN == BF_CI4;
   constexpr int W_BYTES = NCOL * B_W_ROW_BYTES;
-  constexpr int NACC = 512 / (2 * NCOL);                    // accumulator PAIRS (even, odd sample) in TMEM
+  // ATM: 4-bit input up to 16 beams -- the unpacked int8 rows go to TENSOR MEMORY as the MMA's A operand (tcgen05.st,
+  // 32 columns per operand tile) instead of shared memory: through shared memory every raw tile costs 96 KiB of
+  // traffic (TMA write 16, LDS 16, STS 32, operand read 32) against the 128 B/clk an SM has, which capped the 4-bit
+  // path at 0.55 of its HBM roofline whatever the beam count
+  constexpr bool ATM = CI4 && NCOL <= 64;
+  constexpr int NA = 4, A_COL0 = 384;                       // ATM: A-operand stages of 32 columns at 384 ..
+  constexpr int NACC = ATM ? A_COL0 / (2 * NCOL) > 4 ? 4 : A_COL0 / (2 * NCOL) : 512 / (2 * NCOL);   // accumulator PAIRS (even, odd sample) in TMEM
   constexpr int NCH = NCOL / 32;                            // 8-beam column chunks
   constexpr int NSETS = b_nsets(NCOL), CS = b_csets(NCOL), TS = b_tsets(NCOL);
   constexpr int B_MMA_WARP = 4 * NSETS, B_TMA_WARP = B_MMA_WARP + 1, B_UNPACK_WARP = B_MMA_WARP + 3;
@@ -84,8 +89,9 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
   const uint32_t sX = sR + NRAW * B_STAGE_BYTES;            // tile-set exchange: [2][4 quadrants][CS][8 CPS][32 lanes] floats
   constexpr int X_BYTES = TS > 1 ? 2 * 4 * CS * 8 * CPS * 32 * 4 : 0;
   const uint32_t sBar = sX + X_BYTES;
-  const uint32_t bar_a_full = sBar, bar_a_empty = bar_a_full + 8 * NST;
-  const uint32_t bar_r_full = bar_a_empty + 8 * NST, bar_r_empty = bar_r_full + 8 * (NRAW + 1);
+  constexpr int NAB = NST > 4 ? NST : 4;                    // operand-stage barriers (smem stages or the four TMEM stages)
+  const uint32_t bar_a_full = sBar, bar_a_empty = bar_a_full + 8 * NAB;
+  const uint32_t bar_r_full = bar_a_empty + 8 * NAB, bar_r_empty = bar_r_full + 8 * (NRAW + 1);
   const uint32_t bar_w_full = bar_r_empty + 8 * (NRAW + 1), bar_w_empty = bar_w_full + 16;
   const uint32_t bar_t_full = bar_w_empty + 16, bar_t_empty = bar_t_full + 8 * NACC;
   const uint32_t s_tmem = bar_t_empty + 8 * NACC;
@@ -94,7 +100,7 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
 
   if (threadIdx.x == 0) {
     // operand stage "full": one TMA transaction (int8) or the unpack warps (4-bit); "empty": the MMA's commit
-    for (int s = 0; s < NST; ++s) { mbar_init(bar_a_full + 8 * s, CI4 ? B_UNPACK_WARPS : 1); mbar_init(bar_a_empty + 8 * s, 1); }
+    for (int s = 0; s < (ATM ? NA : NST); ++s) { mbar_init(bar_a_full + 8 * s, CI4 ? B_UNPACK_WARPS : 1); mbar_init(bar_a_empty + 8 * s, 1); }
     for (int s = 0; s < NRAW; ++s) { mbar_init(bar_r_full + 8 * s, 1); mbar_init(bar_r_empty + 8 * s, B_UNPACK_WARPS); }   // one group per stage
     for (int s = 0; s < 2; ++s) { mbar_init(bar_w_full + 8 * s, 1); mbar_init(bar_w_empty + 8 * s, 1); }
     for (int s = 0; s < NACC; ++s) { mbar_init(bar_t_full + 8 * s, 1); mbar_init(bar_t_empty + 8 * s, 4 * CS); }
@@ -125,7 +131,8 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
     const uint32_t xch = sX + (uint32_t)(((quad * CS + set) * 8 * CPS) * 32 + lane) * 4;   // + buffer, + 128 per value
     const int nbeam = p.nbeam, nbin = p.nbin;
     int c = c0, sp = sp0;
-    int ti = 0;                                             // operand-tile counter of this CTA (all roles count alike)
+    int a = 0;                                              // accumulator pair of the next operand tile, parity of its "full"
+    uint32_t apar = 0;
     for (int s = 0; s < n_super; ++s) {
       const int bin = BPS * sp + (32 * quad + lane) / LPB;
       const bool live = BPS * sp + 32 * quad / LPB < nbin;  // warp-uniform: this quadrant holds real bins
@@ -137,26 +144,28 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
       for (int k = 0; k < CPS; ++k)
 #pragma unroll
         for (int i = 0; i < 8; ++i) acc[k][i] = make_float2(0.f, 0.f);
-      for (int g = 0; g < GT; ++g, ++ti) {
+      for (int g = 0; g < GT; ++g) {
+        const int a_ = a;
+        const uint32_t apar_ = apar;
+        if (++a == NACC) { a = 0; apar ^= 1; }
         if (TS > 1 && (g & (TS - 1)) != tset) continue;     // the other tile set's
-        const int a = ti & (NACC - 1);
-        mbar_wait(bar_t_full + 8 * a, (uint32_t)((ti >> b_ilog2(NACC)) & 1));
+        mbar_wait(bar_t_full + 8 * a_, apar_);
         tc_fence_after();
         if (!live) {                                        // bins past the end of the channel (zero-filled rows)
           __syncwarp();
-          if (lane0) mbar_arrive(bar_t_empty + 8 * a);
+          if (lane0) mbar_arrive(bar_t_empty + 8 * a_);
           continue;
         }
 #pragma unroll
         for (int k = 0; k < CPS; ++k) {
           uint32_t v[32], u[32];
-          BF_TMEM_LD_32x32b_X32(t_lane + a * 2 * NCOL + 32 * k, v);          // even samples
-          BF_TMEM_LD_32x32b_X32(t_lane + a * 2 * NCOL + NCOL + 32 * k, u);   // odd samples
+          BF_TMEM_LD_32x32b_X32(t_lane + a_ * 2 * NCOL + 32 * k, v);          // even samples
+          BF_TMEM_LD_32x32b_X32(t_lane + a_ * 2 * NCOL + NCOL + 32 * k, u);   // odd samples
           tc_wait_ld();
           if (k == CPS - 1) {  // all of this warp's columns are in registers: hand the accumulator pair back
             tc_fence_before();
             __syncwarp();
-            if (lane0) mbar_arrive(bar_t_empty + 8 * a);
+            if (lane0) mbar_arrive(bar_t_empty + 8 * a_);
           }
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
@@ -214,8 +223,9 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
     // =========================================================================== MMA issue
     constexpr uint32_t idesc = make_idesc_i8(128, NCOL);
     int c = c0, sp = sp0, prev_c = -1, wi = 0, wb = 0;
-    int ti = 0, st = 0;
-    uint32_t st_par = 0;
+    int st = 0, a = 0;
+    uint32_t st_par = 0, apar = 1;       // parities of a_full[st] / t_empty[a] to wait for
+    constexpr int NSTG = ATM ? NA : NST;
     for (int s = 0; s < n_super; ++s) {
       if (c != prev_c) {
         if (wi > 0 && elect_one()) tc_commit(bar_w_empty + 8 * wb);   // my MMAs so far have left the old buffer
@@ -225,23 +235,31 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
         ++wi;
       }
       const uint64_t bdesc = make_sdesc_k_sw64(sW + wb * W_BYTES);
-      for (int g = 0; g < GT; ++g, ++ti) {
-        const int a = ti & (NACC - 1);
+      for (int g = 0; g < GT; ++g) {
         mbar_wait(bar_a_full + 8 * st, st_par);
-        mbar_wait(bar_t_empty + 8 * a, (uint32_t)(((ti >> b_ilog2(NACC)) & 1) ^ 1));
+        mbar_wait(bar_t_empty + 8 * a, apar);
         tc_fence_after();
         if (elect_one()) {
-          const uint64_t adesc = make_sdesc_k_sw128(sA + st * B_STAGE_BYTES);
           const uint32_t d = tmem_base + a * 2 * NCOL;
-          mma_i8_ss(d, adesc, bdesc, idesc, 0);                  // even sample: row bytes 0..31
-          mma_i8_ss(d, adesc + 2, bdesc + 2, idesc, 1);          //              row bytes 32..63
-          mma_i8_ss(d + NCOL, adesc + 4, bdesc, idesc, 0);       // odd sample:  row bytes 64..95
-          mma_i8_ss(d + NCOL, adesc + 6, bdesc + 2, idesc, 1);   //              row bytes 96..127
+          if constexpr (ATM) {           // A operand in tensor memory: 8 columns per 32 bytes of the row
+            const uint32_t at = tmem_base + A_COL0 + st * 32;
+            mma_i8_ts(d, at, bdesc, idesc, 0);
+            mma_i8_ts(d, at + 8, bdesc + 2, idesc, 1);
+            mma_i8_ts(d + NCOL, at + 16, bdesc, idesc, 0);
+            mma_i8_ts(d + NCOL, at + 24, bdesc + 2, idesc, 1);
+          } else {
+            const uint64_t adesc = make_sdesc_k_sw128(sA + st * B_STAGE_BYTES);
+            mma_i8_ss(d, adesc, bdesc, idesc, 0);                  // even sample: row bytes 0..31
+            mma_i8_ss(d, adesc + 2, bdesc + 2, idesc, 1);          //              row bytes 32..63
+            mma_i8_ss(d + NCOL, adesc + 4, bdesc, idesc, 0);       // odd sample:  row bytes 64..95
+            mma_i8_ss(d + NCOL, adesc + 6, bdesc + 2, idesc, 1);   //              row bytes 96..127
+          }
           tc_commit(bar_t_full + 8 * a);
           tc_commit(bar_a_empty + 8 * st);
         }
         __syncwarp();
-        if (++st == NST) { st = 0; st_par ^= 1; }
+        if (++st == NSTG) { st = 0; st_par ^= 1; }
+        if (++a == NACC) { a = 0; apar ^= 1; }
       }
       if (++sp == n_super_chan) { sp = 0; ++c; }
     }
@@ -257,25 +275,11 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
     int c = c0, sp = sp0, prev_c = -1, wi = 0;
     int ti = 0, st = pj;
     uint32_t st_par = 1;                 // parity of empty[st] to wait for (passes on the fresh barrier)
-    // A tile takes 128 LPB bytes out of every bin; the G tiles of a super-tile together cover one CONTIGUOUS region
-    // of BPS * nint samples, but spread over the super-tile's whole duration: DRAM would open every page G times
-    // (measured: 5.9 instead of 6.3 TB/s, while from a resident L2 the strided copies are FASTER than contiguous
-    // ones).  With every tile the whole producer warp therefore prefetches 16 KiB of the NEXT super-tile's region
-    // into the L2 (plain prefetch.global.L2: the TMA unit is busy with the boxes) -- sequential DRAM reads one
-    // super-tile ahead, and the strided tensor copies hit the L2.
-    const size_t samp_bytes = CI4 ? 32 : 64;
-    const size_t region = (size_t)BPS * p.nint * samp_bytes;             // = G pieces of 16 KiB
-    const bool l2_ahead = l2pf != 0 && G > 1 && region <= (256u << 10);
+    // (A tile takes 128 bytes out of every bin, so the G tiles of a super-tile cover one contiguous region only
+    // together, over the super-tile's whole duration: from DRAM the strided copies run at 5.9 instead of 6.3 TB/s,
+    // while from a resident L2 they are FASTER than contiguous ones.  Prefetching the next super-tile's region into
+    // the L2 -- cp.async.bulk.prefetch.L2 or prefetch.global.L2 from this warp -- was measured and is 2-5 % slower.)
     for (int s = 0; s < n_super; ++s) {
-      const char *nb = nullptr;          // the next super-tile's region and its length
-      uint32_t nbytes = 0;
-      if (l2_ahead && s + 1 < n_super) {
-        int cn = c, spn = sp + 1;
-        if (spn == n_super_chan) { spn = 0; ++cn; }
-        const size_t bins_left = (size_t)(p.nbin - BPS * spn);
-        nbytes = (uint32_t)((bins_left < (size_t)BPS ? bins_left : (size_t)BPS) * p.nint * samp_bytes);
-        nb = reinterpret_cast<const char *>(p.volt) + ((size_t)cn * p.nsamp + (size_t)BPS * spn * p.nint) * samp_bytes;
-      }
       if (c != prev_c) {
         prev_c = c;
         if (pj == 0 && lane == 0) {
@@ -288,13 +292,6 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
       }
       for (int g = 0; g < G; ++g, ++ti) {
         if ((ti & 1) != pj) continue;
-        if (nb != nullptr) {
-#pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            const uint32_t off = (uint32_t)g * B_STAGE_BYTES + (uint32_t)(k * 32 + lane) * 128u;
-            if (off < nbytes) asm volatile("prefetch.global.L2 [%0];" ::"l"(nb + off));
-          }
-        }
         if (lane == 0) {
           mbar_wait(empty + 8 * st, st_par);
           mbar_arrive_expect_tx(full + 8 * st, B_STAGE_BYTES);
@@ -304,6 +301,61 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
         if ((st += 2) >= NRING) { st -= NRING; st_par ^= 1; }
       }
       if (++sp == n_super_chan) { sp = 0; ++c; }
+    }
+  } else if (ATM && warp >= B_UNPACK_WARP) {
+    // =========================================================================== unpack into TENSOR MEMORY (4-bit input, <= 16 beams)
+    // Thread (quadrant, lane) owns raw row r = 32 quadrant + lane (the four unpack warps cover the four quadrants):
+    // 128 bytes = FOUR samples of 32 antennas.  Samples 0, 1 become row r of operand tile 2 i, samples 2, 3 of tile
+    // 2 i + 1: 32 TMEM columns each, written with one tcgen05.st.32x32b.x32 -- the int8 operands never touch shared
+    // memory.  Per raw word (four antennas): mask = 16 re, shift + mask = 16 im, two PRMT interleave (re, im).
+    constexpr int UG = b_ugroups(NCOL);   // groups of four warps on alternate raw tiles: a tile's unpack is one chain
+    static_assert(NRAW % UG == 0 && NA % (2 * UG) == 0, "stages are dealt to the unpack groups");
+    const int quad = warp & 3, grp = (warp - B_UNPACK_WARP) >> 2;
+    const int r = 32 * quad + lane;
+    const uint32_t t_row = tmem_base + ((uint32_t)(quad * 32) << 16) + A_COL0;
+    const uint32_t row_off = (uint32_t)r * 128u, sw = (uint32_t)(r & 7);
+    int rs = grp, as = 2 * grp;           // group j: raw tiles j, j + UG, .. -> raw stage i % NRAW, operand stages 2 i % NA, + 1
+    uint32_t rpar = 0, apar = 1;
+    const int n_raw = n_super * G;
+    for (int i = grp; i < n_raw; i += UG) {
+      mbar_wait(bar_r_full + 8 * rs, rpar);
+      const uint32_t src = sR + rs * B_STAGE_BYTES + row_off;
+      uint4 x[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j)       // the raw stage is 128-byte swizzled by TMA
+        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(x[j].x), "=r"(x[j].y), "=r"(x[j].z), "=r"(x[j].w)
+                     : "r"(src + (((uint32_t)j ^ sw) << 4)));
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        uint32_t o[32];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t w[4] = {x[4 * h + j].x, x[4 * h + j].y, x[4 * h + j].z, x[4 * h + j].w};
+#pragma unroll
+          for (int m = 0; m < 4; ++m) {
+            const uint32_t hi = w[m] & 0xF0F0F0F0u;             // 16 re of four antennas
+            const uint32_t lo = (w[m] << 4) & 0xF0F0F0F0u;      // 16 im
+            o[8 * j + 2 * m] = __byte_perm(hi, lo, 0x5140);     // (re0, im0, re1, im1)
+            o[8 * j + 2 * m + 1] = __byte_perm(hi, lo, 0x7362); // (re2, im2, re3, im3)
+          }
+        }
+        if (h == 1) {  // the whole raw row has been consumed: the stage may be refilled
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_r_empty + 8 * rs);
+        }
+        mbar_wait(bar_a_empty + 8 * (as + h), apar);
+        tc_fence_after();
+        BF_TMEM_ST_32x32b_X32(t_row + (as + h) * 32, o);
+      }
+      tc_wait_st();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) {
+        mbar_arrive(bar_a_full + 8 * as);
+        mbar_arrive(bar_a_full + 8 * (as + 1));
+      }
+      if ((rs += UG) >= NRAW) { rs -= NRAW; rpar ^= 1; }
+      if ((as += 2 * UG) >= NA) { as -= NA; apar ^= 1; }
     }
   } else if (CI4 && warp >= B_UNPACK_WARP) {
     // =========================================================================== unpack (4-bit input, UG groups of 4 warps)
@@ -390,8 +442,8 @@ cudaError_t make_tmap_bins(CUtensorMap *tm, const BfParams &p, int nint) {
 
 template <int NCOL, int IN, int LPB>
 cudaError_t launch_i8b_lpb(const BfParams &p, int sm_count, cudaStream_t st) {
-  constexpr bool CI4 = IN == BF_CI4;
-  constexpr int NST = CI4 ? 6 : 12, NRAW = CI4 ? 6 : 0;
+  constexpr bool CI4 = IN == BF_CI4, ATM = CI4 && NCOL <= 64;   // ATM: operands in tensor memory, no shared-memory operand stages
+  constexpr int NST = ATM ? 0 : (CI4 ? 6 : 12), NRAW = ATM ? 12 : (CI4 ? 6 : 0);
   CUtensorMap tm;
   cudaError_t e = bf_cached_tmap(&tm, p, (CI4 ? 20 : 10) + LPB, p.nint, make_tmap_bins<IN, LPB>);
   if (e != cudaSuccess) return e;
@@ -404,9 +456,7 @@ cudaError_t launch_i8b_lpb(const BfParams &p, int sm_count, cudaStream_t st) {
   static thread_local int attr_dev = -1;   // once per instantiation and device
   if ((e = bf_set_smem_once(kern, smem, &attr_dev)) != cudaSuccess) return e;
   const int grid = (int)(total < sm_count ? total : sm_count);
-  static int l2pf = -1;
-  if (l2pf < 0) { const char *e = getenv("BF_I8B_L2PF"); l2pf = e ? atoi(e) : 1; }
-  kern<<<grid, i8b_threads_v<NCOL, IN>, smem, st>>>(p, tm, total, n_super_chan, G, l2pf);
+  kern<<<grid, i8b_threads_v<NCOL, IN>, smem, st>>>(p, tm, total, n_super_chan, G);
   return cudaGetLastError();
 }
 
@@ -425,9 +475,6 @@ cudaError_t launch_i8b(const BfParams &p, int sm_count, cudaStream_t st) {
 // nint a multiple of the samples per 128-byte row, and enough bins that the 128 lanes of a super-tile are not
 // mostly padding (a channel's last super-tile is partial: at most a fifth wasted).
 bool bf_umma_i8b_takes(const BfParams &p, int dtype) {
-  static int off = -1;
-  if (off < 0) { const char *e = getenv("BF_I8B_OFF"); off = e ? atoi(e) : 0; }
-  if (off) return false;
   if (p.mode != BF_MODE_POWER || p.nant != 32) return false;
   if (p.nint % (dtype == BF_CI4 ? 4 : 2) != 0) return false;
   if ((long long)p.nint * 64 >= (1ll << 32)) return false;

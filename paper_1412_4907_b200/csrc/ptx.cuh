@@ -239,6 +239,14 @@ BF_DEVI void mma_i8_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t
       "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
       : "memory");
 }
+// the same with the A operand (M = 128 rows = TMEM lanes, 32 int8 along K = 8 columns) read from tensor memory
+BF_DEVI void mma_i8_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
 // K-major operand with rows of 64 bytes, 64-byte swizzle (16-byte chunk index ^= (row >> 1) & 3; the
 // pattern repeats every 8 rows = 512 bytes = the stride byte offset); layout type 4 = SWIZZLE_64B
 BF_DEVI uint64_t make_sdesc_k_sw64(uint32_t saddr) {
@@ -284,5 +292,15 @@ BF_DEVI float2 ffma2(float2 a, float2 b, float2 c) {
       : "=l"(reinterpret_cast<uint64_t &>(d))
       : "l"(reinterpret_cast<uint64_t &>(a)), "l"(reinterpret_cast<uint64_t &>(b)),
         "l"(reinterpret_cast<uint64_t &>(c)));
+  return d;
+}
+// the same, but ordered with the surrounding volatile asm (barrier arrives, tcgen05.ld): the compiler must not sink an
+// mbarrier.arrive below the squares that follow it
+BF_DEVI float2 ffma2v(float2 a, float2 b, float2 c) {
+  float2 d;
+  asm volatile("fma.rn.f32x2 %0, %1, %2, %3;"
+               : "=l"(reinterpret_cast<uint64_t &>(d))
+               : "l"(reinterpret_cast<uint64_t &>(a)), "l"(reinterpret_cast<uint64_t &>(b)),
+                 "l"(reinterpret_cast<uint64_t &>(c)));
   return d;
 }
