@@ -39,7 +39,8 @@ METRIC = "beamforming TFLOP/s (8 flop/complex MAC)"
 UNIT = "TFLOP/s"
 L2_BYTES = 126e6
 ALL_CONFIGS = ["tiny", "sweep-1", "sweep-4", "sweep-16", "sweep-64", "sweep-256", "sweep-1024", "large-N", "streaming"]
-F1_CONFIGS = ["medium-ci4", "sweep-ci4-16", "sweep-ci4-64", "streaming-ci4"]   # the paper's 4+4-bit input
+EXTRA_CONFIGS = ["sweep-32"]   # not a BASELINE.json point: the top of the int8-operand kernel's range
+F1_CONFIGS = ["medium-ci4", "sweep-ci4-1", "sweep-ci4-16", "sweep-ci4-64", "streaming-ci4"]   # the paper's 4+4-bit input
 
 
 def load_peaks():
@@ -572,7 +573,7 @@ def main():
                               "frac_of_burst": roof.get("frac_of_burst"), "frac_of_sustained": roof.get("frac_of_sustained"),
                               "achieved": roof["achieved"], "unit": roof["unit"], "traffic": roof["traffic"], "kernel": kernel_name,
                               "tflops": flop_step / (avg_kernel_ms * 1e-3) / 1e12, "steps": K, "clocks": clocks, "l2": l2_note}}
-        for name in ALL_CONFIGS + F1_CONFIGS:
+        for name in ALL_CONFIGS + EXTRA_CONFIGS + F1_CONFIGS:
             wc = workload_for(name)
             Tc = Timed(bf, synthetic, torch, wc, dev, bf.BF_KERNEL_AUTO)
             Kc = 200 if name == "tiny" else 30

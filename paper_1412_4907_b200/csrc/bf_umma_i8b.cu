@@ -38,6 +38,9 @@ constexpr int B_W_ROW_BYTES = 64;                      // coefficient rows (bf_i
 #ifndef B_SETS_MAX
 #define B_SETS_MAX 4
 #endif
+#ifndef B_WAIT_NS
+#define B_WAIT_NS 400
+#endif
 constexpr int B_UNPACK_WARPS = 4;
 // epilogue sets of four warps (one per TMEM lane quadrant): CS column sets split the 8-beam chunks of a tile, TS tile
 // sets take alternate tiles of a super-tile (their partial sums meet in shared memory at its end).  A warp's work on
@@ -127,7 +130,12 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
     // =========================================================================== epilogue
     const int quad = warp & 3, set = (warp >> 2) % CS, tset = (warp >> 2) / CS;
     const bool lane0 = lane == 0;
-    const uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16) + set * (CPS * 32);
+    // The kernel is bound by the instructions its sub-partitions issue (profiles/r02_ncu_full_summary.md: issue slots
+    // 74-76 % busy at 16-32 beams), so the visit to an accumulator pair is kept lean: barrier and TMEM base addresses
+    // live in registers, and everything that does not change inside a super-tile is hoisted out of its tile loop.
+    uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16) + set * (CPS * 32);
+    uint32_t bt_full = bar_t_full;
+    asm volatile("" : "+r"(t_lane), "+r"(bt_full));          // keep in registers, do not rematerialise
     const uint32_t xch = sX + (uint32_t)(((quad * CS + set) * 8 * CPS) * 32 + lane) * 4;   // + buffer, + 128 per value
     const int nbeam = p.nbeam, nbin = p.nbin;
     int c = c0, sp = sp0;
@@ -149,23 +157,25 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
         const uint32_t apar_ = apar;
         if (++a == NACC) { a = 0; apar ^= 1; }
         if (TS > 1 && (g & (TS - 1)) != tset) continue;     // the other tile set's
-        mbar_wait(bar_t_full + 8 * a_, apar_);
+        const uint32_t bf_a = bt_full + 8 * a_;             // "full" of this accumulator pair; its "empty" is NACC barriers on
+        mbar_wait_hinted(bf_a, apar_, B_WAIT_NS);
         tc_fence_after();
         if (!live) {                                        // bins past the end of the channel (zero-filled rows)
           __syncwarp();
-          if (lane0) mbar_arrive(bar_t_empty + 8 * a_);
+          if (lane0) mbar_arrive(bf_a + 8 * NACC);
           continue;
         }
+        const uint32_t t_acc = t_lane + a_ * (2 * NCOL);
 #pragma unroll
         for (int k = 0; k < CPS; ++k) {
           uint32_t v[32], u[32];
-          BF_TMEM_LD_32x32b_X32(t_lane + a_ * 2 * NCOL + 32 * k, v);          // even samples
-          BF_TMEM_LD_32x32b_X32(t_lane + a_ * 2 * NCOL + NCOL + 32 * k, u);   // odd samples
+          BF_TMEM_LD_32x32b_X32(t_acc + 32 * k, v);          // even samples
+          BF_TMEM_LD_32x32b_X32(t_acc + NCOL + 32 * k, u);   // odd samples
           tc_wait_ld();
           if (k == CPS - 1) {  // all of this warp's columns are in registers: hand the accumulator pair back
             tc_fence_before();
             __syncwarp();
-            if (lane0) mbar_arrive(bar_t_empty + 8 * a_);
+            if (lane0) mbar_arrive(bf_a + 8 * NACC);
           }
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
