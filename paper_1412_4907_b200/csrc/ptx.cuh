@@ -145,9 +145,10 @@ BF_DEVI void mbar_wait_tight(uint32_t bar, uint32_t parity) {
 }
 
 
-// Bounded wait for roles with MANY waiting warps (the int8-operand kernels' epilogue sets): try_wait with a
-// suspend-time hint, so that a waiting warp sleeps in hardware instead of taking two issue slots every ~40 clk from
-// the warps that work (ncu, sweep-ci4 at 16 beams: a sixth of all instructions were such polls)
+// Bounded wait for roles with MANY waiting warps (the bin-per-lane int8-operand kernel's epilogue sets): try_wait with a
+// suspend-time hint.  The poll count does not fall (ncu: still ~25 polls per visit), but the waits come out 1-2 %
+// faster on sweep-32 and sweep-ci4-16 than the tight spin; in the resident fp16 kernel the same wait is 7 % SLOWER at
+// 64 beams (A/B on one box), so that kernel keeps mbar_wait_tight.
 BF_DEVI void mbar_wait_hinted(uint32_t bar, uint32_t parity, uint32_t ns) {
   if (mbar_try_wait(bar, parity)) return;
   for (uint32_t n = 0;; ++n) {
