@@ -45,9 +45,10 @@ constexpr int B_UNPACK_WARPS = 4;
 // epilogue sets of four warps (one per TMEM lane quadrant): CS column sets split the 8-beam chunks of a tile, TS tile
 // sets take alternate tiles of a super-tile (their partial sums meet in shared memory at its end).  A warp's work on
 // a tile is one chain -- barrier, tcgen05.ld, 5 instructions per beam and sample -- of 300-400 clk whatever the beam
-// count, so up to 16 beams (one chunk per warp) two tile sets are needed to keep up with 4-bit input.
+// count; with a single chunk (<= 8 beams) two tile sets keep up with 4-bit input (at 9-16 beams two column sets
+// alone measured faster than 2 x 2 sets: fewer warps polling).
 __host__ __device__ constexpr int b_csets(int ncol) { return ncol / 32 >= 4 ? 4 : (ncol / 32 >= 2 ? 2 : 1); }
-__host__ __device__ constexpr int b_tsets(int ncol) { return ncol / 32 >= 4 ? 1 : 2; }
+__host__ __device__ constexpr int b_tsets(int ncol) { return ncol / 32 >= 2 ? 1 : 2; }
 __host__ __device__ constexpr int b_nsets(int ncol) { return b_csets(ncol) * b_tsets(ncol); }
 
 __host__ __device__ constexpr int b_ilog2(int x) { return x <= 1 ? 0 : 1 + b_ilog2(x >> 1); }

@@ -219,3 +219,47 @@ except bf.BfError as e:
     lines = [ln for ln in r.stdout.splitlines() if ln.startswith("RESULT")]
     assert lines, (r.returncode, r.stdout[-500:], r.stderr[-1500:])
     assert lines[0].split()[1] == "-3", lines[0]          # BF_ECUDA
+
+
+@pytest.mark.parametrize("dtype,nbeam", [("ci8", 24), ("ci4", 12), ("ci4", 28)])
+def test_bin_per_lane_kernel_with_gains_chunks_and_tracking(bf, dtype, nbeam):
+    """The bin-per-lane int8-operand kernel (bf_umma_i8b.cu: 17-32 beams on int8 input, <= 32 beams on 4+4-bit input, its
+    <= 16-beam form with the operands in tensor memory) behind the rest of the API: per-channel antenna gains folded into
+    its two-limb weights, bf_run_host's channel chunks (other base pointers and channel counts: fresh tensor maps), and a
+    tracking update that switches its weight buffer.  256 bins per channel, so the automatic choice is this kernel."""
+    import torch
+    N, C, T, I = 32, 6, 4096, 16
+    w = synthetic.make_case(N, C, nbeam, T, I, dtype, seed=21)
+    v = w.make_voltages()
+    if dtype == "ci8":
+        x = v[..., 0].astype(np.float64) + 1j * v[..., 1]
+    else:  # high nibble re, low nibble im, two's complement (DESIGN.md A20)
+        re = (v >> 4).astype(np.int16); im = (v & 0xF).astype(np.int16)
+        x = np.where(re > 7, re - 16, re).astype(np.float64) + 1j * np.where(im > 7, im - 16, im)
+    rng = np.random.default_rng(5)
+    g = rng.uniform(0.5, 1.5, (C, N)) * np.exp(2j * np.pi * rng.random((C, N)))
+    dirs = [w.beam_dir, np.roll(w.beam_dir, 3, axis=0)]
+    refs = [oracle.beamform(w.ant_xyz, w.freqs, d, np.ascontiguousarray(x * g[:, None, :]), I) for d in dirs]
+    B = bf.Beamformer(N, C, nbeam, T, I, dtype=bf_dtype(bf, w), weight_buffers=2)
+    assert B.kernel_name == "umma-i8"
+    B.set_antenna_gains(g, per_channel=True)
+    B.set_geometry(w.ant_xyz, w.freqs, dirs[0])
+    vd = torch.from_numpy(v).cuda()
+    direct = B.run(vd).cpu().numpy()
+    err = (np.abs(direct - refs[0]).max(axis=-1) / refs[0].mean(axis=-1)).max()
+    assert err <= 1e-3, err
+    cs, xs = torch.cuda.Stream(), torch.cuda.Stream()
+    pinned = torch.from_numpy(v).pin_memory()
+    for cpc in (4, 1):   # 6 channels in chunks of 4 + 2, then one by one
+        hp = torch.empty((C, nbeam, T // I), dtype=torch.float32).pin_memory()
+        hp.fill_(float("nan"))
+        B.run_host(pinned, hp, cpc, cs, xs)
+        cs.synchronize(); xs.synchronize()
+        np.testing.assert_array_equal(hp.numpy(), direct)
+    upd = torch.cuda.Stream()
+    B.update_geometry(w.ant_xyz, w.freqs, dirs[1], update_stream=upd)
+    out1 = B.run(vd).cpu().numpy()
+    err = (np.abs(out1 - refs[1]).max(axis=-1) / refs[1].mean(axis=-1)).max()
+    assert err <= 1e-3, err
+    assert (np.abs(refs[1] - refs[0]).max(axis=-1) / refs[0].mean(axis=-1)).max() > 0.05
+    B.close()
