@@ -56,7 +56,9 @@ enum bf_dtype {
 
 enum bf_kernel {
   BF_KERNEL_AUTO = 0, /* pick the fastest kernel that supports the shape.  NOTE: for shapes no tensor-core kernel takes (nant
-                         not a multiple of 8 (int8) / 4 (fp16) / 16 (4+4-bit), nint neither 2^k <= 64 nor a multiple of 64 / 32)
+                         not a multiple of 8 (int8) / 4 (fp16) / 16 (4+4-bit), nint neither 2^k <= 64 nor a multiple of 64 / 32 -- except on
+                         32 antennas with <= 32 beams, where any EVEN nint integrates on tensor cores when nsamp / nint is a
+                         multiple of 128 or >= 512)
                          AUTO falls through to BF_KERNEL_SIMT without an error -- about 30x slower on the `tiny` shape;
                          bf_kernel_name / bf_selected_kernel say which family will run, and BF_KERNEL_UMMA turns the
                          fall-through into BF_EUNSUPPORTED */
@@ -64,7 +66,8 @@ enum bf_kernel {
   BF_KERNEL_UMMA = 2, /* tcgen05/TMEM tensor-core kernels with the fused |.|^2 + integrate epilogue (the library
                          picks the variant) */
   BF_KERNEL_UMMA_F16 = 3, /* only the fp16-operand variants (int8 input converted in-kernel) */
-  BF_KERNEL_UMMA_I8 = 4   /* only the int8-operand variant (kind::i8, two-limb weights; few beams, nant <= 32) */
+  BF_KERNEL_UMMA_I8 = 4   /* only the int8-operand variants (kind::i8, two-limb weights; <= 32 beams, nant <= 32; int8 input, and
+                             4+4-bit input on 32 antennas with nint % 4 == 0 and nsamp / nint a multiple of 128 or >= 512) */
 };
 
 /*
