@@ -132,6 +132,12 @@ SMALL = [
     (64, 2, 9, 512, 4, "ci4"),       # K-blocked with two-term coefficients
     (32, 40, 64, 5000, 8, "ci8"),    # 800 items: 5-6 per CTA, both convert groups busy, ragged tail (5000 = 19*256 + 136)
     (32, 30, 100, 3000, 4, "ci4"),   # same for the 4-bit unpack, two M-tiles per item
+    # 33-64 beams with >= 256-bin channels: the bin-per-lane kernel with the voltages in tensor memory (bf_umma_bl.cu)
+    (32, 2, 64, 8192, 16, "ci8"),    # 512 bins: two super-tile pairs per channel, eight raw-tile pairs per item
+    (32, 3, 33, 4096, 16, "ci8"),    # 256 bins: one pair per channel, the second 16-beam chunk holds a single beam
+    (32, 1, 50, 34816, 32, "ci8"),   # 1088 bins = 4 pairs + 64 bins: the last pair is half a super-tile X and an empty Y
+    (32, 5, 64, 9216, 18, "ci8"),    # nint = 18: any even bin length >= 16; 512 bins, CTA ranges straddle channels
+    (32, 2, 40, 65536, 256, "ci8"),  # long bins: 128 raw-tile pairs per item
 ]
 
 
@@ -320,6 +326,7 @@ EXTREME_CASES = [
     # nant nchan nbeam nsamp nint dtype kernel            which kernel this lands on
     (32, 2, 64, 1024, 16, "ci8", "f16"),                  # resident fp16 kernel, int8 -> fp16 0x6400|(x^0x80) at x = 0x80
     (32, 2, 130, 512, 64, "ci8", "auto"),                 # resident, beam groups of 4
+    (32, 2, 64, 4096, 16, "ci8", "auto"),                 # bin-per-lane fp16 kernel (bf_umma_bl.cu): -128 through tcgen05.st operands
     (16, 2, 9, 512, 16, "ci8", "f16"),                    # resident, short rows (generic piece table)
     (64, 2, 33, 512, 32, "ci8", "auto"),                  # K-blocked kernel, int8 input
     (32, 2, 16, 1024, 16, "ci8", "i8"),                   # int8-operand kernel, WIDE: kind::i8 with -128 x limb
