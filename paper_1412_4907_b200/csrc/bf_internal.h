@@ -115,7 +115,7 @@ cudaError_t bf_launch_umma_i8(const BfParams &p, int dtype, int sm_count, cudaSt
 bool bf_umma_i8b_takes(const BfParams &p, int dtype);   // bf_umma_i8b.cu: one output bin per TMEM lane
 cudaError_t bf_launch_umma_i8b(const BfParams &p, int dtype, int sm_count, cudaStream_t st);
 bool bf_umma_bl_takes(const BfParams &p, int dtype);    // bf_umma_bl.cu: 33-64 beams, bin per lane, voltages as the A operand in TMEM
-cudaError_t bf_launch_umma_bl(const BfParams &p, int sm_count, cudaStream_t st);
+cudaError_t bf_launch_umma_bl(const BfParams &p, int dtype, int sm_count, cudaStream_t st);
 cudaError_t bf_launch_incoherent(const bf_ctx *c, const void *volt, float *out, cudaStream_t st);
 cudaError_t bf_launch_umma(const BfParams &p, int dtype, int sm_count, cudaStream_t st);
 cudaError_t bf_launch_umma_kblock(const BfParams &p, int dtype, int sm_count, cudaStream_t st);

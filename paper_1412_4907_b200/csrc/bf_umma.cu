@@ -558,6 +558,6 @@ cudaError_t bf_launch_umma(const BfParams &p, int dtype, int sm_count, cudaStrea
   if (v != 1) return cudaErrorNotSupported;
   // 33-64 beams on 32 antennas, bins of an even number >= 16 of samples: the bin-per-lane kernel with the voltages in
   // tensor memory (bf_umma_bl.cu; sweep at 64 / 48 / 40 beams 0.168 / 0.151 / 0.146 -> 0.145 / 0.137 / 0.132 ms)
-  if (p.nbeam > 32 && bf_umma_bl_takes(p, dtype)) return bf_launch_umma_bl(p, sm_count, st);
+  if (p.nbeam > 32 && bf_umma_bl_takes(p, dtype)) return bf_launch_umma_bl(p, dtype, sm_count, st);
   return dtype == BF_CI4 ? launch_k64_in<BF_CI4>(p, sm_count, st) : launch_k64_in<BF_CI8>(p, sm_count, st);
 }

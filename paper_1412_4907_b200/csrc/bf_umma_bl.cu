@@ -47,8 +47,9 @@ BF_DEVI void bl_tma_load_5d(uint32_t dst_smem, const void *tmap, int x, int y, i
       ::"r"(dst_smem), "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(w), "r"(v), "r"(bar) : "memory");
 }
 
-// NRAW: raw stages.  n_items = channels x super-tile pairs per channel (nSP2), the pair fastest.
-template <int NRAW>
+// NRAW: raw stages.  IN: BF_CI8 (raw rows of 128 bytes = two samples) or BF_CI4 (the paper's 4+4-bit bytes, PAPER.md:102:
+// raw rows of 64 bytes = two samples, 64-byte swizzle).  n_items = channels x super-tile pairs per channel (nSP2).
+template <int NRAW, int IN>
 __global__ void __launch_bounds__(BL_THREADS, 1)
 bf_umma_bl_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, const long long total_items, const int nSP2,
                   const int G) {
@@ -56,6 +57,7 @@ bf_umma_bl_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sW = smem_base;                                  // 2 coefficient buffers (one tile = 64 beams each)
   const uint32_t sR = sW + 2 * A_TILE_BYTES;                      // NRAW raw stages
+  constexpr int RAW_BYTES = IN == BF_CI4 ? BL_RAW_BYTES / 2 : BL_RAW_BYTES;
   const uint32_t sBar = sR + NRAW * BL_RAW_BYTES;
   const uint32_t bar_r_full = sBar, bar_r_empty = bar_r_full + 8 * NRAW;
   const uint32_t bar_a_full = bar_r_empty + 8 * NRAW, bar_a_empty = bar_a_full + 8 * BL_NA;
@@ -164,26 +166,40 @@ bf_umma_bl_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
     const int quad = warp & 3;
     const int r = 32 * quad + lane;
     const uint32_t t_row = tmem_base + ((uint32_t)(quad * 32) << 16) + BL_A_COL0;
-    const uint32_t row_off = (uint32_t)r * 128u, sw = (uint32_t)(r & 7);
+    const uint32_t row_off = IN == BF_CI4 ? (uint32_t)r * 64u : (uint32_t)r * 128u;
+    const uint32_t sw = IN == BF_CI4 ? (uint32_t)((r >> 1) & 3) : (uint32_t)(r & 7);   // 64- / 128-byte swizzle of the TMA box
     int rs = 0, as = 0;
     uint32_t rpar = 0, apar = 1;
     const int n_raw = n_items * 2 * G;
     for (int i = 0; i < n_raw; ++i) {
       mbar_wait(bar_r_full + 8 * rs, rpar);
       const uint32_t src = sR + rs * BL_RAW_BYTES + row_off;
-      uint4 x[8];
+      constexpr int NX = IN == BF_CI4 ? 4 : 8;                     // 16-byte pieces per raw row
+      uint4 x[NX];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) x[j] = ld_shared_v4(src + ((j ^ sw) << 4));   // the raw stage is 128-byte swizzled by TMA
+      for (int j = 0; j < NX; ++j) x[j] = ld_shared_v4(src + ((j ^ sw) << 4));
 #pragma unroll
       for (int h = 0; h < 2; ++h) {                                // sample E, sample O
         uint32_t o[32];
+        if constexpr (IN == BF_CI4) {                              // 32 bytes = 32 antennas -> 32 half2 (re, im), exact
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const uint4 w = x[4 * h + j];
-          cvt_i8x4_f16x4(w.x, o[8 * j + 0], o[8 * j + 1]);
-          cvt_i8x4_f16x4(w.y, o[8 * j + 2], o[8 * j + 3]);
-          cvt_i8x4_f16x4(w.z, o[8 * j + 4], o[8 * j + 5]);
-          cvt_i8x4_f16x4(w.w, o[8 * j + 6], o[8 * j + 7]);
+          for (int j = 0; j < 2; ++j) {
+            const uint4 w = x[2 * h + j];
+            uint32_t t[4];
+            cvt_i4x8_f16x8(w.x, t); o[16 * j + 0] = t[0]; o[16 * j + 1] = t[1]; o[16 * j + 2] = t[2]; o[16 * j + 3] = t[3];
+            cvt_i4x8_f16x8(w.y, t); o[16 * j + 4] = t[0]; o[16 * j + 5] = t[1]; o[16 * j + 6] = t[2]; o[16 * j + 7] = t[3];
+            cvt_i4x8_f16x8(w.z, t); o[16 * j + 8] = t[0]; o[16 * j + 9] = t[1]; o[16 * j + 10] = t[2]; o[16 * j + 11] = t[3];
+            cvt_i4x8_f16x8(w.w, t); o[16 * j + 12] = t[0]; o[16 * j + 13] = t[1]; o[16 * j + 14] = t[2]; o[16 * j + 15] = t[3];
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const uint4 w = x[4 * h + j];
+            cvt_i8x4_f16x4(w.x, o[8 * j + 0], o[8 * j + 1]);
+            cvt_i8x4_f16x4(w.y, o[8 * j + 2], o[8 * j + 3]);
+            cvt_i8x4_f16x4(w.z, o[8 * j + 4], o[8 * j + 5]);
+            cvt_i8x4_f16x4(w.w, o[8 * j + 6], o[8 * j + 7]);
+          }
         }
         if (h == 1) {  // the raw row is in registers (both halves consumed): the stage may be refilled
           __syncwarp();
@@ -276,7 +292,7 @@ bf_umma_bl_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
 #pragma unroll
         for (int h = 0; h < 2; ++h) {   // row g of super-tile X, then of Y (bins past nbin are zero-filled)
           mbar_wait(bar_r_empty + 8 * rs, rpar);
-          mbar_arrive_expect_tx(bar_r_full + 8 * rs, BL_RAW_BYTES);
+          mbar_arrive_expect_tx(bar_r_full + 8 * rs, RAW_BYTES);
           bl_tma_load_5d(sR + rs * BL_RAW_BYTES, &tmap, 0, 0, 128 * (2 * q + h), g, c, bar_r_full + 8 * rs);
           if (++rs == NRAW) { rs = 0; rpar ^= 1; }
         }
@@ -291,43 +307,51 @@ bf_umma_bl_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
   probe_mark(p.probe, 1);
 }
 
-// 5-D view of one launch's int8 voltages: {byte in row, 1, bin, row in bin, channel}, a row = 128 bytes = two samples;
-// box {128, 1, 128, 1, 1}: row g of 128 consecutive bins, 128-byte swizzle; bins past nbin are zero-filled
+// 5-D view of one launch's voltages: {byte in row, 1, bin, row in bin, channel}, a row = two samples (128 bytes of int8,
+// 64 bytes of 4+4-bit); box {row, 1, 128, 1, 1}: row g of 128 consecutive bins; bins past nbin are zero-filled
+template <int IN>
 cudaError_t bl_make_tmap(CUtensorMap *tm, const BfParams &p, int nint) {
   PFN_encodeTiled enc = bf_get_encode();
   if (!enc) return cudaErrorNotSupported;
-  cuuint64_t dims[5] = {128, 1, (cuuint64_t)p.nbin, (cuuint64_t)(nint / 2), (cuuint64_t)p.nchan_run};
-  cuuint64_t strides[4] = {128, (cuuint64_t)nint * 64, 128, (cuuint64_t)p.nsamp * 64};
-  cuuint32_t box[5] = {128, 1, 128, 1, 1};
+  constexpr cuuint32_t ROW = IN == BF_CI4 ? 64 : 128;
+  cuuint64_t dims[5] = {ROW, 1, (cuuint64_t)p.nbin, (cuuint64_t)(nint / 2), (cuuint64_t)p.nchan_run};
+  cuuint64_t strides[4] = {ROW, (cuuint64_t)nint * (ROW / 2), ROW, (cuuint64_t)p.nsamp * (ROW / 2)};
+  cuuint32_t box[5] = {ROW, 1, 128, 1, 1};
   cuuint32_t estr[5] = {1, 1, 1, 1, 1};
   CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 5, const_cast<void *>(p.volt), dims, strides, box, estr,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, IN == BF_CI4 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-}  // namespace
-
-// Shapes this kernel takes: complex int8, 32 antennas, up to 64 beams (one coefficient tile), power mode, single-term
-// coefficients (nint >= BF_LO_NINT), even nint, and enough bins that the 256 lanes of an item are not mostly padding
-bool bf_umma_bl_takes(const BfParams &p, int dtype) {
-  if (dtype != BF_CI8 || p.mode != BF_MODE_POWER || p.nant != 32 || p.nMt != 1 || p.wop_lo != nullptr) return false;
-  if (p.nint < BF_LO_NINT || p.nint % 2 != 0 || (long long)p.nint * 64 >= (1ll << 32)) return false;
-  return p.nbin % 256 == 0 || p.nbin >= 1024;
-}
-
-cudaError_t bf_launch_umma_bl(const BfParams &p, int sm_count, cudaStream_t st) {
+template <int IN>
+cudaError_t launch_bl(const BfParams &p, int sm_count, cudaStream_t st) {
   constexpr int NRAW = 11;
   CUtensorMap tm;
-  cudaError_t e = bf_cached_tmap(&tm, p, 30, p.nint, bl_make_tmap);
+  cudaError_t e = bf_cached_tmap(&tm, p, IN == BF_CI4 ? 31 : 30, p.nint, bl_make_tmap<IN>);
   if (e != cudaSuccess) return e;
   const int nSP2 = (p.nbin + 255) / 256;
   const long long total = (long long)p.nchan_run * nSP2;
   const size_t smem = 1024 + 2 * A_TILE_BYTES + (size_t)NRAW * BL_RAW_BYTES + 512;
-  auto kern = bf_umma_bl_kernel<NRAW>;
+  auto kern = bf_umma_bl_kernel<NRAW, IN>;
   static thread_local int attr_dev = -1;
   if ((e = bf_set_smem_once(kern, smem, &attr_dev)) != cudaSuccess) return e;
   const int grid = (int)(total < sm_count ? total : sm_count);
   kern<<<grid, BL_THREADS, smem, st>>>(p, tm, total, nSP2, p.nint / 2);
   return cudaGetLastError();
+}
+
+}  // namespace
+
+// Shapes this kernel takes: complex int8 or 4+4-bit input, 32 antennas, up to 64 beams (one coefficient tile), power mode,
+// single-term coefficients (nint >= BF_LO_NINT), even nint, and enough bins that the 256 lanes of an item are not mostly
+// padding
+bool bf_umma_bl_takes(const BfParams &p, int dtype) {
+  if ((dtype != BF_CI8 && dtype != BF_CI4) || p.mode != BF_MODE_POWER || p.nant != 32 || p.nMt != 1 || p.wop_lo != nullptr) return false;
+  if (p.nint < BF_LO_NINT || p.nint % 2 != 0 || (long long)p.nint * 64 >= (1ll << 32)) return false;
+  return p.nbin % 256 == 0 || p.nbin >= 1024;
+}
+
+cudaError_t bf_launch_umma_bl(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
+  return dtype == BF_CI4 ? launch_bl<BF_CI4>(p, sm_count, st) : launch_bl<BF_CI8>(p, sm_count, st);
 }

@@ -138,6 +138,9 @@ SMALL = [
     (32, 1, 50, 34816, 32, "ci8"),   # 1088 bins = 4 pairs + 64 bins: the last pair is half a super-tile X and an empty Y
     (32, 5, 64, 9216, 18, "ci8"),    # nint = 18: any even bin length >= 16; 512 bins, CTA ranges straddle channels
     (32, 2, 40, 65536, 256, "ci8"),  # long bins: 128 raw-tile pairs per item
+    (32, 2, 64, 8192, 16, "ci4"),    # the same kernel on 4+4-bit input: raw rows of 64 bytes, 64-byte swizzle
+    (32, 1, 50, 34816, 32, "ci4"),   # partial last pair
+    (32, 3, 33, 5120, 20, "ci4"),    # nint = 20, 256 bins
 ]
 
 
@@ -290,7 +293,7 @@ def test_coherent_gain_property(bf):
 
 
 # ------------------------------------------------------------------ full BASELINE.json sizes, EVERY channel
-FULL = [("medium", None), ("medium-ci4", None), ("streaming-ci4", None), ("sweep-ci4", 16), ("sweep", 1), ("sweep", 4), ("sweep", 16), ("sweep", 64), ("sweep", 256),
+FULL = [("medium", None), ("medium-ci4", None), ("streaming-ci4", None), ("sweep-ci4", 16), ("sweep-ci4", 64), ("sweep", 1), ("sweep", 4), ("sweep", 16), ("sweep", 64), ("sweep", 256),
         ("sweep", 1024), ("large-N", None), ("streaming", None)]
 
 
@@ -327,6 +330,7 @@ EXTREME_CASES = [
     (32, 2, 64, 1024, 16, "ci8", "f16"),                  # resident fp16 kernel, int8 -> fp16 0x6400|(x^0x80) at x = 0x80
     (32, 2, 130, 512, 64, "ci8", "auto"),                 # resident, beam groups of 4
     (32, 2, 64, 4096, 16, "ci8", "auto"),                 # bin-per-lane fp16 kernel (bf_umma_bl.cu): -128 through tcgen05.st operands
+    (32, 2, 64, 4096, 16, "ci4", "auto"),                 # the same kernel's nibble unpack
     (16, 2, 9, 512, 16, "ci8", "f16"),                    # resident, short rows (generic piece table)
     (64, 2, 33, 512, 32, "ci8", "auto"),                  # K-blocked kernel, int8 input
     (32, 2, 16, 1024, 16, "ci8", "i8"),                   # int8-operand kernel, WIDE: kind::i8 with -128 x limb
