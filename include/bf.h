@@ -96,7 +96,7 @@ int bf_set_kernel(bf_ctx *ctx, int kernel);
  * PAPER.md:66-98) or BF_KERNEL_UMMA (tensor cores: the N_b x N_a matrix product of PAPER.md:62). */
 int bf_selected_kernel(const bf_ctx *ctx);
 
-/* Name of the kernel bf_run will launch: "simt", "umma-f16-resident", "umma-f16-kblock", "umma-i8". */
+/* Name of the kernel bf_run will launch: "simt", "umma-f16-resident", "umma-f16-binlane", "umma-f16-kblock", "umma-i8". */
 const char *bf_kernel_name(const bf_ctx *ctx);
 
 /* Number of kernels this context has launched so far (all streams), for accounting (the bench line's
