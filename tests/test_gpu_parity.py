@@ -503,3 +503,36 @@ def test_run_host_and_streaming_match_run(bf, name):
     check_rows(P[2].cpu().numpy(), ref)
     assert B.launches >= 1 + 3 + 3 + 3
     B.close()
+
+
+GUARD_CASES = [
+    # nant nchan nbeam nsamp nint dtype   -- partial last super-tile (pair), beam counts that do not fill a chunk
+    (32, 2, 17, 20480, 32, "ci8"),    # bf_umma_i8b.cu, 640 bins
+    (32, 2, 5, 5120, 8, "ci4"),       # bf_umma_i8b.cu, 4-bit input, operands in tensor memory
+    (32, 2, 28, 10240, 16, "ci4"),    # bf_umma_i8b.cu, 4-bit input, shared-memory operand stages
+    (32, 1, 50, 34816, 32, "ci8"),    # bf_umma_bl.cu, 1088 bins: half a super-tile X and an empty Y at the end
+    (32, 1, 33, 34816, 32, "ci4"),    # bf_umma_bl.cu, 4-bit input
+]
+
+
+@pytest.mark.parametrize("case", GUARD_CASES, ids=lambda c: "N%d-C%d-B%d-T%d-I%d-%s" % c)
+def test_bin_per_lane_kernels_write_only_their_output(bf, case):
+    """compute-sanitizer is not available on the GPU pool, so the bounds of the kernels whose tiles overhang the data
+    (TMA zero-fills bins past nbin; lanes and beam slots past the end must not store) are checked with guard words on
+    both sides of the power cube."""
+    import torch
+    N, C, B, T, I, dtype = case
+    w = synthetic.make_case(N, C, B, T, I, dtype, seed=31)
+    v = torch.from_numpy(w.make_voltages()).cuda()
+    n, guard = C * B * (T // I), 4096
+    big = torch.full((n + 2 * guard,), -12345.0, dtype=torch.float32, device="cuda")
+    P = big[guard:guard + n].view(C, B, T // I)
+    Bf = bf.Beamformer(N, C, B, T, I, dtype=bf_dtype(bf, w))
+    Bf.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
+    assert Bf.kernel_name in ("umma-i8", "umma-f16-binlane"), Bf.kernel_name
+    Bf.run(v, P)
+    torch.cuda.synchronize()
+    assert (big[:guard] == -12345.0).all() and (big[guard + n:] == -12345.0).all()
+    ref = oracle.beamform(w.ant_xyz, w.freqs, w.beam_dir, v.cpu().numpy(), I)
+    check_rows(P.cpu().numpy(), ref)
+    Bf.close()
