@@ -83,6 +83,7 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
   constexpr int NACC = ATM ? A_COL0 / (2 * NCOL) > 4 ? 4 : A_COL0 / (2 * NCOL) : 512 / (2 * NCOL);   // accumulator PAIRS (even, odd sample) in TMEM
   constexpr int NCH = NCOL / 32;                            // 8-beam column chunks
   constexpr int NSETS = b_nsets(NCOL), CS = b_csets(NCOL), TS = b_tsets(NCOL);
+  static_assert(TS == 1 || NACC % TS == 0, "an accumulator slot must always belong to the same tile set");
   constexpr int B_MMA_WARP = 4 * NSETS, B_TMA_WARP = B_MMA_WARP + 1, B_UNPACK_WARP = B_MMA_WARP + 3;
   constexpr int CPS = NCH / CS;                             // chunks per column set
   constexpr int BPS = 128 / LPB;                            // bins per super-tile
@@ -157,7 +158,10 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
         const int a_ = a;
         const uint32_t apar_ = apar;
         if (++a == NACC) { a = 0; apar ^= 1; }
-        if (TS > 1 && (g & (TS - 1)) != tset) continue;     // the other tile set's
+        // (by the parity of the accumulator slot = of the CTA's tile counter, NOT of g: a barrier must be seen in every
+        // phase by the set that waits on it -- a parity wait cannot tell phase n from n + 2 -- and with an odd number of
+        // tiles per super-tile g would hand a slot to the other set every other super-tile)
+        if (TS > 1 && (a_ & (TS - 1)) != tset) continue;    // the other tile set's
         const uint32_t bf_a = bt_full + 8 * a_;             // "full" of this accumulator pair; its "empty" is NACC barriers on
         mbar_wait_hinted(bf_a, apar_, B_WAIT_NS);
         tc_fence_after();

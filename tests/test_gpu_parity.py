@@ -200,6 +200,8 @@ I8_SHAPES = [
     (32, 7, 16, 16384, 16),    # the sweep's per-channel shape: 8 super-tiles x 7 channels on 56 CTAs
     (32, 2, 24, 33280, 4),     # 8320 bins = 65 super-tiles: CTA ranges straddle the channel boundary
     (32, 1, 13, 66560, 130),   # nint = 130 = 65 tiles per super-tile, 512 bins
+    (32, 4, 5, 3072, 6),       # <= 8 beams (two tile sets) with THREE tiles per super-tile: the sets alternate by tile counter
+    (32, 2, 8, 17920, 14),     # seven tiles per super-tile, 1280 bins
 ]
 
 
