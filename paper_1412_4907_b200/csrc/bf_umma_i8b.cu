@@ -5,9 +5,9 @@
 // to integrate ACROSS the lanes of a warp: a transposing butterfly of shuffles, selects and adds that costs as much
 // as the detection itself (profiles/r02_roles.md, sweep-B32: 2723 epilogue instructions per 256 samples, of which
 // FSEL + SHFL + FADD are 450 and the rest is six instructions per beam and sample).  Here the TMA engine does the
-// transposition on the way in: the voltages of one channel are viewed as a 4-D tensor
-//      { 128 bytes = two samples of 32 antennas,  nint / 2 rows per bin,  nbin,  nchan }
-// and a tile is the box {128, 1, 128, 1}: row g of 128 CONSECUTIVE BINS.  Row r of the A operand (= TMEM lane r)
+// transposition on the way in: the voltages are viewed as the tensor
+//      { 128 bytes = two samples of 32 antennas,  1,  nbin,  nint / 2 rows per bin,  nchan }
+// and a tile is the box {128, 1, 128, 1, 1}: row g of 128 CONSECUTIVE BINS.  Row r of the A operand (= TMEM lane r)
 // therefore belongs to bin 128 sp + r in every one of the G = nint / 2 tiles of a super-tile, and the integration
 // P[c][b][j] = sum_t |y|^2 is a plain running sum in the registers of the thread that owns the
 // lane: no shuffle, no select, and the stores of a warp are 32 consecutive bins of one beam (128 bytes).
@@ -17,13 +17,15 @@
 //                   five instructions per beam and sample
 //   a5 integration  in registers over the G tiles, (x + y) * scale^2, one coalesced fp32 store per beam
 // 4+4-bit input (row f1): the raw byte masked to its high nibble IS the int8 number 16 re, shifted
-// left by four it is 16 im -- three ALU instructions per four antennas turn a raw row of 128 bytes (four samples)
-// into two int8 operand rows, which the same MMAs and the same epilogue consume (scale / 16).
+// left by four and masked it is 16 im; two PRMT interleave them -- five ALU instructions per four antennas turn a raw
+// row of 128 bytes (four samples) into two int8 operand rows, which the same MMAs and the same epilogue consume
+// (scale / 16).  Up to 16 beams the operand rows are written to TENSOR MEMORY (tcgen05.st) and the MMAs take their A
+// operand from there; 17-32 beams keep shared-memory operand stages (no TMEM columns left).
 //
-// Warp roles (one persistent CTA per SM over a contiguous range of (channel, super-tile)): warps 0-7 epilogue in
-// two sets that split the 8-beam column chunks of EVERY tile between them (set 1 idles for <= 8 beams), warp 8 MMA
-// issue + TMEM allocation, warps 9-10 one TMA thread each (tiles of even / odd index), warps 11-14 (4-bit input
-// only) unpack.
+// Warp roles (one persistent CTA per SM over a contiguous range of (channel, super-tile)): 4 * NSETS epilogue warps
+// (sets of one warp per TMEM lane quadrant: column sets split the 8-beam chunks of a tile, tile sets take alternate
+// tiles -- see b_csets / b_tsets), then one MMA-issuing warp (+ TMEM allocation), two TMA producer warps (tiles of even
+// / odd index) and, for 4-bit input, four unpack warps.
 #include <cuda.h>
 
 #include "bf_internal.h"
@@ -59,10 +61,9 @@ BF_DEVI void tma_load_5d(uint32_t dst_smem, const void *tmap, int x, int y, int 
       ::"r"(dst_smem), "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(w), "r"(v), "r"(bar) : "memory");
 }
 
-// unpack groups (4-bit input): groups of four warps on alternate raw tiles (a tile's unpack is one chain of dependent
-// latencies -- barrier, LDS, barrier, STS, proxy fence, arrive -- that a group walks once per tile); one group only
-// next to four epilogue sets (registers)
-__host__ __device__ constexpr int b_ugroups(int ncol) { return 1; }   // measured: neither a second unpack group nor a second MMA-issuing warp changes the time (0.0638 / 0.0646 / 0.0667 ms)
+// unpack groups (4-bit input): groups of four warps on alternate raw tiles.  ONE: a second group (and likewise a second
+// MMA-issuing warp) was measured and changes nothing (sweep-ci4, 8 beams: 0.0638 / 0.0646 / 0.0667 ms)
+__host__ __device__ constexpr int b_ugroups(int ncol) { return 1; }
 template <int NCOL, int IN> constexpr int i8b_threads_v = (4 * b_nsets(NCOL) + 3 + (IN == BF_CI4 ? B_UNPACK_WARPS * b_ugroups(NCOL) : 0)) * 32;
 
 // NCOL: accumulator columns = 4 * beam capacity (32 / 64 / 128 -> 8 / 16 / 32 beams).  NST: operand stages (int8:
