@@ -162,6 +162,28 @@ int bf_set_antenna_gains(bf_ctx *ctx, const double *gains, int per_channel, void
 int bf_get_weights(bf_ctx *ctx, float *host_out, void *stream);
 
 /*
+ * bf_get_weights for callers that must not allocate device memory.  bf_get_weights cudaMalloc's (and cudaFree's) a
+ * buffer for the decoded weights; that is out of the question (a) while an observation runs -- cudaFree synchronises
+ * the whole device, so reading back the coefficients of a tracking update would stall every stream that
+ * is beamforming, (b) in a process whose device memory is owned by a pool (a framework's caching allocator, a backend
+ * that sizes everything at start-up), where a raw cudaMalloc fails or steals from the pool, and (c) on any thread while
+ * another thread captures a stream in the default global mode, where cudaMalloc is forbidden.  This variant decodes
+ * into a fixed array inside the library image instead and calls no cudaMalloc / cudaFree / allocating routine.
+ *   chan0, nchan_out  the channels wanted, [chan0, chan0 + nchan_out) inside [0, nchan)
+ *   host_out          HOST fp32 (re, im) pairs [nchan_out][nbeam][nant][2]; same values as bf_get_weights gives
+ *                     for those channels
+ * Limit: nchan_out * nbeam * nant * 8 bytes <= BF_NOALLOC_MAX_BYTES (8 MiB: one channel of 1024 beams x 1024
+ * antennas); more is refused with BF_ENOMEM and a message that says how many channels fit -- read a large weight set
+ * a few channels per call.  Cost: each GPU on which the process loads this library holds the 8 MiB until exit.
+ * The first call on a device looks up the array's device address (no allocation); make that call before any stream
+ * capture begins.  All contexts, streams and threads of a process share the one array per GPU: the call synchronises
+ * `stream` before it returns and holds a process-wide lock meanwhile, because two such read-backs overlapping on the
+ * GPU would overwrite each other's scratch.  Other errors as bf_get_weights (BF_EINVAL, BF_ENOGEOM, BF_ECUDA).
+ */
+#define BF_NOALLOC_MAX_BYTES (8u << 20)
+int bf_get_weights_noalloc(bf_ctx *ctx, int chan0, int nchan_out, float *host_out, void *stream);
+
+/*
  * The hot path.  voltages: DEVICE, [nchan][nsamp][nant][2] (re, im interleaved) of the context's
  * dtype ([nchan][nsamp][nant] bytes for BF_CI4), 16-byte aligned.  powers: DEVICE fp32 [nchan][nbeam][nsamp/nint], fully overwritten.
  * Enqueues on `stream` and returns.  BF_ENOGEOM before bf_set_geometry.

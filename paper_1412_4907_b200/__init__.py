@@ -36,6 +36,7 @@ SYMBOLS = {
     "bf_set_geometry": (_i, [_vp, _dp, _dp, _dp, _vp]),
     "bf_set_antenna_gains": (_i, [_vp, _dp, _i, _vp]),
     "bf_get_weights": (_i, [_vp, _vp, _vp]),
+    "bf_get_weights_noalloc": (_i, [_vp, _i, _i, _vp, _vp]),
     "bf_run": (_i, [_vp, _vp, _vp, _vp]),
     "bf_run_beams": (_i, [_vp, _vp, _vp, ctypes.c_float, _vp]),
     "bf_run_incoherent": (_i, [_vp, _vp, _vp, _vp]),
@@ -171,6 +172,16 @@ def bf_get_weights(ctx, host_out, stream=None):
     return lib().bf_get_weights(ctx, _ptr(host_out), _stream(stream))
 
 
+BF_NOALLOC_MAX_BYTES = 8 << 20  # include/bf.h
+
+
+def bf_get_weights_noalloc(ctx, chan0, nchan_out, host_out, stream=None):
+    """bf_get_weights without cudaMalloc / cudaFree (for callers that must not allocate on the device: a running
+    observation, a process whose memory belongs to a pool, a thread beside a global-mode stream capture).  At most
+    BF_NOALLOC_MAX_BYTES of weights per call -- see include/bf.h."""
+    return lib().bf_get_weights_noalloc(ctx, int(chan0), int(nchan_out), _ptr(host_out), _stream(stream))
+
+
 def bf_run(ctx, voltages, powers, stream=None):
     return lib().bf_run(ctx, _ptr(voltages), _ptr(powers), _stream(stream))
 
@@ -260,6 +271,18 @@ class Beamformer:
         nant, nchan, nbeam = self.shape[:3]
         out = np.empty((nchan, nbeam, nant, 2), dtype=np.float32)
         self._check(bf_get_weights(self.ctx, out))
+        return out[..., 0] + 1j * out[..., 1]
+
+    def weights_noalloc(self):
+        """weights() through bf_get_weights_noalloc: no device allocation, as many channels per call as fit."""
+        import numpy as np
+
+        nant, nchan, nbeam = self.shape[:3]
+        out = np.empty((nchan, nbeam, nant, 2), dtype=np.float32)
+        step = max(1, BF_NOALLOC_MAX_BYTES // (nbeam * nant * 8))
+        for c0 in range(0, nchan, step):
+            n = min(step, nchan - c0)
+            self._check(bf_get_weights_noalloc(self.ctx, c0, n, out[c0:c0 + n]))
         return out[..., 0] + 1j * out[..., 1]
 
     def empty_powers(self):

@@ -403,6 +403,21 @@ extern "C" int bf_get_weights(bf_ctx *c, float *host_out, void *stream) {
   return BF_OK;
 }
 
+// For bf_weights_noalloc.cu (bf_get_weights_noalloc): the preparation bf_get_weights does before it decodes -- adopt a
+// pending tracking update behind its event on `st`, and say which operand bf_run reads (the int8 two-limb one or the
+// fp16 one).  The caller has already checked c and have_geom.
+int bf_prepare_weight_readback(bf_ctx *c, cudaStream_t st, bool *int8_operand) {
+  if (c->pending >= 0) {
+    int rc = wait_event(c, st, c->ev_upd);
+    if (rc != BF_OK) return rc;
+    c->active = c->pending; c->pending = -1;
+    select_buffer(c, c->active);
+  }
+  const char *why;
+  *int8_operand = pick_kernel(c, BF_MODE_POWER, &why) == BF_KERNEL_UMMA_I8 && c->d_wop8 != nullptr;
+  return BF_OK;
+}
+
 // launch the selected kernel over channels [chan0, chan0 + nchan_run); mode BF_MODE_POWER writes `out` as
 // fp32 powers, BF_MODE_BEAMS as fp16 (re, im) voltage beams scaled by `scale`
 static int launch_range(bf_ctx *c, const void *volt, void *out, int chan0, int nchan_run, cudaStream_t st,

@@ -107,6 +107,7 @@ size_t bf_wop_bytes_per_chan(const bf_ctx *c);
 // kernels (each returns a cudaError_t from the launch)
 cudaError_t bf_launch_weights(const bf_ctx *c, cudaStream_t st);
 cudaError_t bf_launch_decode_weights(const bf_ctx *c, float *d_out, bool int8_operand, cudaStream_t st);
+int bf_prepare_weight_readback(bf_ctx *c, cudaStream_t st, bool *int8_operand);   // bf_api.cu, for bf_weights_noalloc.cu
 cudaError_t bf_launch_simt(const BfParams &p, int dtype, cudaStream_t st);
 bool bf_umma_supported(const bf_ctx *c, const char **why);
 bool bf_umma_shape_supported(const bf_ctx *c, const char **why);  // ignoring nint (voltage-beam mode)
