@@ -58,7 +58,8 @@ enum bf_kernel {
   BF_KERNEL_AUTO = 0, /* pick the fastest kernel that supports the shape.  NOTE: for shapes no tensor-core kernel takes (nant
                          not a multiple of 8 (int8) / 4 (fp16) / 16 (4+4-bit), nint neither 2^k <= 64 nor a multiple of 64 / 32 -- except on
                          32 antennas with <= 32 beams, where any EVEN nint integrates on tensor cores when nsamp / nint is a
-                         multiple of 128 or >= 512)
+                         multiple of 128 or >= 512, and with 33-64 beams, where any even nint >= 16 does when nsamp / nint is a
+                         multiple of 256 or >= 1024)
                          AUTO falls through to BF_KERNEL_SIMT without an error -- about 30x slower on the `tiny` shape;
                          bf_kernel_name / bf_selected_kernel say which family will run, and BF_KERNEL_UMMA turns the
                          fall-through into BF_EUNSUPPORTED */

@@ -164,9 +164,7 @@ extern "C" const char *bf_kernel_name(const bf_ctx *c) {
     case BF_KERNEL_UMMA_I8: return "umma-i8";
     case BF_KERNEL_UMMA_F16: {
       if (!(2 * c->nant <= 64 && c->dtype != BF_CF16)) return "umma-f16-kblock";
-      // 33-64 beams on 32 antennas with >= 256-bin channels: bf_umma_bl.cu (the same test as bf_umma_bl_takes)
-      const bool binlane = c->nant == 32 && c->nbeam > 32 && c->nMt == 1 && c->nint >= BF_LO_NINT && c->nint % 2 == 0 &&
-                           (c->nbin % 256 == 0 || c->nbin >= 1024);
+      const bool binlane = bf_bl_shape(c->dtype, BF_MODE_POWER, c->nant, c->nbeam, c->nint, c->nbin);   // bf_umma_bl.cu
       return binlane ? "umma-f16-binlane" : "umma-f16-resident";
     }
     default: return "unsupported";

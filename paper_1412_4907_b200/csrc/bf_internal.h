@@ -66,6 +66,17 @@ struct BfParams {
 #define BF_I8_QSCALE 16256.0
 __host__ __device__ inline int bf_i8_ncol(int nbeam) { return nbeam <= 8 ? 32 : nbeam <= 16 ? 64 : 128; }
 
+// ---- shapes of the bin-per-lane fp16 kernel (bf_umma_bl.cu) -------------------------------------
+// THE predicate: bf_umma_supported (does the fp16 family integrate this nint?), bf_launch_umma (which kernel) and
+// bf_kernel_name (what to report) all call it.  Complex int8 or 4+4-bit input, 32 antennas, 33-64 beams (one coefficient
+// tile), power mode, single-term coefficients (nint >= BF_LO_NINT), any EVEN nint (the running sum of a bin lives in the
+// registers of the thread that owns its TMEM lane), and enough bins that the 256 lanes of an item are not mostly padding.
+inline bool bf_bl_shape(int dtype, int mode, int nant, int nbeam, int nint, int nbin) {
+  if ((dtype != BF_CI8 && dtype != BF_CI4) || mode != BF_MODE_POWER || nant != 32 || nbeam <= 32 || nbeam > BF_TILE_BEAMS) return false;
+  if (nint < BF_LO_NINT || nint % 2 != 0 || (long long)nint * 64 >= (1ll << 32)) return false;
+  return nbin % 256 == 0 || nbin >= 1024;
+}
+
 struct bf_ctx {
   int nant, nchan, nbeam, nsamp, nint, nbin;
   int dtype, kernel_forced;

@@ -525,7 +525,12 @@ bool bf_umma_shape_supported(const bf_ctx *c, const char **why) {
 
 bool bf_umma_supported(const bf_ctx *c, const char **why) {
   if (!bf_umma_shape_supported(c, why)) return false;
-  if (!nint_ok(c->nint)) { *why = "needs nint a power of two <= 64 or a multiple of 64"; return false; }
+  // 33-64 beams on 32 antennas: the bin-per-lane kernel integrates any even nint >= 16 (bf_bl_shape)
+  if (!nint_ok(c->nint) && !bf_bl_shape(c->dtype, BF_MODE_POWER, c->nant, c->nbeam, c->nint, c->nbin)) {
+    *why = "needs nint a power of two <= 64 or a multiple of 64 (33-64 beams on 32 antennas: any even nint >= 16 with nsamp / nint "
+           "a multiple of 256 or >= 1024)";
+    return false;
+  }
   return true;
 }
 
@@ -548,7 +553,9 @@ static cudaError_t launch_k64_in(const BfParams &p, int sm_count, cudaStream_t s
     case 16: return launch_k64_nint<16, IN>(p, sm_count, st);
     case 32: return launch_k64_nint<32, IN>(p, sm_count, st);
     case 64: return launch_k64_nint<64, IN>(p, sm_count, st);
-    default: return launch_k64_nint<0, IN>(p, sm_count, st);  // multiples of 64: atomic partial sums
+    default:
+      if (p.nint % 64 != 0) return cudaErrorNotSupported;   // bf_umma_supported lets no such shape through
+      return launch_k64_nint<0, IN>(p, sm_count, st);       // multiples of 64: atomic partial sums
   }
 }
 
@@ -558,6 +565,6 @@ cudaError_t bf_launch_umma(const BfParams &p, int dtype, int sm_count, cudaStrea
   if (v != 1) return cudaErrorNotSupported;
   // 33-64 beams on 32 antennas, bins of an even number >= 16 of samples: the bin-per-lane kernel with the voltages in
   // tensor memory (bf_umma_bl.cu; sweep at 64 / 48 / 40 beams 0.168 / 0.151 / 0.146 -> 0.145 / 0.137 / 0.132 ms)
-  if (p.nbeam > 32 && bf_umma_bl_takes(p, dtype)) return bf_launch_umma_bl(p, dtype, sm_count, st);
+  if (bf_umma_bl_takes(p, dtype)) return bf_launch_umma_bl(p, dtype, sm_count, st);
   return dtype == BF_CI4 ? launch_k64_in<BF_CI4>(p, sm_count, st) : launch_k64_in<BF_CI8>(p, sm_count, st);
 }

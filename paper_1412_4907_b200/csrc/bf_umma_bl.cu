@@ -343,13 +343,10 @@ cudaError_t launch_bl(const BfParams &p, int sm_count, cudaStream_t st) {
 
 }  // namespace
 
-// Shapes this kernel takes: complex int8 or 4+4-bit input, 32 antennas, up to 64 beams (one coefficient tile), power mode,
-// single-term coefficients (nint >= BF_LO_NINT), even nint, and enough bins that the 256 lanes of an item are not mostly
-// padding
+// Shapes this kernel takes: bf_bl_shape (bf_internal.h) -- the one predicate the dispatcher, bf_kernel_name and
+// bf_umma_supported share -- on a launch without the residual coefficient plane
 bool bf_umma_bl_takes(const BfParams &p, int dtype) {
-  if ((dtype != BF_CI8 && dtype != BF_CI4) || p.mode != BF_MODE_POWER || p.nant != 32 || p.nMt != 1 || p.wop_lo != nullptr) return false;
-  if (p.nint < BF_LO_NINT || p.nint % 2 != 0 || (long long)p.nint * 64 >= (1ll << 32)) return false;
-  return p.nbin % 256 == 0 || p.nbin >= 1024;
+  return p.wop_lo == nullptr && bf_bl_shape(dtype, p.mode, p.nant, p.nbeam, p.nint, p.nbin);
 }
 
 cudaError_t bf_launch_umma_bl(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {

@@ -98,57 +98,63 @@ def test_tiny_full(bf, kernel):
 
 
 SMALL = [
-    # nant nchan nbeam nsamp nint dtype
-    (32, 3, 1, 256, 16, "ci8"),
-    (32, 2, 3, 1000, 8, "ci8"),      # ragged time tail (1000 = 3*256 + 232)
-    (32, 2, 17, 272, 1, "ci8"),      # nint = 1
-    (32, 2, 64, 512, 64, "ci8"),
-    (32, 2, 65, 768, 256, "ci8"),    # beams spill into a second M tile
-    (32, 1, 130, 1024, 1024, "ci8"),  # nint = nsamp, three M tiles
-    (32, 2, 16, 2048, 512, "ci8"),   # nint spans two time tiles
-    (32, 1, 5, 96, 48, "ci8"),       # nint not a power of two
-    (8, 2, 4, 128, 16, "ci8"),
-    (16, 2, 9, 300, 4, "ci8"),
-    (64, 2, 33, 512, 32, "ci8"),
-    (5, 2, 3, 77, 7, "ci8"),         # odd everything: generic kernel only
-    (32, 2, 16, 256, 16, "cf16"),
-    (256, 1, 70, 512, 32, "cf16"),   # K-blocked kernel, 2 M-tiles, second one ragged
-    (12, 2, 6, 200, 8, "cf16"),      # K' = 24 < one K-block (TMA zero-fills the rest)
-    (40, 2, 20, 520, 8, "ci8"),      # K' = 80: second K-block only a quarter full
-    (64, 1, 130, 768, 64, "ci8"),    # three M-tiles: the last beam group has a single tile
-    (128, 1, 9, 512, 128, "ci8"),    # nint > 64: atomic partial sums, K-blocked
-    (96, 2, 64, 300, 4, "cf16"),     # ragged time tail, K' = 192
-    (1024, 1, 16, 256, 64, "ci8"),   # the streaming config's antenna count
-    (32, 2, 16, 1000, 8, "ci4"),     # the paper's 4+4-bit format, BEST-2's 32 antennas, ragged tail
-    (32, 1, 130, 512, 64, "ci4"),
-    (16, 2, 5, 256, 1, "ci4"),       # K' = 32: half a K-block
-    (24, 2, 7, 128, 16, "ci4"),      # rows of 24 bytes: generic kernel only
-    (64, 3, 256, 992, 32, "ci8"),    # K-blocked, two beam groups: CTA pairs with multicast voltages (int8: raw stages), ragged tail
-    (128, 2, 200, 528, 16, "cf16"),  # the same for fp16 input (operand stages are the multicast target), last M-tile partial
-    (72, 5, 300, 704, 64, "cf16"),   # three beam groups... odd: no pairs; 5 channels
-    (64, 7, 512, 512, 64, "ci8"),    # four beam groups, 7 x 2 x 4 = 56 items on 56 CTAs
-    (1024, 1, 16, 256, 64, "ci4"),   # 4-bit input on the K-blocked kernel: the streaming array's antenna count
-    (48, 2, 70, 608, 16, "ci4"),     # K-blocked, second K-block half full (TMA zero-fills), two M-tiles, ragged tail
-    (64, 2, 9, 512, 4, "ci4"),       # K-blocked with two-term coefficients
-    (32, 40, 64, 5000, 8, "ci8"),    # 800 items: 5-6 per CTA, both convert groups busy, ragged tail (5000 = 19*256 + 136)
-    (32, 30, 100, 3000, 4, "ci4"),   # same for the 4-bit unpack, two M-tiles per item
+    # nant nchan nbeam nsamp nint dtype, and the kernel BF_KERNEL_AUTO must pick (asserted: a shape that silently runs another
+    # kernel than its comment says tests nothing)
+    (32, 3, 1, 256, 16, "ci8", "i8"),
+    (32, 2, 3, 1000, 8, "ci8", "i8"),      # ragged time tail (1000 = 3*256 + 232)
+    (32, 2, 17, 272, 1, "ci8", "i8"),      # nint = 1
+    (32, 2, 64, 512, 64, "ci8", "resident"),
+    (32, 2, 65, 768, 256, "ci8", "resident"),    # beams spill into a second M tile
+    (32, 1, 130, 1024, 1024, "ci8", "resident"),  # nint = nsamp, three M tiles
+    (32, 2, 16, 2048, 512, "ci8", "i8"),   # nint spans two time tiles
+    (32, 1, 5, 96, 48, "ci8", "simt"),       # nint not a power of two
+    (8, 2, 4, 128, 16, "ci8", "i8"),
+    (16, 2, 9, 300, 4, "ci8", "i8"),
+    (64, 2, 33, 512, 32, "ci8", "kblock"),
+    (5, 2, 3, 77, 7, "ci8", "simt"),         # odd everything: generic kernel only
+    (32, 2, 16, 256, 16, "cf16", "kblock"),
+    (256, 1, 70, 512, 32, "cf16", "kblock"),   # K-blocked kernel, 2 M-tiles, second one ragged
+    (12, 2, 6, 200, 8, "cf16", "kblock"),      # K' = 24 < one K-block (TMA zero-fills the rest)
+    (40, 2, 20, 520, 8, "ci8", "kblock"),      # K' = 80: second K-block only a quarter full
+    (64, 1, 130, 768, 64, "ci8", "kblock"),    # three M-tiles: the last beam group has a single tile
+    (128, 1, 9, 512, 128, "ci8", "kblock"),    # nint > 64: atomic partial sums, K-blocked
+    (96, 2, 64, 300, 4, "cf16", "kblock"),     # ragged time tail, K' = 192
+    (1024, 1, 16, 256, 64, "ci8", "kblock"),   # the streaming config's antenna count
+    (32, 2, 16, 1000, 8, "ci4", "resident"),     # the paper's 4+4-bit format, BEST-2's 32 antennas, ragged tail
+    (32, 1, 130, 512, 64, "ci4", "resident"),
+    (16, 2, 5, 256, 1, "ci4", "resident"),       # K' = 32: half a K-block
+    (24, 2, 7, 128, 16, "ci4", "simt"),      # rows of 24 bytes: generic kernel only
+    (64, 3, 256, 992, 32, "ci8", "kblock"),    # K-blocked, two beam groups: CTA pairs with multicast voltages (int8: raw stages), ragged tail
+    (128, 2, 200, 528, 16, "cf16", "kblock"),  # the same for fp16 input (operand stages are the multicast target), last M-tile partial
+    (72, 5, 300, 704, 64, "cf16", "kblock"),   # three beam groups... odd: no pairs; 5 channels
+    (64, 7, 512, 512, 64, "ci8", "kblock"),    # four beam groups, 7 x 2 x 4 = 56 items on 56 CTAs
+    (1024, 1, 16, 256, 64, "ci4", "kblock"),   # 4-bit input on the K-blocked kernel: the streaming array's antenna count
+    (48, 2, 70, 608, 16, "ci4", "kblock"),     # K-blocked, second K-block half full (TMA zero-fills), two M-tiles, ragged tail
+    (64, 2, 9, 512, 4, "ci4", "kblock"),       # K-blocked with two-term coefficients
+    (32, 40, 64, 5000, 8, "ci8", "resident"),    # 800 items: 5-6 per CTA, both convert groups busy, ragged tail (5000 = 19*256 + 136)
+    (32, 30, 100, 3000, 4, "ci4", "resident"),   # same for the 4-bit unpack, two M-tiles per item
     # 33-64 beams with >= 256-bin channels: the bin-per-lane kernel with the voltages in tensor memory (bf_umma_bl.cu)
-    (32, 2, 64, 8192, 16, "ci8"),    # 512 bins: two super-tile pairs per channel, eight raw-tile pairs per item
-    (32, 3, 33, 4096, 16, "ci8"),    # 256 bins: one pair per channel, the second 16-beam chunk holds a single beam
-    (32, 1, 50, 34816, 32, "ci8"),   # 1088 bins = 4 pairs + 64 bins: the last pair is half a super-tile X and an empty Y
-    (32, 5, 64, 9216, 18, "ci8"),    # nint = 18: any even bin length >= 16; 512 bins, CTA ranges straddle channels
-    (32, 2, 40, 65536, 256, "ci8"),  # long bins: 128 raw-tile pairs per item
-    (32, 2, 64, 8192, 16, "ci4"),    # the same kernel on 4+4-bit input: raw rows of 64 bytes, 64-byte swizzle
-    (32, 1, 50, 34816, 32, "ci4"),   # partial last pair
-    (32, 3, 33, 5120, 20, "ci4"),    # nint = 20, 256 bins
+    (32, 2, 64, 8192, 16, "ci8", "binlane"),    # 512 bins: two super-tile pairs per channel, eight raw-tile pairs per item
+    (32, 3, 33, 4096, 16, "ci8", "binlane"),    # 256 bins: one pair per channel, the second 16-beam chunk holds a single beam
+    (32, 1, 50, 34816, 32, "ci8", "binlane"),   # 1088 bins = 4 pairs + 64 bins: the last pair is half a super-tile X and an empty Y
+    (32, 5, 64, 9216, 18, "ci8", "binlane"),    # nint = 18: any even bin length >= 16; 512 bins, CTA ranges straddle channels
+    (32, 2, 40, 65536, 256, "ci8", "binlane"),  # long bins: 128 raw-tile pairs per item
+    (32, 2, 64, 8192, 16, "ci4", "binlane"),    # the same kernel on 4+4-bit input: raw rows of 64 bytes, 64-byte swizzle
+    (32, 1, 50, 34816, 32, "ci4", "binlane"),   # partial last pair
+    (32, 3, 33, 5120, 20, "ci4", "binlane"),    # nint = 20, 256 bins
+    (32, 2, 48, 11264, 22, "ci8", "binlane"),   # nint = 22: an ODD number (11) of raw rows per bin, 512 bins
+    (32, 1, 64, 34816, 34, "ci4", "binlane"),   # nint = 34 (17 rows per bin), 1024 bins
 ]
+
+KERNEL_NAMES = {"i8": "umma-i8", "resident": "umma-f16-resident", "kblock": "umma-f16-kblock", "binlane": "umma-f16-binlane",
+                "simt": "simt"}
 
 
 @pytest.mark.parametrize("kernel", ["simt", "auto", "f16"])
-@pytest.mark.parametrize("shape", SMALL, ids=lambda s: "N%d-C%d-B%d-T%d-I%d-%s" % s)
+@pytest.mark.parametrize("shape", SMALL, ids=lambda s: "N%d-C%d-B%d-T%d-I%d-%s" % s[:6])
 def test_small_shapes(bf, shape, kernel):
-    N, C, B, T, I, dtype = shape
-    rng = np.random.default_rng(abs(hash(shape)) % (2 ** 31))
+    N, C, B, T, I, dtype, auto_kernel = shape
+    rng = np.random.default_rng([N, C, B, T, I, len(dtype)])
     r = rng.uniform(-40, 40, size=(N, 3)); r[:, 2] *= 0.05
     f = np.linspace(380e6, 420e6, C) if C > 1 else np.array([408e6])
     s = rng.normal(size=(B, 3)); s[:, 2] = np.abs(s[:, 2]) + 1.5; s /= np.linalg.norm(s, axis=1, keepdims=True)
@@ -157,12 +163,20 @@ def test_small_shapes(bf, shape, kernel):
     v = w.make_voltages()
     ref = oracle.beamform(r, f, s, v, I)
     k = {"simt": bf.BF_KERNEL_SIMT, "auto": bf.BF_KERNEL_AUTO, "f16": bf.BF_KERNEL_UMMA_F16}[kernel]
-    if kernel == "f16":
-        B_ = bf.Beamformer(N, C, B, T, I, dtype=bf_dtype(bf, w), kernel=k)
-        name = B_.kernel_name
-        B_.close()
+    B_ = bf.Beamformer(N, C, B, T, I, dtype=bf_dtype(bf, w), kernel=k)
+    name = B_.kernel_name
+    B_.close()
+    if kernel == "auto":
+        assert name == KERNEL_NAMES[auto_kernel], f"AUTO picks {name}, the table says {auto_kernel}"
+    elif kernel == "f16":
         if name == "unsupported":
+            assert auto_kernel in ("simt", "i8"), f"an fp16-family shape ({auto_kernel}) refused when forced"
             pytest.skip("no fp16 tensor-core variant for this shape")
+        assert name.startswith("umma-f16-")
+        if auto_kernel not in ("simt", "i8"):
+            assert name == KERNEL_NAMES[auto_kernel]
+    else:
+        assert name == "simt"
     out, used = run_gpu(bf, w, v, k)
     check_rows(out, ref, TOL)   # the plain bar at every nint (two-term coefficients below nint 16)
 
