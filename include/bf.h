@@ -221,7 +221,8 @@ int bf_run_incoherent(bf_ctx *ctx, const void *voltages, float *powers, void *st
  *   host_voltages  HOST (pinned for overlap; pageable works but serialises), same layout as bf_run
  *   host_powers    HOST fp32 [nchan][nbeam][nsamp/nint]
  *   staging        DEVICE scratch of >= bf_staging_bytes(ctx, chan_per_chunk) bytes, 1024-byte aligned
- * Returns after enqueuing; synchronise both streams before reading host_powers.
+ * Returns after enqueuing; synchronise both streams before reading host_powers.  If the call fails part-way (BF_ECUDA),
+ * it first waits for the read-backs it had already queued, so host_powers and staging are not touched after it returns.
  */
 size_t bf_staging_bytes(const bf_ctx *ctx, int chan_per_chunk);
 int bf_run_host(bf_ctx *ctx, const void *host_voltages, float *host_powers, void *staging,
@@ -242,7 +243,8 @@ int bf_run_streaming(bf_ctx *ctx, const void *const *host_blocks, int nblocks, f
  *   { clock64 at start, globaltimer (ns) at start, clock64 at end, globaltimer (ns) at end }
  * so the caller can compute the SM clock the kernel really ran at, (c1 - c0) / (t1 - t0) GHz -- nvidia-smi's
  * sampled clock is too coarse for a millisecond kernel.  NULL switches it off (the default).  Two scalar
- * stores per launch; no effect on the result.
+ * stores per launch; no effect on the result.  The four words must stay allocated until the probe is switched off (NULL)
+ * or the context is destroyed and every launch made meanwhile has finished: the library keeps only the address.
  */
 int bf_set_clock_probe(bf_ctx *ctx, void *dev_u64x4);
 

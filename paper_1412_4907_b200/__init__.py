@@ -246,6 +246,7 @@ class Beamformer:
         off = (-self.workspace.data_ptr()) % 1024
         self._check(bf_set_workspace(self.ctx, self.workspace.data_ptr() + off, nbytes))
         self._staging = None
+        self._probe = None   # the tensor bf_set_clock_probe points at, kept alive while the library may write to it
 
     def _check(self, rc):
         if rc != BF_OK:
@@ -347,8 +348,17 @@ class Beamformer:
         self._check(bf_run_streaming(self.ctx, host_blocks, powers, st, nbytes, compute_stream, copy_stream))
 
     def set_clock_probe(self, dev_u64x4):
-        """dev_u64x4: torch int64 tensor of 4 elements on the device (or None): see bf_set_clock_probe."""
+        """dev_u64x4: torch int64 tensor of 4 elements on the device (or None): see bf_set_clock_probe.  The library keeps
+        only the address and every later launch writes there, so this object holds on to the tensor until the probe is
+        switched off or the context is closed."""
+        if dev_u64x4 is not None:
+            import torch
+
+            if not (isinstance(dev_u64x4, torch.Tensor) and dev_u64x4.is_cuda and dev_u64x4.dtype == torch.int64
+                    and dev_u64x4.numel() >= 4 and dev_u64x4.is_contiguous()):
+                raise BfError(BF_EINVAL, "clock probe must be a contiguous int64 CUDA tensor of at least 4 elements")
         self._check(bf_set_clock_probe(self.ctx, dev_u64x4))
+        self._probe = dev_u64x4
 
     @property
     def selected_kernel(self):
@@ -366,6 +376,7 @@ class Beamformer:
         if self.ctx:
             bf_destroy(self.ctx)
             self.ctx = None
+        self._probe = None
 
     def __del__(self):
         try:

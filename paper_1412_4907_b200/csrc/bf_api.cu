@@ -577,6 +577,10 @@ extern "C" int bf_run_host(bf_ctx *c, const void *host_volt, float *host_pow, vo
     if ((rc = wait_event(c, cs, c->ev_done[b])) != BF_OK) break;
     rc = wait_event(c, xs, c->ev_done[b]);
   }
+  // A failure part-way leaves read-backs of earlier chunks queued on the library's own stream: they still write host_pow
+  // and read staging, and nothing the caller can synchronise covers them (its streams were not made to wait above).  Do not
+  // hand the error back while that DMA is in flight -- the caller may free or reuse both buffers straight away.
+  if (rc != BF_OK) (void)cudaStreamSynchronize(ds);
   return finish_run(c, cs, rc);
 }
 
