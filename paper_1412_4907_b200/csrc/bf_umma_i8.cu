@@ -612,6 +612,10 @@ cudaError_t launch_i8_nint(const BfParams &p, int sm_count, cudaStream_t st) {
 
 }  // namespace
 
+// bins the time-on-M kernels of this file integrate (lane butterfly / one bin per warp / running sums over whole tiles);
+// any other even nint needs the bin-per-lane variant (bf_umma_i8b.cu)
+static bool i8_tiled_nint_ok(int I) { return (I <= 32 && (I & (I - 1)) == 0) || I % 32 == 0; }
+
 // which shapes the int8 kernel takes: complex int8, nant a multiple of 8 up to 32 (rows of <= 64 bytes that
 // TMA can address), up to BF_I8_MAX_BEAMS beams, nint a power of two <= 32 or a multiple of 32
 bool bf_umma_i8_supported(const bf_ctx *c, int mode) {
@@ -623,10 +627,8 @@ bool bf_umma_i8_supported(const bf_ctx *c, int mode) {
   const int I = c->nint;
   // the bin-per-lane variant (bf_umma_i8b.cu) integrates ANY even nint in registers
   if (c->nant == 32 && I % 2 == 0 && (c->nbin % 128 == 0 || c->nbin >= 512)) return true;
-  return (I <= 32 && (I & (I - 1)) == 0) || I % 32 == 0;
+  return i8_tiled_nint_ok(I);
 }
-
-static bool old_nint_ok(int I) { return (I <= 32 && (I & (I - 1)) == 0) || I % 32 == 0; }
 
 cudaError_t bf_launch_umma_i8(const BfParams &p, int dtype, int sm_count, cudaStream_t st) {
   if (dtype == BF_CI4) return bf_umma_i8b_takes(p, dtype) ? bf_launch_umma_i8b(p, dtype, sm_count, st) : cudaErrorNotSupported;
@@ -638,7 +640,7 @@ cudaError_t bf_launch_umma_i8(const BfParams &p, int dtype, int sm_count, cudaSt
   // 32 antennas, even nint and enough bins to fill the lanes: the bin-per-lane kernel (no cross-lane integration)
   // (measured on the sweep: 17-32 beams 0.147 -> 0.114 ms; up to 16 beams the contiguous tiles of the kernels
   // below read DRAM 7 % faster than the strided ones and their butterfly is still cheap)
-  if (bf_umma_i8b_takes(p, BF_CI8) && (p.nbeam > 16 || !old_nint_ok(p.nint)))
+  if (bf_umma_i8b_takes(p, BF_CI8) && (p.nbeam > 16 || !i8_tiled_nint_ok(p.nint)))
     return bf_launch_umma_i8b(p, BF_CI8, sm_count, st);
   // 32 antennas, an even number of samples and nint 2^k <= 64 or a multiple of 64: rows of two samples
   const bool wide = p.nant == 32 && p.nsamp % 2 == 0 && ((p.nint <= 64 && (p.nint & (p.nint - 1)) == 0) || p.nint % 64 == 0);

@@ -37,9 +37,6 @@ namespace {
 constexpr int B_ROW_BYTES = 128;                       // one operand row: two samples x 32 antennas x (re, im)
 constexpr int B_STAGE_BYTES = 128 * B_ROW_BYTES;       // 16 KiB: 128 bins x two samples
 constexpr int B_W_ROW_BYTES = 64;                      // coefficient rows (bf_internal.h: int8 two-limb operand)
-#ifndef B_SETS_MAX
-#define B_SETS_MAX 4
-#endif
 #ifndef B_WAIT_NS
 #define B_WAIT_NS 400
 #endif
@@ -68,7 +65,7 @@ template <int NCOL, int IN> constexpr int i8b_threads_v = (4 * b_nsets(NCOL) + 3
 
 // NCOL: accumulator columns = 4 * beam capacity (32 / 64 / 128 -> 8 / 16 / 32 beams).  NST: operand stages (int8:
 // filled by TMA; 4-bit: filled by the unpack warps from NRAW raw stages).
-template <int NCOL, int NST, int NRAW, int IN, int LPB>
+template <int NCOL, int NST, int NRAW, int IN>
 __global__ void __launch_bounds__(i8b_threads_v<NCOL, IN>, 1)
 bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, const long long total_super,
                    const int n_super_chan, const int G) {
@@ -87,7 +84,7 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
   static_assert(TS == 1 || NACC % TS == 0, "an accumulator slot must always belong to the same tile set");
   constexpr int B_MMA_WARP = 4 * NSETS, B_TMA_WARP = B_MMA_WARP + 1, B_UNPACK_WARP = B_MMA_WARP + 3;
   constexpr int CPS = NCH / CS;                             // chunks per column set
-  constexpr int BPS = 128 / LPB;                            // bins per super-tile
+  constexpr int BPS = 128;                                  // bins per super-tile: one per TMEM lane
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sW = smem_base;                            // 2 coefficient buffers
   const uint32_t sA = sW + 2 * W_BYTES;                     // NST operand stages (W_BYTES is a multiple of 1024)
@@ -145,8 +142,8 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
     int a = 0;                                              // accumulator pair of the next operand tile, parity of its "full"
     uint32_t apar = 0;
     for (int s = 0; s < n_super; ++s) {
-      const int bin = BPS * sp + (32 * quad + lane) / LPB;
-      const bool live = BPS * sp + 32 * quad / LPB < nbin;  // warp-uniform: this quadrant holds real bins
+      const int bin = BPS * sp + 32 * quad + lane;
+      const bool live = BPS * sp + 32 * quad < nbin;  // warp-uniform: this quadrant holds real bins
       // requested now, used after the G tiles: a load at the END of the super-tile would stall every warp for a
       // DRAM round trip per super-tile
       const float sc = (float)p.i8scale[c] * (CI4 ? 0.0625f : 1.0f);         // 4-bit operands carry 16 x
@@ -221,14 +218,12 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
       if (live && tset == 0) {
         const float sc2 = sc * sc;
         float *out = p.pow + (size_t)c * nbeam * nbin + bin;
-        const bool writer = (lane & (LPB - 1)) == 0 && bin < nbin;
+        const bool writer = bin < nbin;
 #pragma unroll
         for (int k = 0; k < CPS; ++k)
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
-            float tot = acc[k][i].x + acc[k][i].y;
-#pragma unroll
-            for (int o = LPB / 2; o >= 1; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);   // the LPB lanes of a bin
+            const float tot = acc[k][i].x + acc[k][i].y;
             const int beam = 8 * (set * CPS + k) + i;
             if (writer && beam < nbeam) out[(size_t)beam * nbin] = tot * sc2;
           }
@@ -311,7 +306,7 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
         if (lane == 0) {
           mbar_wait(empty + 8 * st, st_par);
           mbar_arrive_expect_tx(full + 8 * st, B_STAGE_BYTES);
-          tma_load_5d(ring + st * B_STAGE_BYTES, &tmap, 0, 0, BPS * sp, g, c, full + 8 * st);   // rows LPB g .. of bins BPS sp ..
+          tma_load_5d(ring + st * B_STAGE_BYTES, &tmap, 0, 0, BPS * sp, g, c, full + 8 * st);   // row g of bins BPS sp ..
         }
         __syncwarp();
         if ((st += 2) >= NRING) { st -= NRING; st_par ^= 1; }
@@ -439,16 +434,16 @@ bf_umma_i8b_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, c
 
 // 4-D view of one launch's voltages: {128 bytes, rows per bin, nbin, nchan}; box {128, 1, 128, 1}, 128-byte swizzle.
 // A row is two int8 samples (rows per bin = nint / 2) or four 4-bit samples (nint / 4); bins past nbin are zero-filled.
-template <int IN, int LPB>
+template <int IN>
 cudaError_t make_tmap_bins(CUtensorMap *tm, const BfParams &p, int nint) {
   PFN_encodeTiled enc = bf_get_encode();
   if (!enc) return cudaErrorNotSupported;
   const int spr = IN == BF_CI4 ? 4 : 2;                                 // samples per 128-byte row
   const cuuint64_t chan_bytes = (cuuint64_t)p.nsamp * (128 / spr);
-  // {byte in row, row in chunk, bin, chunk in bin, channel}: a tile = chunk g of 128 / LPB consecutive bins
-  cuuint64_t dims[5] = {128, LPB, (cuuint64_t)p.nbin, (cuuint64_t)(nint / spr / LPB), (cuuint64_t)p.nchan_run};
-  cuuint64_t strides[4] = {128, (cuuint64_t)nint * (128 / spr), 128 * LPB, chan_bytes};
-  cuuint32_t box[5] = {128, LPB, 128 / LPB, 1, 1};
+  // {byte in row, 1, bin, row in bin, channel}: a tile = row g of 128 consecutive bins
+  cuuint64_t dims[5] = {128, 1, (cuuint64_t)p.nbin, (cuuint64_t)(nint / spr), (cuuint64_t)p.nchan_run};
+  cuuint64_t strides[4] = {128, (cuuint64_t)nint * (128 / spr), 128, chan_bytes};
+  cuuint32_t box[5] = {128, 1, 128, 1, 1};
   cuuint32_t estr[5] = {1, 1, 1, 1, 1};
   CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 5, const_cast<void *>(p.volt), dims, strides, box, estr,
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -456,19 +451,19 @@ cudaError_t make_tmap_bins(CUtensorMap *tm, const BfParams &p, int nint) {
   return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-template <int NCOL, int IN, int LPB>
-cudaError_t launch_i8b_lpb(const BfParams &p, int sm_count, cudaStream_t st) {
+template <int NCOL, int IN>
+cudaError_t launch_i8b(const BfParams &p, int sm_count, cudaStream_t st) {
   constexpr bool CI4 = IN == BF_CI4, ATM = CI4 && NCOL <= 64;   // ATM: operands in tensor memory, no shared-memory operand stages
   constexpr int NST = ATM ? 0 : (CI4 ? 6 : 12), NRAW = ATM ? 12 : (CI4 ? 6 : 0);
   CUtensorMap tm;
-  cudaError_t e = bf_cached_tmap(&tm, p, (CI4 ? 20 : 10) + LPB, p.nint, make_tmap_bins<IN, LPB>);
+  cudaError_t e = bf_cached_tmap(&tm, p, CI4 ? 21 : 11, p.nint, make_tmap_bins<IN>);
   if (e != cudaSuccess) return e;
-  const int G = p.nint / (CI4 ? 4 : 2) / LPB;
-  const int n_super_chan = (p.nbin + 128 / LPB - 1) / (128 / LPB);
+  const int G = p.nint / (CI4 ? 4 : 2);           // raw rows per bin
+  const int n_super_chan = (p.nbin + 127) / 128;
   const long long total = (long long)p.nchan_run * n_super_chan;
   constexpr int X_BYTES = b_tsets(NCOL) > 1 ? 2 * 4 * 8 * (NCOL / 32) * 32 * 4 : 0;   // tile-set exchange buffers
   const size_t smem = 1024 + 2 * NCOL * B_W_ROW_BYTES + (size_t)(NST + NRAW) * B_STAGE_BYTES + X_BYTES + 1024;
-  auto kern = bf_umma_i8b_kernel<NCOL, NST, NRAW, IN, LPB>;
+  auto kern = bf_umma_i8b_kernel<NCOL, NST, NRAW, IN>;
   static thread_local int attr_dev = -1;   // once per instantiation and device
   if ((e = bf_set_smem_once(kern, smem, &attr_dev)) != cudaSuccess) return e;
   const int grid = (int)(total < sm_count ? total : sm_count);
@@ -476,14 +471,9 @@ cudaError_t launch_i8b_lpb(const BfParams &p, int sm_count, cudaStream_t st) {
   return cudaGetLastError();
 }
 
-// LPB = lanes per bin.  1: every 128-byte row of a tile comes from another bin, no cross-lane sum at all.  2 / 4
-// (chunks of 256 / 512 contiguous bytes, one / two shuffle-adds per beam at the end of a super-tile) were measured
-// on the sweep and are slower at every beam count (32 beams: 0.117 / 0.156 / 0.237 ms for LPB 1 / 2 / 4): a
-// super-tile then has half / a quarter of the tiles to amortise its reduction and stores over.  Only 1 is built.
-template <int NCOL, int IN>
-cudaError_t launch_i8b(const BfParams &p, int sm_count, cudaStream_t st) {
-  return launch_i8b_lpb<NCOL, IN, 1>(p, sm_count, st);
-}
+// (Tiles with two / four lanes per bin -- chunks of 256 / 512 contiguous bytes, one / two shuffle-adds per beam at the end
+// of a super-tile -- were measured on the sweep and are slower at every beam count, 32 beams: 0.117 / 0.156 / 0.237 ms for
+// 1 / 2 / 4 lanes per bin; DESIGN.md 5.3d.  Only one lane per bin is built.)
 
 }  // namespace
 

@@ -84,28 +84,20 @@ BF_DEVI bool mbar_try_wait_hint(uint32_t bar, uint32_t parity, uint32_t ns) {
       : "memory");
   return ok != 0;
 }
-// Bounded wait: a mis-phased pipeline must fail (trap), not hang the GPU.  The poll loop is two
-// instructions; the clock is looked at once per 4096 polls and the wait gives up after ~2 s.
-#ifndef BF_WAIT_HINT_NS
-#define BF_WAIT_HINT_NS 0
-#endif
+// Waits.  ONE policy for all four flavours below: a wait never spins for ever -- a mis-phased pipeline must fail (trap),
+// not hang the GPU -- and its bound is far above anything a healthy run needs (tens of seconds and more: a time-sliced
+// or profiled GPU must never trip it), so the exact figure is no part of any contract.  mbar_wait counts SM clocks (it
+// looks at clock64 once per 4096 polls, ~20 s at 2 GHz); mbar_wait_backoff / _tight / _hinted count 2^26 polls, each of
+// which blocks for the hardware's try_wait time slice (plus the sleep / suspend hint), which comes to the same order.
+// They differ only in what a failed poll costs the other warps of the SM.
 BF_DEVI void mbar_wait(uint32_t bar, uint32_t parity) {
-#if BF_WAIT_HINT_NS > 0
-  if (mbar_try_wait_hint(bar, parity, BF_WAIT_HINT_NS)) return;
-#else
   if (mbar_try_wait(bar, parity)) return;
-#endif
   const long long t0 = clock64();
   for (;;) {
 #pragma unroll 1
     for (int k = 0; k < 4096; ++k) {
-#if BF_WAIT_HINT_NS > 0
-      if (mbar_try_wait_hint(bar, parity, BF_WAIT_HINT_NS)) return;
-#else
       if (mbar_try_wait(bar, parity)) return;
-#endif
     }
-    // ~20 s at 2 GHz: long enough for a time-sliced or profiled GPU, short enough to fail instead of hanging
     if (clock64() - t0 > 40000000000LL) asm volatile("trap;");
   }
 }
