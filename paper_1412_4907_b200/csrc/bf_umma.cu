@@ -68,6 +68,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
   extern __shared__ uint8_t smem_raw[];
   constexpr int CONV_THREADS = CONV_WARPS * 32;
   static_assert(CONV_WARPS == 8, "role table below assumes 8 convert warps");
+  static_assert(GROUP > 1 || NSTAGE == 2, "GROUP == 1: each MMA warp must see every completion of the operand stages it waits on");
 
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   constexpr int APB = (LO ? 2 : 1) * GROUP;                       // coefficient tiles per buffer
@@ -396,6 +397,13 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         ++ag;
       }
       const bool mine = GROUP == 1 ? ((i & 1) == id) : (id < gm);
+      // A warp with no tile in this item (the second warp when the last beam group holds ONE M-tile) must still wait for
+      // the item's operand stage: a parity wait cannot tell completion n from n + 2, so a warp that walked past a whole
+      // run of such items without looking at their barriers would find the "full" barrier of its next own item already
+      // satisfied by an OLD phase and multiply a stale stage (seen as wrong powers in the second M-tile of the next
+      // channel's first time tile, one launch in a few -- tests/test_gpu_combos.py::test_fifty_runs_are_bit_equal).
+      // (GROUP == 1: the warps alternate items on two stages, i.e. each waits for every completion of its own stage.)
+      if (GROUP > 1 && !mine) mbar_wait(bar_b_full + 8 * st, st_par);
       if (mine) {
         const uint32_t b_full = bar_b_full + 8 * st, b_empty = bar_b_empty + 8 * st;
         mbar_wait(b_full, st_par);

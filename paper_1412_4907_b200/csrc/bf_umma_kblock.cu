@@ -178,9 +178,12 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
       const bool mine = id < gm;  // an odd last group has no second M-tile
       if (mine) { mbar_wait(bar_t_empty + 8 * id, tpar); tpar ^= 1; tc_fence_after(); }
       for (int kb = 0; kb < nKb; ++kb) {
+        // both warps wait for EVERY K-block, also the warp without a tile in this item: a parity wait cannot tell
+        // completion n from n + 2, so a warp that skipped the barriers of a whole item (nKb K-blocks, more than twice the
+        // ring) would find the barriers of its next own item satisfied by an old phase (see bf_umma.cu)
+        mbar_wait(bar_a_full + 8 * sa, apar);
+        mbar_wait(bar_b_full + 8 * sb, bpar);
         if (mine) {
-          mbar_wait(bar_a_full + 8 * sa, apar);
-          mbar_wait(bar_b_full + 8 * sb, bpar);
           tc_fence_after();
           if (elect_one()) {
             const uint64_t bdesc = bdesc0 + (uint64_t)(sb * (B_STAGE_BYTES >> 4));

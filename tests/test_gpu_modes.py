@@ -47,6 +47,8 @@ BEAM_CASES = [
     (32, 2, 16, 256, "ci4"),
     (32, 3, 1, 2050, "ci8"),     # int8 kernel: one beam, several tiles, ragged tail of one sample pair
     (32, 2, 32, 768, "ci8"),     # int8 kernel: 128 accumulator columns
+    (64, 2, 16, 256, "ci4"),     # 4+4-bit input on the K-blocked kernel in voltage-beam mode
+    (1024, 1, 70, 256, "ci4"),   # ... with 32 K-blocks and a second, partial M-tile
 ]
 
 
