@@ -14,7 +14,8 @@ import ctypes
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libbf.so")
+# BF_LIBRARY: load another build of the same library instead (the tests point it at the jitter build, libbf_jitter.so)
+LIB_PATH = os.environ.get("BF_LIBRARY") or os.path.join(_HERE, "libbf.so")
 
 BF_OK, BF_EINVAL, BF_ENOGEOM, BF_ECUDA, BF_EUNSUPPORTED, BF_ENOMEM = 0, -1, -2, -3, -4, -5
 BF_CI8, BF_CF16, BF_CI4 = 0, 1, 2

@@ -57,7 +57,11 @@ static size_t wop8_bytes(const bf_ctx *c) {
   return i8_shape(c) ? align_up((size_t)c->nchan * bf_i8_ncol(c->nbeam) * 64, BF_ALIGN) : 0;
 }
 
+#ifdef BF_JITTER
+extern "C" const char *bf_version(void) { return "paper_1412_4907_b200 0.1 (sm_100a) [jitter build: test only]"; }
+#else
 extern "C" const char *bf_version(void) { return "paper_1412_4907_b200 0.1 (sm_100a)"; }
+#endif
 
 extern "C" bf_ctx *bf_create(int nant, int nchan, int nbeam, int nsamp, int nint) {
   if (nant <= 0 || nchan <= 0 || nbeam <= 0 || nsamp <= 0 || nint <= 0) return nullptr;

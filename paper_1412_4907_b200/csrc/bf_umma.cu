@@ -397,13 +397,18 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
         ++ag;
       }
       const bool mine = GROUP == 1 ? ((i & 1) == id) : (id < gm);
-      // A warp with no tile in this item (the second warp when the last beam group holds ONE M-tile) must still wait for
-      // the item's operand stage: a parity wait cannot tell completion n from n + 2, so a warp that walked past a whole
-      // run of such items without looking at their barriers would find the "full" barrier of its next own item already
-      // satisfied by an OLD phase and multiply a stale stage (seen as wrong powers in the second M-tile of the next
-      // channel's first time tile, one launch in a few -- tests/test_gpu_combos.py::test_fifty_runs_are_bit_equal).
-      // (GROUP == 1: the warps alternate items on two stages, i.e. each waits for every completion of its own stage.)
-      if (GROUP > 1 && !mine) mbar_wait(bar_b_full + 8 * st, st_par);
+      // A warp with no tile in this item (the second warp when the last beam group holds ONE M-tile) still takes part in
+      // the hand-shake of the item's operand stage: it waits for "full" and gives its own arrival to "empty".  A parity wait
+      // cannot tell completion n from n + 2, so the warp must neither run ahead of a stage it does not look at (it walked
+      // past a run of such items and then multiplied a STALE stage at its next own item: wrong powers in the second M-tile
+      // of one time tile, one launch in a few) nor fall two completions behind it (if the other warp arrived twice on its
+      // behalf, nothing would hold the ring back for a late warp, and it would wait for ever).  Found by
+      // tests/test_gpu_combos.py::test_fifty_runs_are_bit_equal and tests/test_zy_jitter.py.
+      // (GROUP == 1: the warps alternate items on two stages; each owns every completion of its own stage.)
+      if (GROUP > 1 && !mine) {
+        mbar_wait(bar_b_full + 8 * st, st_par);
+        if (elect_one()) mbar_arrive(bar_b_empty + 8 * st);   // nothing of mine reads the stage: a plain arrival
+      }
       if (mine) {
         const uint32_t b_full = bar_b_full + 8 * st, b_empty = bar_b_empty + 8 * st;
         mbar_wait(b_full, st_par);
@@ -426,7 +431,7 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
             tc_commit(t_full);
             if (last) {
               tc_commit(b_empty);
-              if (gm == 1) tc_commit(b_empty);  // the other warp has no tile in this item
+              if (GROUP == 1) tc_commit(b_empty);  // the stage is mine alone: both arrivals
             }
           }
         }

@@ -178,11 +178,13 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
       const bool mine = id < gm;  // an odd last group has no second M-tile
       if (mine) { mbar_wait(bar_t_empty + 8 * id, tpar); tpar ^= 1; tc_fence_after(); }
       for (int kb = 0; kb < nKb; ++kb) {
-        // both warps wait for EVERY K-block, also the warp without a tile in this item: a parity wait cannot tell
-        // completion n from n + 2, so a warp that skipped the barriers of a whole item (nKb K-blocks, more than twice the
-        // ring) would find the barriers of its next own item satisfied by an old phase (see bf_umma.cu)
+        // Both warps take part in the hand-shake of EVERY K-block, also the warp without a tile in this item (an odd last
+        // beam group): it waits for "full" and gives its own arrival to "empty".  A parity wait cannot tell completion n
+        // from n + 2: a warp that skipped the barriers of a whole item would find those of its next own item satisfied by
+        // an old phase, and a warp the other one arrived for could fall two completions behind and wait for ever (bf_umma.cu).
         mbar_wait(bar_a_full + 8 * sa, apar);
         mbar_wait(bar_b_full + 8 * sb, bpar);
+        if (!mine && elect_one()) { mbar_arrive(bar_a_empty + 8 * sa); mbar_arrive(bar_b_empty + 8 * sb); }
         if (mine) {
           tc_fence_after();
           if (elect_one()) {
@@ -197,7 +199,6 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
             }
             tc_commit(bar_a_empty + 8 * sa);
             tc_commit(bar_b_empty + 8 * sb);
-            if (gm == 1) { tc_commit(bar_a_empty + 8 * sa); tc_commit(bar_b_empty + 8 * sb); }  // other warp idle
             if (kb == nKb - 1) tc_commit(bar_t_full + 8 * id);
           }
         }

@@ -84,6 +84,22 @@ BF_DEVI bool mbar_try_wait_hint(uint32_t bar, uint32_t parity, uint32_t ns) {
       : "memory");
   return ok != 0;
 }
+// Test-only jitter build (python -m paper_1412_4907_b200.build --jitter -> libbf_jitter.so, -DBF_JITTER=1): every
+// mbarrier wait below first sleeps for a pseudo-random 0-2 us drawn from the SM clock, the CTA and the warp, so that the
+// warp-specialised roles meet their barriers in orders and with leads that the undisturbed kernel never shows.  The
+// results must not change (tests/test_zy_jitter.py): compute-sanitizer is closed on this pool, and a protocol that only
+// holds for the usual timing is exactly what an undisturbed parity test cannot see.  The product library has no trace of it.
+#ifdef BF_JITTER
+BF_DEVI void bf_jitter() {
+  uint32_t x = (uint32_t)clock64() * 2654435761u ^ (threadIdx.x >> 5) * 40503u ^ blockIdx.x * 69069u;
+  x ^= x >> 15; x *= 2246822519u; x ^= x >> 13;
+  if (x & 0x30000u) return;                    // three waits in four go straight through: leads build up and collapse
+  asm volatile("nanosleep.u32 %0;" ::"r"(x & 2047u));
+}
+#else
+BF_DEVI void bf_jitter() {}
+#endif
+
 // Waits.  ONE policy for all four flavours below: a wait never spins for ever -- a mis-phased pipeline must fail (trap),
 // not hang the GPU -- and its bound is far above anything a healthy run needs (tens of seconds and more: a time-sliced
 // or profiled GPU must never trip it), so the exact figure is no part of any contract.  mbar_wait counts SM clocks (it
@@ -91,6 +107,7 @@ BF_DEVI bool mbar_try_wait_hint(uint32_t bar, uint32_t parity, uint32_t ns) {
 // which blocks for the hardware's try_wait time slice (plus the sleep / suspend hint), which comes to the same order.
 // They differ only in what a failed poll costs the other warps of the SM.
 BF_DEVI void mbar_wait(uint32_t bar, uint32_t parity) {
+  bf_jitter();
   if (mbar_try_wait(bar, parity)) return;
   const long long t0 = clock64();
   for (;;) {
@@ -105,6 +122,7 @@ BF_DEVI void mbar_wait(uint32_t bar, uint32_t parity) {
 // that the waiting warps stop taking issue slots from the working ones (ncu: 56 % of the streaming kernel's
 // instructions were such polls).  Bounded like the others.
 BF_DEVI void mbar_wait_backoff(uint32_t bar, uint32_t parity, uint32_t sleep_ns) {
+  bf_jitter();
   if (mbar_try_wait(bar, parity)) return;
   for (uint32_t n = 0;; ++n) {
     asm volatile("nanosleep.u32 %0;" ::"r"(sleep_ns));
@@ -115,6 +133,7 @@ BF_DEVI void mbar_wait_backoff(uint32_t bar, uint32_t parity, uint32_t sleep_ns)
 // Tight bounded wait for roles on the critical chain (the epilogue): two instructions per failed poll, trap after
 // 2^26 polls (a try_wait blocks for a hardware-defined slice, so this is seconds, not a hang).
 BF_DEVI void mbar_wait_tight(uint32_t bar, uint32_t parity) {
+  bf_jitter();
   // four polls per trip of the bounding counter: a failed poll costs two issue slots, and every slot a waiting
   // warp takes is one a working warp of the same sub-partition does not get
   asm volatile(
@@ -142,6 +161,7 @@ BF_DEVI void mbar_wait_tight(uint32_t bar, uint32_t parity) {
 // faster on sweep-32 and sweep-ci4-16 than the tight spin; in the resident fp16 kernel the same wait is 7 % SLOWER at
 // 64 beams (A/B on one box), so that kernel keeps mbar_wait_tight.
 BF_DEVI void mbar_wait_hinted(uint32_t bar, uint32_t parity, uint32_t ns) {
+  bf_jitter();
   if (mbar_try_wait(bar, parity)) return;
   for (uint32_t n = 0;; ++n) {
     if (mbar_try_wait_hint(bar, parity, ns)) return;
