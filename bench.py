@@ -332,6 +332,29 @@ class Timed:
         else:
             self.B.run(v, self.P, self.stream)
 
+    def graph_replay_ms(self, replays=20):
+        """The short-launch regime (hard part 8): n consecutive bf_run calls, each on another copy of the
+        input, captured into ONE CUDA graph and replayed; returns ms per call.  Against the plain back-to-back figure
+        this separates what the kernel costs from what launching it costs."""
+        torch = self.torch
+        n = max(self.ncopy, 16)
+        g, s = torch.cuda.CUDAGraph(), torch.cuda.Stream(self.dev)
+        torch.cuda.synchronize(self.dev)
+        with torch.cuda.graph(g, stream=s):
+            cur = torch.cuda.current_stream(self.dev)
+            for k in range(n):
+                self.B.run(self.v[k % self.ncopy], self.P, cur)
+        for _ in range(3):
+            g.replay()
+        torch.cuda.synchronize(self.dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(replays):
+            g.replay()
+        e1.record()
+        torch.cuda.synchronize(self.dev)
+        return e0.elapsed_time(e1) / (replays * n), n
+
     def flop_step(self):
         w = self.w
         return 8.0 * w.cmac if self.mode != "incoherent" else 4.0 * w.nchan * w.nsamp * w.nant  # |x|^2 + add
@@ -598,6 +621,31 @@ def main():
                 "frac_of_sustained": r.get("frac_of_sustained"), "achieved": r["achieved"], "unit": r["unit"],
                 "traffic": r["traffic"], "kernel": Tc.B.kernel_name, "tflops": Tc.flop_step() / (ms * 1e-3) / 1e12,
                 "steps": Kc, "clocks": clk, "l2": Tc.l2}
+            if name == "tiny":
+                # the same launches out of a CUDA graph: per-call time without the host's launch cost
+                gms, gn = Tc.graph_replay_ms()
+                rg = Tc.roofline(gms, gms * gn * 20, clk, peaks, None)
+                configs["tiny:graph"] = dict(configs[wc.name], ms=gms, frac=rg["frac"], achieved=rg["achieved"], traffic=None,
+                                             tflops=Tc.flop_step() / (gms * 1e-3) / 1e12, steps=gn * 20,
+                                             note="%d bf_run calls captured in one CUDA graph, 20 replays" % gn)
+            Tc.close()
+            del Tc
+            torch.cuda.empty_cache()
+        # side modes on medium's input: voltage beams (the S-engine ships 8 of the beams as 16-bit
+        # complex words; 32 and 128 show the output-bound regime) and the incoherent beam
+        for label, mode, nb in (("medium:beams-8", "beams", 8), ("medium:beams-32", "beams", 32), ("medium:beams-128", "beams", 128),
+                                ("medium:incoherent", "incoherent", 0)):
+            wc = workload_for("medium")
+            if nb:
+                wc = wc.sub(nbeam=nb)
+            Tc = Timed(bf, synthetic, torch, wc, dev, bf.BF_KERNEL_AUTO, mode)
+            tot, per, _, clk = Tc.measure(20, 3, barrier)
+            ms = statistics.mean(per)
+            r = Tc.roofline(ms, tot, clk, peaks, None)
+            configs[label] = {"ms": ms, "bound": r["bound"], "frac": r["frac"], "frac_of_burst": r.get("frac_of_burst"),
+                              "frac_of_sustained": r.get("frac_of_sustained"), "achieved": r["achieved"], "unit": r["unit"],
+                              "traffic": None, "kernel": Tc.B.kernel_name if mode == "beams" else "incoherent-dp4a",
+                              "tflops": Tc.flop_step() / (ms * 1e-3) / 1e12, "steps": 20, "clocks": clk, "l2": Tc.l2}
             Tc.close()
             del Tc
             torch.cuda.empty_cache()

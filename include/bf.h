@@ -186,8 +186,21 @@ int bf_get_weights_noalloc(bf_ctx *ctx, int chan0, int nchan_out, float *host_ou
 
 /*
  * The hot path.  voltages: DEVICE, [nchan][nsamp][nant][2] (re, im interleaved) of the context's
- * dtype ([nchan][nsamp][nant] bytes for BF_CI4), 16-byte aligned.  powers: DEVICE fp32 [nchan][nbeam][nsamp/nint], fully overwritten.
- * Enqueues on `stream` and returns.  BF_ENOGEOM before bf_set_geometry.
+ * dtype ([nchan][nsamp][nant] bytes for BF_CI4), 16-byte aligned.  powers: DEVICE fp32 [nchan][nbeam][nsamp/nint], 4-byte
+ * aligned (16-byte aligned powers with nsamp/nint a multiple of 4 get vector stores), fully overwritten.
+ * Enqueues on `stream` and returns.  BF_ENOGEOM before bf_set_geometry; BF_EINVAL for a misaligned pointer.
+ *
+ * Reproducibility: the result of a call depends only on its inputs -- repeated calls give bit-equal powers (tested: 50
+ * launches per kernel, also with randomly delayed barrier waits) -- with ONE exception: nint a multiple of 64 above 64
+ * on the fp16-operand kernels (more than 32 beams, or nant > 32) is integrated with fp32 atomic adds into powers zeroed
+ * by a cudaMemsetAsync the call enqueues first; the order of those adds varies, so such results agree from run to run
+ * only to fp32 rounding of the partial sums (well inside the 1e-3 bar).
+ *
+ * CUDA graphs: a bf_run on a context with ONE weight buffer enqueues only a kernel (plus that memset) and may be captured
+ * into a graph once the SAME call has been made un-captured before (the first launch of a kernel variant sets function
+ * attributes and encodes tensor maps on the host; the maps are then taken from a cache keyed by the buffer addresses).  The
+ * captured launch refers to the voltages / powers / workspace addresses it was given.  With two weight buffers the call
+ * also records events for bf_update_geometry and is not meant to be captured.
  */
 int bf_run(bf_ctx *ctx, const void *voltages, float *powers, void *stream);
 

@@ -488,6 +488,7 @@ extern "C" int bf_run(bf_ctx *c, const void *voltages, float *powers, void *stre
   int rc = check_run(c, voltages, powers);
   if (rc != BF_OK) return rc;
   if (((uintptr_t)voltages) % 16) return fail(c, BF_EINVAL, "voltages must be 16-byte aligned");
+  if (((uintptr_t)powers) % 4) return fail(c, BF_EINVAL, "powers must be 4-byte aligned");
   if ((rc = begin_run(c, (cudaStream_t)stream)) != BF_OK) return rc;
   rc = launch_range(c, voltages, powers, 0, c->nchan, (cudaStream_t)stream);
   return finish_run(c, (cudaStream_t)stream, rc);

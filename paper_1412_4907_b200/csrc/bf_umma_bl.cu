@@ -41,12 +41,6 @@ constexpr int BL_RAW_BYTES = 128 * 128;                // 16 KiB: 128 bins x two
 constexpr int BL_EPI_WARPS = 16, BL_MMA_WARP0 = 20, BL_TMA_WARP = 22;
 constexpr int BL_THREADS = 23 * 32;
 
-BF_DEVI void bl_tma_load_5d(uint32_t dst_smem, const void *tmap, int x, int y, int z, int w, int v, uint32_t bar) {
-  asm volatile(
-      "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];"
-      ::"r"(dst_smem), "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(w), "r"(v), "r"(bar) : "memory");
-}
-
 // NRAW: raw stages.  IN: BF_CI8 (raw rows of 128 bytes = two samples) or BF_CI4 (the paper's 4+4-bit bytes, PAPER.md:102:
 // raw rows of 64 bytes = two samples, 64-byte swizzle).  n_items = channels x super-tile pairs per channel (nSP2).
 template <int NRAW, int IN>
@@ -293,7 +287,7 @@ bf_umma_bl_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap, co
         for (int h = 0; h < 2; ++h) {   // row g of super-tile X, then of Y (bins past nbin are zero-filled)
           mbar_wait(bar_r_empty + 8 * rs, rpar);
           mbar_arrive_expect_tx(bar_r_full + 8 * rs, RAW_BYTES);
-          bl_tma_load_5d(sR + rs * BL_RAW_BYTES, &tmap, 0, 0, 128 * (2 * q + h), g, c, bar_r_full + 8 * rs);
+          tma_load_5d(sR + rs * BL_RAW_BYTES, &tmap, 0, 0, 128 * (2 * q + h), g, c, bar_r_full + 8 * rs);
           if (++rs == NRAW) { rs = 0; rpar ^= 1; }
         }
       }

@@ -52,12 +52,6 @@ __host__ __device__ constexpr int b_nsets(int ncol) { return b_csets(ncol) * b_t
 
 __host__ __device__ constexpr int b_ilog2(int x) { return x <= 1 ? 0 : 1 + b_ilog2(x >> 1); }
 
-BF_DEVI void tma_load_5d(uint32_t dst_smem, const void *tmap, int x, int y, int z, int w, int v, uint32_t bar) {
-  asm volatile(
-      "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];"
-      ::"r"(dst_smem), "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(w), "r"(v), "r"(bar) : "memory");
-}
-
 // unpack groups (4-bit input): groups of four warps on alternate raw tiles.  ONE: a second group (and likewise a second
 // MMA-issuing warp) was measured and changes nothing (sweep-ci4, 8 beams: 0.0638 / 0.0646 / 0.0667 ms)
 __host__ __device__ constexpr int b_ugroups(int ncol) { return 1; }

@@ -57,6 +57,13 @@ BF_DEVI void tma_load_3d(uint32_t dst_smem, const void *tmap, int x, int y, int 
       "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
       ::"r"(dst_smem), "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(bar) : "memory");
 }
+// the same in 5-D: the bin-per-lane kernels (bf_umma_i8b.cu, bf_umma_bl.cu) view the voltages as
+// {byte in row, 1, bin, row in bin, channel} and fetch one row of 128 consecutive bins per copy
+BF_DEVI void tma_load_5d(uint32_t dst_smem, const void *tmap, int x, int y, int z, int w, int v, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];"
+      ::"r"(dst_smem), "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(w), "r"(v), "r"(bar) : "memory");
+}
 BF_DEVI void tma_prefetch_desc(const void *tmap) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(tmap) : "memory");
 }

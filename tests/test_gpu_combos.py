@@ -178,3 +178,74 @@ def test_fifty_runs_are_bit_equal(bf, case):
     torch.cuda.synchronize()
     assert bad == 0, f"{bad} of 50 runs differ from the first"
     Bf.close()
+
+
+GRAPH_CASES = [
+    # nant nchan nbeam nsamp nint dtype kernel
+    (32, 64, 16, 1024, 16, "ci8", "umma-i8"),              # BASELINE.json's `tiny`
+    (32, 24, 24, 4096, 16, "ci8", "umma-i8"),              # bin per lane (5-D tensor map from the cache)
+    (32, 24, 64, 8192, 16, "ci4", "umma-f16-binlane"),
+    (32, 24, 128, 2048, 64, "ci8", "umma-f16-resident"),
+    (256, 4, 256, 1024, 32, "cf16", "umma-f16-kblock"),
+    (64, 4, 70, 1024, 128, "ci8", "umma-f16-kblock"),      # nint = 128: the memset + atomics path is two graph nodes
+]
+
+
+@pytest.mark.parametrize("case", GRAPH_CASES, ids=lambda s: "N%d-C%d-B%d-T%d-I%d-%s" % s[:6])
+def test_bf_run_in_a_cuda_graph(bf, case):
+    """include/bf.h: bf_run with one weight buffer may be captured once the same call has run un-captured.  Capture three
+    calls on two alternating inputs, replay the graph 100 times, and compare with the direct calls."""
+    import torch
+    N, C, B, T, I, dtype, name = case
+    dev = torch.device("cuda")
+    w = synthetic.make_case(N, C, B, T, I, dtype, seed=29)
+    va = synthetic.fill_voltages_torch(w, dev, chunk_chan=8)
+    vb = torch.roll(va, 1, dims=1).contiguous()
+    Bf = bf.Beamformer(N, C, B, T, I, dtype=DT[dtype])
+    assert Bf.kernel_name == name
+    Bf.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
+    Pa, Pb = Bf.run(va), Bf.run(vb)          # un-captured first: attributes set, tensor maps cached
+    torch.cuda.synchronize()
+    ref = oracle.beamform(w.ant_xyz, w.freqs[:1], w.beam_dir, va[:1].cpu().numpy(), I)
+    assert worst_row(Pa[:1].cpu().numpy(), ref) <= TOL
+    atomic = name != "umma-i8" and I > 64
+    Ga, Gb, Ga2 = (Bf.empty_powers() for _ in range(3))
+    s = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    n0 = Bf.launches
+    with torch.cuda.graph(g, stream=s):
+        cur = torch.cuda.current_stream()
+        Bf.run(va, Ga, stream=cur)
+        Bf.run(vb, Gb, stream=cur)
+        Bf.run(va, Ga2, stream=cur)
+    assert Bf.launches - n0 == 3
+    for rep in range(100):
+        if rep in (0, 57):
+            for G_ in (Ga, Gb, Ga2):
+                G_.fill_(float("nan"))
+            torch.cuda.synchronize()
+        g.replay()
+    torch.cuda.synchronize()
+    for got, want in ((Ga, Pa), (Gb, Pb), (Ga2, Pa)):
+        if atomic:   # fp32 atomics: equal to rounding of the partial sums
+            assert worst_row(got.cpu().numpy(), want.cpu().numpy().astype(np.float64)) <= 1e-5
+        else:
+            assert torch.equal(got, want)
+    Bf.close()
+
+
+def test_bf_run_rejects_misaligned_pointers(bf):
+    import torch
+    w = synthetic.make_case(32, 2, 16, 256, 16, "ci8", seed=31)
+    Bf = bf.Beamformer(32, 2, 16, 256, 16)
+    Bf.set_geometry(w.ant_xyz, w.freqs, w.beam_dir)
+    v = torch.zeros(2 * 256 * 32 * 2 + 64, dtype=torch.int8, device="cuda")
+    P = torch.zeros(2 * 16 * 16 * 4 + 64, dtype=torch.uint8, device="cuda")
+    assert bf.bf_run(Bf.ctx, v.data_ptr(), P.data_ptr()) == bf.BF_OK
+    assert bf.bf_run(Bf.ctx, v.data_ptr(), P.data_ptr() + 4) == bf.BF_OK        # 4-byte aligned powers are fine
+    assert bf.bf_run(Bf.ctx, v.data_ptr(), P.data_ptr() + 2) == bf.BF_EINVAL
+    assert "powers" in bf.bf_last_error(Bf.ctx)
+    assert bf.bf_run(Bf.ctx, v.data_ptr() + 8, P.data_ptr()) == bf.BF_EINVAL
+    assert "voltages" in bf.bf_last_error(Bf.ctx)
+    torch.cuda.synchronize()
+    Bf.close()
