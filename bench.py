@@ -430,6 +430,44 @@ class Timed:
 TRAFFIC_SOURCE = "profiles/traffic.json (ncu --set full capture, per launch; not measured in this run)"
 
 
+def streaming_e2e_row(bf, synthetic, torch, dev, barrier, kernel_ms):
+    """BASELINE.json config 5's own end-to-end leg: "continuous blocks ... from pinned host memory with H2D copies overlapped
+    on a side stream ... reports end-to-end sustained samples/s vs input data rate".  8 pinned host blocks per
+    bf_run_streaming call (two distinct ones cycled), double-buffered staging, powers stay on the device; what the input
+    link delivers (H2D GB/s) is the input data rate D = C*T*A*W of PAPER.md:176 that the GPU can be fed with."""
+    w = workload_for("streaming")
+    T = Timed(bf, synthetic, torch, w, dev, bf.BF_KERNEL_AUTO)
+    v = T.v[0]
+    hv = torch.empty(v.shape, dtype=v.dtype, pin_memory=True)
+    hv.copy_(v)
+    hv2 = torch.empty(v.shape, dtype=v.dtype, pin_memory=True)
+    hv2.copy_(torch.roll(v, 1, dims=1))
+    nblk, calls = 8, 3
+    blocks = [hv if (i % 2 == 0) else hv2 for i in range(nblk)]
+    Pb = torch.empty((nblk,) + tuple(T.P.shape), dtype=torch.float32, device=dev)
+    cs, xs = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+    T.B.run_streaming(blocks, Pb, cs, xs)
+    cs.synchronize(); xs.synchronize()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(cs)
+    for _ in range(calls):
+        T.B.run_streaming(blocks, Pb, cs, xs)
+    cs.wait_stream(xs)
+    e1.record(cs)
+    cs.synchronize(); xs.synchronize()
+    ms = e0.elapsed_time(e1) / (calls * nblk)
+    row = {"ms": ms, "bound": "pcie", "frac": None, "unit": "GB/s", "achieved": w.in_bytes / (ms * 1e-3) / 1e9,
+           "h2d_gbs": w.in_bytes / (ms * 1e-3) / 1e9, "ant_samples_per_s": w.nchan * w.nsamp * w.nant / (ms * 1e-3),
+           "tflops": T.flop_step() / (ms * 1e-3) / 1e12, "kernel_ms_per_block": kernel_ms,
+           "kernel_share_of_block_time": kernel_ms / ms, "steps": calls * nblk, "traffic": None, "kernel": T.B.kernel_name,
+           "api": "bf_run_streaming (8 pinned host blocks per call, 2 streams, double-buffered staging, powers stay on device)",
+           "note": "frac is null: the bound is the host link, for which MEASURED_PEAKS.json has no figure; the kernel needs "
+                   "kernel_share_of_block_time of each block's transfer time"}
+    T.close()
+    return row
+
+
 def load_traffic(name):
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     try:
@@ -631,6 +669,12 @@ def main():
             Tc.close()
             del Tc
             torch.cuda.empty_cache()
+        if "streaming" in configs:
+            try:
+                configs["streaming:e2e"] = streaming_e2e_row(bf, synthetic, torch, dev, barrier, configs["streaming"]["ms"])
+            except Exception as exc:  # a leg that cannot run (no pinned memory left) must not cost the whole line
+                configs["streaming:e2e"] = {"error": repr(exc)[:200]}
+            torch.cuda.empty_cache()
         # side modes on medium's input: voltage beams (the S-engine ships 8 of the beams as 16-bit
         # complex words; 32 and 128 show the output-bound regime) and the incoherent beam
         for label, mode, nb in (("medium:beams-8", "beams", 8), ("medium:beams-32", "beams", 32), ("medium:beams-128", "beams", 128),
@@ -669,8 +713,9 @@ def main():
             # compact copy of the table as the LAST key, so that it survives a reader that keeps only the tail of the line:
             # name -> [ms per launch, frac of roofline (tensor rows: burst GEMM peak; hbm rows: copy bandwidth), "t" | "h",
             # SM MHz from the kernel's own clock probe]
-            line["summary"] = {n: [round(c["ms"], 5), round(c["frac"], 4), c["bound"][0],
-                                   round((c.get("clocks") or {}).get("kernel_sm_mhz") or 0)] for n, c in configs.items()}
+            line["summary"] = {n: [round(c["ms"], 5), None if c["frac"] is None else round(c["frac"], 4), c["bound"][0],
+                                   round((c.get("clocks") or {}).get("kernel_sm_mhz") or 0)]
+                               for n, c in configs.items() if "ms" in c}
         print(json.dumps(line))
     if dist:
         td.destroy_process_group()
