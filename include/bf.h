@@ -55,14 +55,13 @@ enum bf_dtype {
 };
 
 enum bf_kernel {
-  BF_KERNEL_AUTO = 0, /* pick the fastest kernel that supports the shape.  NOTE: for shapes no tensor-core kernel takes (nant
-                         not a multiple of 8 (int8) / 4 (fp16) / 16 (4+4-bit), nint neither 2^k <= 64 nor a multiple of 64 / 32 -- except on
-                         32 antennas with <= 32 beams, where any EVEN nint integrates on tensor cores when nsamp / nint is a
-                         multiple of 128 or >= 512, and with 33-64 beams, where any even nint >= 16 does when nsamp / nint is a
-                         multiple of 256 or >= 1024)
-                         AUTO falls through to BF_KERNEL_SIMT without an error -- about 30x slower on the `tiny` shape;
-                         bf_kernel_name / bf_selected_kernel say which family will run, and BF_KERNEL_UMMA turns the
-                         fall-through into BF_EUNSUPPORTED */
+  BF_KERNEL_AUTO = 0, /* pick the fastest kernel that supports the shape.  NOTE: shapes no tensor-core kernel takes -- nant
+                         not a multiple of 8 (int8) / 4 (fp16) / 16 (4+4-bit), or an nint below 16 that is no power of two
+                         (except on 32 antennas with <= 32 beams, where any EVEN nint integrates on tensor cores when
+                         nsamp / nint is a multiple of 128 or >= 512) -- fall through to BF_KERNEL_SIMT without an error,
+                         about 30x slower on the `tiny` shape; bf_kernel_name / bf_selected_kernel say which family will
+                         run, and BF_KERNEL_UMMA turns the fall-through into BF_EUNSUPPORTED.  Every nint >= 16 that
+                         divides nsamp runs on tensor cores */
   BF_KERNEL_SIMT = 1, /* generic fp32 CUDA-core kernel (any shape; Algorithm 1's structure) */
   BF_KERNEL_UMMA = 2, /* tcgen05/TMEM tensor-core kernels with the fused |.|^2 + integrate epilogue (the library
                          picks the variant) */
@@ -191,10 +190,11 @@ int bf_get_weights_noalloc(bf_ctx *ctx, int chan0, int nchan_out, float *host_ou
  * Enqueues on `stream` and returns.  BF_ENOGEOM before bf_set_geometry; BF_EINVAL for a misaligned pointer.
  *
  * Reproducibility: the result of a call depends only on its inputs -- repeated calls give bit-equal powers (tested: 50
- * launches per kernel, also with randomly delayed barrier waits) -- with ONE exception: nint a multiple of 64 above 64
- * on the fp16-operand kernels (more than 32 beams, or nant > 32) is integrated with fp32 atomic adds into powers zeroed
- * by a cudaMemsetAsync the call enqueues first; the order of those adds varies, so such results agree from run to run
- * only to fp32 rounding of the partial sums (well inside the 1e-3 bar).
+ * launches per kernel, also with randomly delayed barrier waits) -- with ONE exception: an nint that is no power of two
+ * <= 64 on the fp16-operand kernels ("umma-f16-resident" / "umma-f16-kblock": multiples of 64 above 64, and any other
+ * length >= 16) is integrated with fp32 atomic adds into powers zeroed by a cudaMemsetAsync the call enqueues first; the
+ * order of those adds varies, so such results agree from run to run only to fp32 rounding of the partial sums (well
+ * inside the 1e-3 bar).
  *
  * CUDA graphs: a bf_run on a context with ONE weight buffer enqueues only a kernel (plus that memset) and may be captured
  * into a graph once the SAME call has been made un-captured before (the first launch of a kernel variant sets function

@@ -244,6 +244,13 @@ bf_umma_k64_kernel(const BfParams p, const long long total_items, const int nG, 
             epilogue_skip(b_full + 16 + 8 * ACC, lane0);
             return;
           }
+          if constexpr (!BEAMS && NINT_T == 0) {
+            if (p.nint % 64 != 0) {   // any other bin length >= 16: running sums per lane, flushed where a bin ends
+              epilogue_tile_anynint(t_lane + ACC * TILE_T, ptr + m * mstride, (wr >> m) & 1, tt * TILE_T + slot * 64, p.nint, nbin,
+                                    b_full + 16 + 8 * ACC, lane0);
+              return;
+            }
+          }
           if constexpr (BEAMS)
             epilogue_beams_tile(t_lane + ACC * TILE_T, bptr + (size_t)m * BF_TILE_BEAMS * p.nsamp, (bok >> m) & 1, nvalid,
                                 bvec_ok, p.beam_scale, lane >= 16, b_full + 16 + 8 * ACC, lane0);
@@ -519,7 +526,10 @@ cudaError_t launch_k64_nint(const BfParams &p, int sm_count, cudaStream_t st) {
 
 }  // namespace
 
-static bool nint_ok(int I) { return (I <= 64 && (I & (I - 1)) == 0) || I % 64 == 0; }
+// bins the fp16 kernels integrate: 2^k <= 64 in registers / by shuffles (compile-time), multiples of 64 as one atomic add per
+// warp and tile, and ANY other length >= BF_LO_NINT through epilogue_tile_anynint (atomic adds where a bin ends).  Below
+// BF_LO_NINT only the powers of two exist: those kernels also contract the residual coefficient plane.
+static bool nint_ok(int I) { return (I <= 64 && (I & (I - 1)) == 0) || I >= BF_LO_NINT; }
 
 // which tensor-core kernel takes this shape: 1 = coefficients-resident (2*nant <= 64), 2 = K-blocked
 static int umma_variant(int dtype, int nant) {
@@ -540,8 +550,7 @@ bool bf_umma_supported(const bf_ctx *c, const char **why) {
   if (!bf_umma_shape_supported(c, why)) return false;
   // 33-64 beams on 32 antennas: the bin-per-lane kernel integrates any even nint >= 16 (bf_bl_shape)
   if (!nint_ok(c->nint) && !bf_bl_shape(c->dtype, BF_MODE_POWER, c->nant, c->nbeam, c->nint, c->nbin)) {
-    *why = "needs nint a power of two <= 64 or a multiple of 64 (33-64 beams on 32 antennas: any even nint >= 16 with nsamp / nint "
-           "a multiple of 256 or >= 1024)";
+    *why = "needs nint a power of two or >= 16";
     return false;
   }
   return true;
@@ -567,8 +576,8 @@ static cudaError_t launch_k64_in(const BfParams &p, int sm_count, cudaStream_t s
     case 32: return launch_k64_nint<32, IN>(p, sm_count, st);
     case 64: return launch_k64_nint<64, IN>(p, sm_count, st);
     default:
-      if (p.nint % 64 != 0) return cudaErrorNotSupported;   // bf_umma_supported lets no such shape through
-      return launch_k64_nint<0, IN>(p, sm_count, st);       // multiples of 64: atomic partial sums
+      if (p.nint < BF_LO_NINT) return cudaErrorNotSupported;   // bf_umma_supported lets no such shape through
+      return launch_k64_nint<0, IN>(p, sm_count, st);          // any other length: atomic partial sums into zeroed powers
   }
 }
 

@@ -166,6 +166,45 @@ __device__ __forceinline__ void epilogue_tile(uint32_t taddr, float *out, bool w
     }
   }
 }
+// ANY integration length (the sizes of a real observation do not divide a tile).  The warp's 64 columns are
+// the time samples t_first .. t_first + 63 of one beam row, and a bin ends after every column with (t + 1) % nint == 0.  The
+// squares of each run of columns inside one bin are summed in registers and added atomically into the ZEROED power cube
+// (`row` = first bin of this lane's beam), so a bin may straddle warps, tiles and CTAs.  Bin ends are a warp-uniform 64-bit
+// mask, so the 64 unrolled flush sites branch uniformly; one integer division per tile.  Columns past nsamp hold finite
+// garbage; nsamp % nint == 0 makes sample nsamp - 1 a bin end, so they only ever reach bins >= nbin, which are dropped.
+__device__ __forceinline__ void epilogue_tile_anynint(uint32_t taddr, float *row, bool writer, int t_first, int nint, int nbin,
+                                                      uint32_t bar_empty, bool lane0) {
+  constexpr int CPW = TILE_T / (EPI_WARPS / 4);                          // columns per warp (64)
+  constexpr int NCH = CPW / 32;
+  int bin = t_first / nint;
+  unsigned long long ends = 0;
+  for (int k = nint - 1 - (t_first - bin * nint); k < CPW; k += nint) ends |= 1ull << k;
+  float acc = 0.f;
+#pragma unroll
+  for (int ch = 0; ch < NCH; ++ch) {
+    uint32_t v[32];
+    BF_TMEM_LD_32x32b_X32(taddr + 32 * ch, v);
+    tc_wait_ld();
+    if (ch == NCH - 1) {  // all of this warp's columns are in registers: release the stage
+      tc_fence_before();
+      __syncwarp();
+      if (lane0) mbar_arrive(bar_empty);
+    }
+    const uint32_t e = (uint32_t)(ends >> (32 * ch));
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+      const float d = __uint_as_float(v[j]);
+      acc = fmaf(d, d, acc);
+      const bool end = (e >> j) & 1u;
+      if (end || (ch == NCH - 1 && j == 31)) {   // the bin ends here, or this warp's part of it does
+        const float tot = acc + __shfl_xor_sync(0xffffffffu, acc, 16);  // re^2 rows + im^2 rows
+        if (writer && bin < nbin) atomicAdd(row + bin, tot);
+        acc = 0.f;
+        if (end) ++bin;
+      }
+    }
+  }
+}
 // ---- deferred tail ----------------------------------------------------------------------------------------------
 // The epilogue warps are the critical chain of the resident kernel (profiles/: busy ~90 % of the time while every
 // other role waits), and a fifth of that chain was the tail of each tile: add tree -> SHFL -> FADD -> STG, the FADD

@@ -117,7 +117,9 @@ bf_umma_kblock_kernel(const BfParams p, const __grid_constant__ CUtensorMap tmap
           continue;
         }
         float *row = p.pow + ((size_t)it.c * p.nbeam + beam) * p.nbin;
-        if (NINT_T == 0) {
+        if (NINT_T == 0 && p.nint % 64 != 0) {   // any bin length >= 16 that is no power of two <= 64 and no multiple of 64
+          epilogue_tile_anynint(t_lane + m * TILE_T, row, writer, t_first, p.nint, p.nbin, bar_t_empty + 8 * m, lane0);
+        } else if (NINT_T == 0) {
           epilogue_tile<NINT_T>(t_lane + m * TILE_T, row + t_first / p.nint, writer, t_first < p.nsamp ? 1 : 0, false,
                                 bar_t_empty + 8 * m, lane0);
         } else {
@@ -322,7 +324,9 @@ cudaError_t launch_kb_nint(const BfParams &p, int dtype, int sm_count, cudaStrea
     case 16: return launch_kb<16, IN>(p, dtype, sm_count, st);
     case 32: return launch_kb<32, IN>(p, dtype, sm_count, st);
     case 64: return launch_kb<64, IN>(p, dtype, sm_count, st);
-    default: return launch_kb<0, IN>(p, dtype, sm_count, st);
+    default:
+      if (p.nint < BF_LO_NINT) return cudaErrorNotSupported;   // bf_umma_supported lets no such shape through
+      return launch_kb<0, IN>(p, dtype, sm_count, st);
   }
 }
 

@@ -107,7 +107,7 @@ SMALL = [
     (32, 2, 65, 768, 256, "ci8", "resident"),    # beams spill into a second M tile
     (32, 1, 130, 1024, 1024, "ci8", "resident"),  # nint = nsamp, three M tiles
     (32, 2, 16, 2048, 512, "ci8", "i8"),   # nint spans two time tiles
-    (32, 1, 5, 96, 48, "ci8", "simt"),       # nint not a power of two
+    (32, 1, 5, 96, 48, "ci8", "resident"),   # nint not a power of two: running sums flushed where a bin ends (atomics)
     (8, 2, 4, 128, 16, "ci8", "i8"),
     (16, 2, 9, 300, 4, "ci8", "i8"),
     (64, 2, 33, 512, 32, "ci8", "kblock"),
@@ -144,6 +144,18 @@ SMALL = [
     (32, 3, 33, 5120, 20, "ci4", "binlane"),    # nint = 20, 256 bins
     (32, 2, 48, 11264, 22, "ci8", "binlane"),   # nint = 22: an ODD number (11) of raw rows per bin, 512 bins
     (32, 1, 64, 34816, 34, "ci4", "binlane"),   # nint = 34 (17 rows per bin), 1024 bins
+]
+
+SMALL += [
+    # any nint >= 16 on the fp16 kernels (epilogue_tile_anynint): bins that straddle warps, tiles and CTAs
+    (32, 4, 128, 4000, 100, "ci8", "resident"),  # VERDICT r2's cliff shape: 100 = 64 + 36, ragged tail (4000 = 15*256 + 160)
+    (32, 2, 64, 900, 18, "ci8", "resident"),     # 50 bins: too few for the bin-per-lane kernel; 18 does not divide 64
+    (32, 3, 130, 1700, 17, "ci4", "resident"),   # odd nint, 4-bit unpack, three M-tiles, ragged tail
+    (32, 2, 20, 1500, 25, "ci8", "resident"),    # <= 32 beams but no int8 variant for nint 25 (60 bins)
+    (32, 1, 70, 2304, 2304, "ci8", "resident"),  # one bin per channel, 9 tiles
+    (64, 2, 70, 1536, 48, "ci8", "kblock"),      # K-blocked, int8 conversion
+    (256, 1, 100, 1000, 25, "cf16", "kblock"),   # K-blocked fp16 input, odd nint, ragged tail
+    (1024, 1, 16, 768, 96, "ci4", "kblock"),     # K-blocked 4-bit, 32 K-blocks
 ]
 
 KERNEL_NAMES = {"i8": "umma-i8", "resident": "umma-f16-resident", "kblock": "umma-f16-kblock", "binlane": "umma-f16-binlane",
