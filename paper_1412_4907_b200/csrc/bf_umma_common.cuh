@@ -180,6 +180,12 @@ __device__ __forceinline__ void epilogue_tile_anynint(uint32_t taddr, float *row
   unsigned long long ends = 0;
   for (int k = nint - 1 - (t_first - bin * nint); k < CPW; k += nint) ends |= 1ull << k;
   float acc = 0.f;
+  auto flush = [&](bool end) {   // warp-uniform call sites
+    const float tot = acc + __shfl_xor_sync(0xffffffffu, acc, 16);  // re^2 rows + im^2 rows
+    if (writer && bin < nbin) atomicAdd(row + bin, tot);
+    acc = 0.f;
+    if (end) ++bin;
+  };
 #pragma unroll
   for (int ch = 0; ch < NCH; ++ch) {
     uint32_t v[32];
@@ -190,17 +196,40 @@ __device__ __forceinline__ void epilogue_tile_anynint(uint32_t taddr, float *row
       __syncwarp();
       if (lane0) mbar_arrive(bar_empty);
     }
-    const uint32_t e = (uint32_t)(ends >> (32 * ch));
+    // Groups of 8 columns.  With nint >= 16 a group holds at most ONE bin end.  A group with none before its last column
+    // (all but one or two per tile at nint >= 64) is four packed FMAs into two independent sums; a group with an end inside
+    // is split by selects into the part up to the end and the part after it, with a single flush between them -- 16 flush
+    // sites in all, not one per column.  (Measured on a medium-sized buffer at nint 100: one dependent FMA chain with a test
+    // after every column 5.2 ms, per-column walks only in the groups with an end 3.1 ms; nint 64 at compile time 0.91 ms.)
 #pragma unroll
-    for (int j = 0; j < 32; ++j) {
-      const float d = __uint_as_float(v[j]);
-      acc = fmaf(d, d, acc);
-      const bool end = (e >> j) & 1u;
-      if (end || (ch == NCH - 1 && j == 31)) {   // the bin ends here, or this warp's part of it does
-        const float tot = acc + __shfl_xor_sync(0xffffffffu, acc, 16);  // re^2 rows + im^2 rows
-        if (writer && bin < nbin) atomicAdd(row + bin, tot);
-        acc = 0.f;
-        if (end) ++bin;
+    for (int g = 0; g < 4; ++g) {
+      const uint32_t e8 = (uint32_t)(ends >> (32 * ch + 8 * g)) & 0xffu;
+      const bool last = ch == NCH - 1 && g == 3;                      // this warp's part of a bin ends with its columns
+      if ((e8 & 0x7fu) == 0) {
+        float2 a0 = make_float2(0.f, 0.f), a1 = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const float2 d = make_float2(__uint_as_float(v[8 * g + 2 * j]), __uint_as_float(v[8 * g + 2 * j + 1]));
+          if (j & 1) a1 = ffma2(d, d, a1);
+          else a0 = ffma2(d, d, a0);
+        }
+        a0 = fadd2(a0, a1);
+        acc += a0.x + a0.y;
+        if (e8 != 0 || last) flush(e8 != 0);
+      } else {
+        const int je = __ffs((int)e8) - 1;                             // the end is after column je (0 .. 6) of the group
+        float lo = 0.f, hi = 0.f;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const float d = __uint_as_float(v[8 * g + j]);
+          const float sq = d * d;
+          lo += j <= je ? sq : 0.f;
+          hi += j <= je ? 0.f : sq;
+        }
+        acc += lo;
+        flush(true);
+        acc = hi;
+        if (last) flush(false);
       }
     }
   }
